@@ -1,0 +1,197 @@
+"""Pins for the oracle's walker (CPU only): closed forms and invariants of the random walk as a whole.
+Analytic spectra are [literature] forms (Neufeld 1990; Dijkstra et al. 2006), cited by the paper at PAPER.md:326,
+342-350 but not printed there; SURVEY.md §8(c) P4 lists them and their closed-form CDFs."""
+import math
+
+import numpy as np
+import pytest
+from scipy import special, stats
+
+from paper_2507_11603_b200 import workloads as W
+
+
+def _conserved(res, n):
+    c = res["counters"]
+    assert c["escaped"] + c["absorbed"] + c["terminated"] + c["capped"] == n          # P8
+    assert int(res["nscat_hist"].sum()) == n
+    assert int(res["spectrum"].sum()) == c["escaped"] + c["terminated"]
+    assert int(res["raw"]["nscat"].astype(np.int64).sum()) == c["scatterings"]
+
+
+# ---------------------------------------------------------------- P4: Neufeld slab, Dijkstra sphere
+def test_slab_neufeld_spectrum(oracle):
+    """Config 3 (tau0 = 1e7, T = 1e4 K, a tau0 = 4718) with x_crit core-skipping: escaped |x| against the analytic
+    CDF (4/pi) atan(tanh(k|x|^3/2)), k = sqrt(pi^3/54)/(a tau0)."""
+    n = 4000
+    w = W.static_slab(n_photons=n)
+    res = oracle.run(w["grid"], w["sources"], w["opts"], n, seed=1)
+    _conserved(res, n)
+    assert res["counters"]["escaped"] == n
+    atau = oracle.voigt_a(1e4) * 1e7
+    ax = np.abs(res["raw"]["V"].astype(float)) / oracle.vth_kms(1e4)
+    k = math.sqrt(math.pi ** 3 / 54) / atau
+    cdf = lambda x: 4 / math.pi * np.arctan(np.tanh(k * x ** 3 / 2))
+    ks = stats.kstest(ax, cdf)
+    assert ks.statistic < 0.05, ks                           # asymptotic solution: shape check
+    assert abs(np.median(ax) / atau ** (1 / 3) - 1.052) < 0.05
+    # symmetric red/blue
+    assert abs(np.mean(res["raw"]["V"] > 0) - 0.5) < 4 * 0.5 / math.sqrt(n)
+    # exit directions: only through the z faces of the slab
+    assert np.all(np.abs(res["raw"]["kz"]) > 0)
+    assert 500 < res["counters"]["scatterings"] / n < 6000   # core-skipping at work (≈2e7 without)
+
+
+def test_sphere_dijkstra_spectrum(oracle):
+    """Config 1's sphere (tau0 = 1e5, T = 10 K, a tau0 = 1492), accelerated with x_crit = 0.2 (a tau0)^(1/3):
+    escaped |x| against tanh(k|x|^3/2), k = sqrt(2 pi^3/27)/(a tau0).  The voxelised surface loosens the match."""
+    n = 3000
+    w = W.static_sphere(n_photons=n)
+    atau = oracle.voigt_a(10.0) * 1e5
+    opts = dict(w["opts"], core_skip_mode=1, x_crit=0.2 * atau ** (1 / 3))
+    res = oracle.run(w["grid"], w["sources"], opts, n, seed=1)
+    _conserved(res, n)
+    ax = np.abs(res["raw"]["V"].astype(float)) / oracle.vth_kms(10.0)
+    k = math.sqrt(2 * math.pi ** 3 / 27) / atau
+    ks = stats.kstest(ax, lambda x: np.tanh(k * x ** 3 / 2))
+    assert ks.statistic < 0.06, ks
+    assert abs(np.median(ax) / atau ** (1 / 3) - 0.898) < 0.06
+    # isotropic emergent directions from a sphere
+    assert abs(res["raw"]["kz"].mean()) < 4 / math.sqrt(3 * n)
+
+
+# ---------------------------------------------------------------- P7: optically thin limits
+def test_slab_unscattered_fraction_E2(oracle):
+    """Line-centre source in the midplane of a static slab: P(N_scat = 0) = E_2(tau0 H(a,0)) exactly."""
+    n = 40000
+    for tau0 in (0.3, 2.0):
+        w = W.static_slab(nz=16, tau0=tau0, T=1e4, core_skip=False, n_photons=n)
+        res = oracle.run(w["grid"], w["sources"], w["opts"], n, seed=3)
+        _conserved(res, n)
+        # the recipe's sigma0 literal fixes the density; the oracle's own sigma0 decides the realised tau0
+        tau_real = tau0 * oracle.sigma0_cm2(1e4) / W.RECIPE_SIGMA0_T4
+        p = special.expn(2, tau_real * oracle.voigt_H(oracle.voigt_a(1e4), 0.0).item())
+        got = res["nscat_hist"][0] / n
+        assert abs(got - p) < 4.5 * math.sqrt(p * (1 - p) / n), (tau0, got, p)
+
+
+def test_thin_limit_returns_source_spectrum(oracle):
+    """tau0 -> 0: nothing scatters and the escaped spectrum is the source's Gaussian line, in the lab frame."""
+    n = 20000
+    w = W.expanding_shell(n=16, N_HI=1e3, tau_d=0.0, sigma_src=50.0, n_photons=n, bins=60, v_range=300.0)
+    w["grid"]["kdust"] = None
+    res = oracle.run(w["grid"], w["sources"], w["opts"], n, seed=2)
+    _conserved(res, n)
+    assert res["counters"]["scatterings"] == 0 and res["counters"]["escaped"] == n
+    V = res["raw"]["V"].astype(float)
+    assert stats.kstest(V, stats.norm(0, 50.0).cdf).pvalue > 1e-3
+    # spectrum bins are the histogram of dv = -V
+    edges = np.linspace(-300, 300, 61)
+    ref, _ = np.histogram(-V, edges)
+    assert np.abs(res["spectrum"][:60].astype(int) - ref).sum() <= 2      # fp32 storage of V at bin edges
+    # isotropic emission
+    assert abs(res["raw"]["kz"].mean()) < 4 / math.sqrt(3 * n)
+    assert abs((res["raw"]["kz"] ** 2).mean() - 1 / 3) < 0.01
+
+
+# ---------------------------------------------------------------- P6: dust
+def test_dust_only_cube_escape_fraction(oracle):
+    """No gas, uniform absorbing dust in an n^3 cube, central source: f_esc = <exp(-kappa d(k))> over isotropic
+    directions with d the centre-to-face distance (n/2)/max|k_i| — evaluated here by quadrature on the sphere."""
+    n_cells, n = 8, 40000
+    w = W.static_sphere(n=n_cells, tau0=0.0, n_photons=n)
+    tau_half = 1.3                                              # optical depth over n/2 cells
+    w["grid"]["kdust"] = np.full((n_cells,) * 3, tau_half / (n_cells / 2 * w["grid"]["cell_cm"]), np.float32)
+    res = oracle.run(w["grid"], w["sources"], w["opts"], n, seed=4)
+    _conserved(res, n)
+    mu = np.linspace(-1, 1, 2001)[:, None]
+    ph = np.linspace(0, 2 * math.pi, 2001)[None, :]
+    st = np.sqrt(1 - mu ** 2)
+    m = np.maximum(np.maximum(np.abs(st * np.cos(ph)), np.abs(st * np.sin(ph))), np.abs(mu))
+    f = np.exp(-tau_half / m)
+    fesc = np.trapezoid(np.trapezoid(f, ph[0], axis=1), mu[:, 0]) / (4 * math.pi)
+    got = res["counters"]["escaped"] / n
+    assert abs(got - fesc) < 4.5 * math.sqrt(fesc * (1 - fesc) / n), (got, fesc)
+    assert res["counters"]["scatterings"] == 0
+
+
+def test_interaction_kind_probability(oracle):
+    """interaction i occurs with probability tau_i / tau.  Line-centre packets in a uniform static
+    slab with gas + dust: of the packets whose FIRST event happens, a fraction kappa_d/(kappa_d + kappa_line(x=0))
+    is absorbed with N_scat = 0."""
+    n = 40000
+    tau0, tau_d = 3.0, 1.5
+    w = W.static_slab(nz=16, tau0=tau0, T=1e4, core_skip=False, n_photons=n, tau_d=tau_d)
+    res = oracle.run(w["grid"], w["sources"], w["opts"], n, seed=6)
+    _conserved(res, n)
+    raw = res["raw"]
+    first_abs = np.sum((raw["status"] == 1) & (raw["nscat"] == 0))
+    no_event = np.sum((raw["status"] == 0) & (raw["nscat"] == 0))
+    interacted = n - no_event
+    tau_line = tau0 * oracle.sigma0_cm2(1e4) / W.RECIPE_SIGMA0_T4 * oracle.voigt_H(oracle.voigt_a(1e4), 0.0).item()
+    p = tau_d / (tau_d + tau_line)
+    assert abs(first_abs / interacted - p) < 4.5 * math.sqrt(p * (1 - p) / interacted)
+    # and the unscattered, unabsorbed fraction is E2 of the total depth
+    pe = special.expn(2, tau_line + tau_d)
+    assert abs(no_event / n - pe) < 4.5 * math.sqrt(pe * (1 - pe) / n)
+
+
+# ---------------------------------------------------------------- P14: core-skipping leaves the spectrum unchanged
+def test_core_skipping_invariance(oracle):
+    n = 2500
+    w = W.static_slab(nz=32, tau0=3000.0, T=10.0, core_skip=False, n_photons=n)
+    full = oracle.run(w["grid"], w["sources"], w["opts"], n, seed=8)
+    atau = oracle.voigt_a(10.0) * 3000.0
+    skip = oracle.run(w["grid"], w["sources"], dict(w["opts"], core_skip_mode=1, x_crit=0.2 * atau ** (1 / 3)), n, seed=9)
+    _conserved(full, n)
+    _conserved(skip, n)
+    xf = np.abs(full["raw"]["V"].astype(float))
+    xs = np.abs(skip["raw"]["V"].astype(float))
+    assert stats.ks_2samp(xf, xs).pvalue > 1e-3
+    assert skip["counters"]["scatterings"] < 0.9 * full["counters"]["scatterings"]
+
+
+# ---------------------------------------------------------------- frames: bulk motion and Hubble drift
+def test_galilean_invariance_of_bulk_motion(oracle):
+    """A medium moving uniformly with velocity v gives the static spectrum shifted by v.k_exit (Eq. 4's gas-frame
+    evaluation; emission in the gas frame)."""
+    n = 3000
+    w0 = W.static_slab(nz=16, tau0=300.0, T=1e4, core_skip=False, n_photons=n)
+    w1 = W.static_slab(nz=16, tau0=300.0, T=1e4, core_skip=False, n_photons=n)
+    v = np.array([30.0, -80.0, 120.0])
+    for ax, name in enumerate(("vx", "vy", "vz")):
+        w1["grid"][name][:] = v[ax]
+    r0 = oracle.run(w0["grid"], w0["sources"], w0["opts"], n, seed=1)
+    r1 = oracle.run(w1["grid"], w1["sources"], w1["opts"], n, seed=1)
+    k1 = np.stack([r1["raw"]["kx"], r1["raw"]["ky"], r1["raw"]["kz"]], 1).astype(float)
+    # same seed, same arithmetic in the gas frame: identical trajectories up to rounding of (V - v.k)
+    assert np.mean(r0["raw"]["nscat"] == r1["raw"]["nscat"]) > 0.9
+    same = r0["raw"]["nscat"] == r1["raw"]["nscat"]
+    resid = r1["raw"]["V"].astype(float) - k1 @ v - r0["raw"]["V"].astype(float)
+    assert np.median(np.abs(resid[same])) < 1e-3
+    assert stats.ks_2samp(r1["raw"]["V"].astype(float) - k1 @ v, r0["raw"]["V"].astype(float)).pvalue > 1e-3
+
+
+def test_hubble_drift_gunn_peterson(oracle):
+    """Uniform static gas with a pure Hubble drift Hc (km/s per cell length): a packet redshifting through the whole
+    line sees tau_GP = n sigma0 dl (v_th/Hc) Int H dx = n sigma0 dl (v_th/Hc) sqrt(pi), whatever its direction.
+    Packets born AT line centre see the red half, Int_0^inf H dx = sqrt(pi)/2:  P(N_scat = 0) = exp(-tau_GP/2).
+    Pins the sub-cell stepping (reading A12) and the sign of the drift."""
+    n = 20000
+    T, Hc = 1e4, 2.0
+    vth = oracle.vth_kms(T)
+    w = W.static_slab(nz=512, tau0=1.0, T=T, core_skip=False, n_photons=n)
+    tau_gp = 0.8
+    cell_tau0 = tau_gp * Hc / (vth * math.sqrt(math.pi))               # n sigma0 dl per cell at line centre
+    w["grid"]["nHI"][:] = cell_tau0 / (oracle.sigma0_cm2(T) * w["grid"]["cell_cm"])
+    opts = dict(w["opts"], hubble_kms_per_cell=Hc, hubble_eps=0.25, v_max_kms=10.0 * vth)
+    res = oracle.run(w["grid"], w["sources"], opts, n, seed=5)
+    _conserved(res, n)
+    p = math.exp(-tau_gp / 2)
+    got = res["nscat_hist"][0] / n
+    assert abs(got - p) < 4.5 * math.sqrt(p * (1 - p) / n), (got, p)
+    # unscattered packets are terminated at |V| = v_max having only ever redshifted
+    un = res["raw"][res["raw"]["nscat"] == 0]
+    assert np.all(un["V"] < -10.0 * vth + 1e-3) and np.all(un["status"] == 2)
+    # halving eps changes nothing within noise (the midpoint rule has converged)
+    res2 = oracle.run(w["grid"], w["sources"], dict(opts, hubble_eps=0.05), n, seed=5)
+    assert abs(res2["nscat_hist"][0] / n - p) < 4.5 * math.sqrt(p * (1 - p) / n)
