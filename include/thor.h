@@ -1,0 +1,158 @@
+/* thor.h — C-ABI of the B200-native hot path of THOR (arXiv 2507.11603): the Monte Carlo resonant-scattering random
+ * walk of Lyα photon packets through a 3D Cartesian gas grid (§3.4, Fig. 1).
+ *
+ * Implemented by libthor_b200.so (paper_2507_11603_b200/csrc, CUDA, sm_100a only).  Every step of the path runs in
+ * CUDA kernels; there is no CPU fallback.  Nothing here throws or aborts: every call returns a thor_status and the
+ * reason is available from thor_last_error().  "DEVICE" / "HOST" say where a pointer must live.
+ *
+ * Entry points of the path (BASELINE.json north_star): thor_grid_create, thor_sources_set, thor_run, thor_tally_get.
+ * The thor_unit_* calls run single steps of the path (RNG, DDA, Voigt, samplers) in isolation for parity tests.
+ */
+#ifndef THOR_B200_H
+#define THOR_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct thor_ctx thor_ctx; /* opaque; one per grid; not thread-safe */
+
+typedef enum {
+    THOR_OK = 0,
+    THOR_ERR_ARG = 1,         /* bad argument (NULL, size, NaN/negative field, source outside grid, ...) */
+    THOR_ERR_STATE = 2,       /* call order (run before sources_set, tally not produced by the last run, ...) */
+    THOR_ERR_OOM = 3,         /* device or host allocation failed */
+    THOR_ERR_CUDA = 4,        /* a CUDA runtime call or kernel failed; text in thor_last_error */
+    THOR_ERR_UNSUPPORTED = 5  /* no CUDA device / device is not sm_100 */
+} thor_status;
+
+/* ---- grid flags ---- */
+#define THOR_GRID_BORROW 0x0u     /* default: field arrays are DEVICE pointers the caller keeps alive and unmodified
+                                     until thor_grid_destroy; nothing is copied (the 72 GB grid of config 5) */
+#define THOR_GRID_HOST 0x1u       /* field arrays are HOST pointers; the library copies them to the device */
+#define THOR_PERIODIC_X 0x10u
+#define THOR_PERIODIC_Y 0x20u
+#define THOR_PERIODIC_Z 0x40u
+#define THOR_GRID_NO_VALIDATE 0x100u /* skip the device-side scan for NaN / negative fields */
+
+/* The dataset (uniform Cartesian grid, fields constant per cell).  Six SoA fp32 arrays, dense
+ * row-major [nz][ny][nx] (x fastest): nHI [cm^-3], T [K], vx, vy, vz [km/s], and kdust [cm^-1], the dust ABSORPTION
+ * coefficient (NULL = no dust; reading A21).  cell_cm = cell edge in cm.  A periodic axis of extent 1 is
+ * treated as infinite (DDA).  stream = cudaStream_t as void* (NULL = default stream); all later work
+ * of this context is issued on it.  Errors: THOR_ERR_ARG for n<=0, NULL arrays, cell_cm<=0, n>0 with T<=0 or any
+ * NaN (reading A19); THOR_ERR_UNSUPPORTED without a CUDA sm_100 device. */
+thor_status thor_grid_create(thor_ctx **out, int nx, int ny, int nz, double cell_cm,
+                             const float *nHI, const float *T, const float *vx, const float *vy, const float *vz,
+                             const float *kdust, unsigned flags, void *stream);
+void thor_grid_destroy(thor_ctx *ctx);
+
+/* The generator: a list of point sources.  HOST arrays, copied: pos_xyz [n_src][3] in cell units
+ * (grid spans [0,nx) x [0,ny) x [0,nz)), lum [n_src] >= 0 relative luminosities (a packet picks source j with
+ * probability lum_j / sum, reading A18), sigma_kms [n_src] Gaussian line width in the source cell's gas frame
+ * (0 = line centre, reading A10).  Replaces any earlier list.  THOR_ERR_ARG if a source lies outside the grid,
+ * a luminosity is negative/NaN, or the total is zero. */
+thor_status thor_sources_set(thor_ctx *ctx, long long n_src, const float *pos_xyz, const float *lum,
+                             const float *sigma_kms);
+
+/* phase functions */
+#define THOR_PHASE_ISOTROPIC 0
+#define THOR_PHASE_DIPOLE 1
+#define THOR_PHASE_MIX 2 /* 1/3 isotropic + 2/3 dipole */
+
+/* Run options.  Set struct_size = sizeof(thor_opts); use thor_opts_default() for the defaults. */
+typedef struct thor_opts {
+    uint32_t struct_size;
+    int32_t phase_core, phase_wing;   /* THOR_PHASE_*; default isotropic / isotropic */
+    int32_t phase_frame;              /* 0: split on atom-frame |x_in - u_par| (default), 1: gas-frame |x_in| (A3) */
+    double phase_split_x;             /* 0.2 */
+    int32_t core_skip_mode;           /* 0 off, 1 global x_crit, 2 local per cell (reading A7) */
+    double x_crit;
+    int32_t spec_mode;                /* escape spectrum axis: 0: x = V / v_th(spec_T_ref); 1: dv = -V km/s (A14) */
+    double spec_T_ref;
+    int32_t spec_bins;                /* 0 = no spectrum; <= 4096 */
+    double spec_lo, spec_hi;
+    double hubble_kms_per_cell;       /* frequency drift per cell length travelled (A12, A15); 0 = off */
+    double hubble_eps;                /* sub-step size in units of v_th (0.25) */
+    double v_max_kms;                 /* stop when |V| exceeds this; 0 = off */
+    int32_t peel_on;                  /* peel-off toward k_obs at emission and at every scattering */
+    double k_obs[3];
+    int32_t peel_nx, peel_ny, peel_nv;/* image pixels and spectral bins of the IFU cube [ny][nx][nv] */
+    double peel_v_lo, peel_v_hi;      /* spectral axis dv = -V (km/s) at the box face */
+    double peel_width_cells;          /* image side in cell units, centred on the grid centre */
+    double tau_peel_max;              /* peel rays are dropped beyond this optical depth (30; A13) */
+    uint64_t photon_id_offset;        /* the run covers photon ids [offset, offset + n_photons) */
+    uint64_t max_scatter;             /* safety cap per packet (0 = none); capped packets are counted, not tallied */
+    int32_t raw_output;               /* keep one thor_raw_record per packet (THOR_TALLY_RAW) */
+    int32_t accumulate;               /* do not zero the tallies before this run */
+} thor_opts;
+
+void thor_opts_default(thor_opts *o);
+
+/* Walks photon ids [photon_id_offset, +n_photons) under `seed` (Philox4x32-10 keyed on (seed, photon id, draw
+ * index), reading A16): emit, draw tau = -ln u, DDA march with Voigt optical depth in each cell's gas frame, scatter
+ * (u_par by rejection from Eq. 6, u_perp Gaussian, phase function, Eq. 7), until escape / dust absorption, tallying
+ * into the context's spectrum / cube / counters.  One persistent kernel launch; synchronous: returns after the
+ * stream has drained.  opts == NULL -> defaults.  Errors: THOR_ERR_STATE without sources; THOR_ERR_ARG for
+ * inconsistent opts; THOR_ERR_OOM if tallies cannot be allocated; THOR_ERR_CUDA. */
+thor_status thor_run(thor_ctx *ctx, unsigned long long n_photons, unsigned long long seed, const thor_opts *opts);
+
+/* Duration of the walk kernel of the last thor_run in milliseconds, from CUDA events on the context's stream. */
+thor_status thor_last_run_ms(const thor_ctx *ctx, float *ms);
+
+/* tallies */
+#define THOR_TALLY_SPECTRUM 0   /* uint64[spec_bins + 2]: bins, then underflow, overflow */
+#define THOR_TALLY_NSCAT_HIST 1 /* uint64[64]: bin 0: nscat = 0; bin b: 2^(b-1) <= nscat < 2^b */
+#define THOR_TALLY_COUNTERS 2   /* uint64[THOR_N_COUNTERS] */
+#define THOR_TALLY_CUBE 3       /* double[peel_ny][peel_nx][peel_nv] (kept as 2^-32 fixed point on the device) */
+#define THOR_TALLY_RAW 4        /* thor_raw_record[n_photons] of the last run */
+#define THOR_TALLY_DEVICE_DST 0x100 /* OR into kind: dst is a DEVICE pointer (CUBE then yields uint64 fixed point) */
+
+enum { THOR_CT_ESCAPED = 0, THOR_CT_ABSORBED, THOR_CT_TERMINATED, THOR_CT_CAPPED, THOR_CT_SCATTERINGS,
+       THOR_CT_CROSSINGS, THOR_CT_REJ_ITERS, THOR_CT_PEEL_RAYS, THOR_CT_PEEL_CELLS, THOR_N_COUNTERS };
+
+typedef struct thor_raw_record {
+    float V;          /* lab-frame velocity offset from line centre at the end, km/s */
+    uint32_t nscat;   /* saturates at 2^32-1 */
+    int32_t status;   /* THOR_CT_ESCAPED .. THOR_CT_CAPPED */
+    float kx, ky, kz; /* final direction */
+} thor_raw_record;
+
+/* Copies tally `kind` into dst (HOST unless THOR_TALLY_DEVICE_DST).  *needed (may be NULL) receives the size in
+ * bytes; THOR_ERR_ARG if dst_bytes is smaller (nothing is written); dst == NULL just queries the size.
+ * THOR_ERR_STATE if the last run did not produce that tally. */
+thor_status thor_tally_get(thor_ctx *ctx, int kind, void *dst, size_t dst_bytes, size_t *needed);
+
+/* Static-lifetime or context-owned text of the last error (ctx may be NULL for create-time errors). */
+const char *thor_last_error(const thor_ctx *ctx);
+
+/* ---- single steps of the path, for parity tests and micro-benchmarks.  All arrays are DEVICE pointers; `stream`
+ * as above.  Each call launches one kernel and synchronises. ---- */
+
+/* a1 RNG: out[i*n_draws + d] = draw d of photon (id0 + i) under seed — Philox4x32-10, counter = (d>>2 lo, d>>2 hi,
+ * id lo, id hi), key = (seed lo, seed hi), word d&3 (reading A16; cuRAND's curand_init(seed, id, 0) layout). */
+thor_status thor_unit_philox(uint64_t seed, uint64_t id0, long long n_ids, int n_draws, uint32_t *out, void *stream);
+
+/* a4 DDA: traces n rays (org, dir: float[n][3], cell units) through an (nx,ny,nz) grid with `periodic_flags`
+ * (THOR_PERIODIC_*), at most max_steps cells each.  Per ray: hash_idx = word-wise FNV-1a (offset 0xCBF29CE484222325,
+ * prime 0x100000001B3, h = (h ^ w) * prime) over the 64-bit linear indices of the visited cells, hash_len = the same
+ * over the fp32 bit patterns of the segment lengths, count = cells visited.  If seq_idx/seq_len are non-NULL (n must
+ * be 1) the visited indices / lengths are written there (max_steps entries). */
+thor_status thor_unit_dda_trace(int nx, int ny, int nz, unsigned periodic_flags, long long n, const float *org,
+                                const float *dir, long long max_steps, uint64_t *hash_idx, uint64_t *hash_len,
+                                uint32_t *count, int64_t *seq_idx, float *seq_len, void *stream);
+
+/* a6 Voigt: out[i] = H(a[i], x[i]) (normalisation of Eq. 6). */
+thor_status thor_unit_voigt(long long n, const float *a, const float *x, float *out, void *stream);
+
+/* a8-a11: n independent scatterings at gas-frame x_in with Voigt parameter a, incoming direction +z, photon stream
+ * (seed, id0 + i): writes u_par[n], x_out[n], k_out[n][3], iters[n] (rejection iterations).  Any output may be NULL. */
+thor_status thor_unit_scatter(float a, float x_in, float x_crit, int phase, uint64_t seed, uint64_t id0, long long n,
+                              float *u_par, float *x_out, float *k_out, uint32_t *iters, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* THOR_B200_H */

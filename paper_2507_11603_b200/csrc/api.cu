@@ -1,0 +1,359 @@
+// C-ABI of include/thor.h: context, argument validation, tally storage, kernel launches.  Host logic only; every
+// step of the path runs in the kernels of walk.cu / unit_kernels.cu.
+#include <cuda_runtime.h>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/thor.h"
+#include "params.cuh"
+
+namespace thor {
+cudaError_t launch_walk(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out);
+cudaError_t launch_validate_fields(const float* nHI, const float* T, const float* vx, const float* vy, const float* vz,
+                                   const float* kdust, long long n, unsigned* d_flags, cudaStream_t stream);
+}  // namespace thor
+
+struct thor_ctx {
+    cudaStream_t stream = nullptr;
+    int device = 0, n_sm = 0;
+    thor::GridDims g{};
+    double cell_cm = 0;
+    long long n_cells = 0;
+    const float* f[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // nHI, T, vx, vy, vz, kdust
+    float* owned[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    // sources
+    long long n_src = 0;
+    float* d_src_pos = nullptr;
+    float* d_src_sigma = nullptr;
+    double* d_src_cdf = nullptr;
+    // tallies
+    unsigned long long* d_small = nullptr;      // [1 next_photon][N_COUNTERS][64 hist][4098 spectrum]
+    unsigned long long* d_cube = nullptr;
+    size_t cube_elems = 0;
+    thor::RawRecord* d_raw = nullptr;
+    size_t raw_cap = 0;
+    // last run
+    bool have_run = false;
+    thor_opts last{};
+    unsigned long long last_n = 0;
+    float last_ms = 0.f;
+    int last_blocks = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    std::string err;
+};
+
+static thread_local std::string g_err;
+
+static constexpr size_t SMALL_NEXT = 0, SMALL_COUNTERS = 1, SMALL_HIST = SMALL_COUNTERS + thor::N_COUNTERS,
+                        SMALL_SPEC = SMALL_HIST + 64, SMALL_TOTAL = SMALL_SPEC + 4096 + 2;
+
+static thor_status fail(thor_ctx* c, thor_status s, const std::string& msg) {
+    if (c) c->err = msg;
+    g_err = msg;
+    return s;
+}
+
+static thor_status cuda_fail(thor_ctx* c, cudaError_t e, const char* what) {
+    return fail(c, e == cudaErrorMemoryAllocation ? THOR_ERR_OOM : THOR_ERR_CUDA,
+                std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define CU(call)                                                   \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);   \
+    } while (0)
+
+extern "C" const char* thor_last_error(const thor_ctx* ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }
+
+extern "C" void thor_opts_default(thor_opts* o) {
+    if (!o) return;
+    std::memset(o, 0, sizeof *o);
+    o->struct_size = (uint32_t)sizeof *o;
+    o->phase_split_x = 0.2;
+    o->spec_T_ref = 1e4;
+    o->spec_hi = 1.0;
+    o->hubble_eps = 0.25;
+    o->k_obs[2] = 1.0;
+    o->peel_v_hi = 1.0;
+    o->tau_peel_max = 30.0;
+}
+
+extern "C" void thor_grid_destroy(thor_ctx* ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    for (float* p : ctx->owned) if (p) cudaFree(p);
+    if (ctx->d_src_pos) cudaFree(ctx->d_src_pos);
+    if (ctx->d_src_sigma) cudaFree(ctx->d_src_sigma);
+    if (ctx->d_src_cdf) cudaFree(ctx->d_src_cdf);
+    if (ctx->d_small) cudaFree(ctx->d_small);
+    if (ctx->d_cube) cudaFree(ctx->d_cube);
+    if (ctx->d_raw) cudaFree(ctx->d_raw);
+    if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+    if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+    delete ctx;
+}
+
+extern "C" thor_status thor_grid_create(thor_ctx** out, int nx, int ny, int nz, double cell_cm, const float* nHI,
+                                        const float* T, const float* vx, const float* vy, const float* vz,
+                                        const float* kdust, unsigned flags, void* stream) {
+    if (!out) return fail(nullptr, THOR_ERR_ARG, "thor_grid_create: out is NULL");
+    *out = nullptr;
+    if (nx <= 0 || ny <= 0 || nz <= 0) return fail(nullptr, THOR_ERR_ARG, "thor_grid_create: grid extents must be > 0");
+    if (!(cell_cm > 0) || !std::isfinite(cell_cm)) return fail(nullptr, THOR_ERR_ARG, "thor_grid_create: cell_cm must be > 0");
+    if (!nHI || !T || !vx || !vy || !vz) return fail(nullptr, THOR_ERR_ARG, "thor_grid_create: a field array is NULL");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, THOR_ERR_UNSUPPORTED, "thor_grid_create: no CUDA device (this library has no CPU fallback)");
+    }
+    thor_ctx* ctx = new (std::nothrow) thor_ctx;
+    if (!ctx) return fail(nullptr, THOR_ERR_OOM, "thor_grid_create: host allocation failed");
+    struct Guard { thor_ctx* c; ~Guard() { if (c) thor_grid_destroy(c); } } guard{ctx};
+    CU(cudaGetDevice(&ctx->device));
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, ctx->device));
+    if (prop.major != 10) {
+        return fail(nullptr, THOR_ERR_UNSUPPORTED,
+                    std::string("thor_grid_create: device '") + prop.name + "' is not sm_100 (built for sm_100a only)");
+    }
+    ctx->n_sm = prop.multiProcessorCount;
+    ctx->stream = (cudaStream_t)stream;
+    ctx->g.nx = nx; ctx->g.ny = ny; ctx->g.nz = nz;
+    ctx->g.periodic = ((flags & THOR_PERIODIC_X) ? 1u : 0u) | ((flags & THOR_PERIODIC_Y) ? 2u : 0u) |
+                      ((flags & THOR_PERIODIC_Z) ? 4u : 0u);
+    ctx->g.frozen = ((ctx->g.periodic & 1u) && nx == 1 ? 1u : 0u) | ((ctx->g.periodic & 2u) && ny == 1 ? 2u : 0u) |
+                    ((ctx->g.periodic & 4u) && nz == 1 ? 4u : 0u);
+    ctx->cell_cm = cell_cm;
+    ctx->n_cells = (long long)nx * ny * nz;
+    const float* src[6] = {nHI, T, vx, vy, vz, kdust};
+    const size_t bytes = (size_t)ctx->n_cells * sizeof(float);
+    for (int i = 0; i < 6; ++i) {
+        if (!src[i]) continue;
+        if (flags & THOR_GRID_HOST) {
+            CU(cudaMalloc(&ctx->owned[i], bytes));
+            CU(cudaMemcpyAsync(ctx->owned[i], src[i], bytes, cudaMemcpyHostToDevice, ctx->stream));
+            ctx->f[i] = ctx->owned[i];
+        } else {
+            cudaPointerAttributes at;
+            if (cudaPointerGetAttributes(&at, src[i]) != cudaSuccess ||
+                (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)) {
+                cudaGetLastError();
+                return fail(nullptr, THOR_ERR_ARG, "thor_grid_create: field array is not a device pointer (pass THOR_GRID_HOST for host arrays)");
+            }
+            ctx->f[i] = src[i];
+        }
+    }
+    CU(cudaMalloc(&ctx->d_small, SMALL_TOTAL * sizeof(unsigned long long)));
+    CU(cudaEventCreate(&ctx->ev0));
+    CU(cudaEventCreate(&ctx->ev1));
+    if (!(flags & THOR_GRID_NO_VALIDATE)) {
+        // reading A19: NaN anywhere, negative n or kdust, or T <= 0 where n > 0 -> THOR_ERR_ARG
+        unsigned* d_flags = reinterpret_cast<unsigned*>(ctx->d_small);
+        CU(cudaMemsetAsync(d_flags, 0, sizeof(unsigned), ctx->stream));
+        CU(thor::launch_validate_fields(ctx->f[0], ctx->f[1], ctx->f[2], ctx->f[3], ctx->f[4], ctx->f[5], ctx->n_cells,
+                                        d_flags, ctx->stream));
+        unsigned h_flags = 0;
+        CU(cudaMemcpyAsync(&h_flags, d_flags, sizeof h_flags, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        if (h_flags) {
+            std::string m = "thor_grid_create: invalid field values:";
+            if (h_flags & 1u) m += " NaN/Inf";
+            if (h_flags & 2u) m += " negative nHI or kdust";
+            if (h_flags & 4u) m += " T <= 0 in a cell with nHI > 0";
+            return fail(nullptr, THOR_ERR_ARG, m);
+        }
+    } else {
+        CU(cudaStreamSynchronize(ctx->stream));
+    }
+    guard.c = nullptr;
+    *out = ctx;
+    return THOR_OK;
+}
+
+extern "C" thor_status thor_sources_set(thor_ctx* ctx, long long n_src, const float* pos_xyz, const float* lum,
+                                        const float* sigma_kms) {
+    if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_sources_set: ctx is NULL");
+    if (n_src <= 0 || !pos_xyz || !lum || !sigma_kms) return fail(ctx, THOR_ERR_ARG, "thor_sources_set: empty or NULL source list");
+    const int n[3] = {ctx->g.nx, ctx->g.ny, ctx->g.nz};
+    std::vector<double> cdf((size_t)n_src);
+    double tot = 0;
+    for (long long i = 0; i < n_src; ++i) {
+        for (int ax = 0; ax < 3; ++ax) {
+            const float p = pos_xyz[3 * i + ax];
+            if (!(p >= 0.f && p <= (float)n[ax])) return fail(ctx, THOR_ERR_ARG, "thor_sources_set: source " + std::to_string(i) + " lies outside the grid");
+        }
+        if (!(lum[i] >= 0.f) || !std::isfinite(lum[i])) return fail(ctx, THOR_ERR_ARG, "thor_sources_set: luminosity " + std::to_string(i) + " is negative or not finite");
+        if (!(sigma_kms[i] >= 0.f) || !std::isfinite(sigma_kms[i])) return fail(ctx, THOR_ERR_ARG, "thor_sources_set: sigma " + std::to_string(i) + " is negative or not finite");
+        tot += lum[i];
+    }
+    if (!(tot > 0)) return fail(ctx, THOR_ERR_ARG, "thor_sources_set: total luminosity is zero");
+    double acc = 0;
+    for (long long i = 0; i < n_src; ++i) { acc += lum[i]; cdf[(size_t)i] = acc / tot; }
+    cdf[(size_t)n_src - 1] = 1.0;
+    CU(cudaSetDevice(ctx->device));
+    if (ctx->d_src_pos) { cudaFree(ctx->d_src_pos); ctx->d_src_pos = nullptr; }
+    if (ctx->d_src_sigma) { cudaFree(ctx->d_src_sigma); ctx->d_src_sigma = nullptr; }
+    if (ctx->d_src_cdf) { cudaFree(ctx->d_src_cdf); ctx->d_src_cdf = nullptr; }
+    ctx->n_src = 0;
+    CU(cudaMalloc(&ctx->d_src_pos, (size_t)n_src * 3 * sizeof(float)));
+    CU(cudaMalloc(&ctx->d_src_sigma, (size_t)n_src * sizeof(float)));
+    CU(cudaMalloc(&ctx->d_src_cdf, (size_t)n_src * sizeof(double)));
+    CU(cudaMemcpyAsync(ctx->d_src_pos, pos_xyz, (size_t)n_src * 3 * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->d_src_sigma, sigma_kms, (size_t)n_src * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->d_src_cdf, cdf.data(), (size_t)n_src * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->n_src = n_src;
+    return THOR_OK;
+}
+
+static bool phase_ok(int p) { return p == THOR_PHASE_ISOTROPIC || p == THOR_PHASE_DIPOLE || p == THOR_PHASE_MIX; }
+
+extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, unsigned long long seed,
+                                const thor_opts* opts) {
+    if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_run: ctx is NULL");
+    if (ctx->n_src <= 0) return fail(ctx, THOR_ERR_STATE, "thor_run: call thor_sources_set first");
+    thor_opts o;
+    thor_opts_default(&o);
+    if (opts) {
+        if (opts->struct_size == 0 || opts->struct_size > sizeof o) return fail(ctx, THOR_ERR_ARG, "thor_run: opts->struct_size is not set (use thor_opts_default)");
+        std::memcpy(&o, opts, opts->struct_size);
+        o.struct_size = (uint32_t)sizeof o;
+    }
+    if (!phase_ok(o.phase_core) || !phase_ok(o.phase_wing)) return fail(ctx, THOR_ERR_ARG, "thor_run: unknown phase function");
+    if (o.core_skip_mode < 0 || o.core_skip_mode > 2 || !(o.x_crit >= 0)) return fail(ctx, THOR_ERR_ARG, "thor_run: bad core-skip options");
+    if (o.spec_bins < 0 || o.spec_bins > 4096) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_bins must be in [0, 4096]");
+    if (o.spec_bins > 0 && !(o.spec_hi > o.spec_lo)) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_hi must exceed spec_lo");
+    if (o.spec_mode != 0 && o.spec_mode != 1) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_mode must be 0 or 1");
+    if (o.spec_mode == 0 && !(o.spec_T_ref > 0)) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_T_ref must be > 0");
+    if (!(o.hubble_eps > 0) || !(o.v_max_kms >= 0) || !std::isfinite(o.hubble_kms_per_cell)) return fail(ctx, THOR_ERR_ARG, "thor_run: bad Hubble / v_max options");
+    const thor::LyaConstants K = thor::lya_constants();
+    thor::WalkParams p{};
+    p.g = ctx->g;
+    p.nHI = ctx->f[0]; p.T = ctx->f[1]; p.vx = ctx->f[2]; p.vy = ctx->f[3]; p.vz = ctx->f[4]; p.kdust = ctx->f[5];
+    p.sig_cell = (float)(K.c_sig * ctx->cell_cm);
+    p.c_a = (float)K.c_a; p.c_vth = (float)K.c_vth; p.inv_c_vth = (float)(1.0 / K.c_vth);
+    p.cell_cm = (float)ctx->cell_cm;
+    p.n_src = ctx->n_src; p.src_pos = ctx->d_src_pos; p.src_sigma = ctx->d_src_sigma; p.src_cdf = ctx->d_src_cdf;
+    p.phase_core = o.phase_core; p.phase_wing = o.phase_wing; p.phase_frame = o.phase_frame;
+    p.phase_split_x = (float)o.phase_split_x;
+    p.core_skip_mode = o.core_skip_mode; p.x_crit = (float)o.x_crit;
+    p.spec_mode = o.spec_mode; p.spec_bins = o.spec_bins;
+    p.spec_inv_vth_ref = (float)(1.0 / (K.c_vth * std::sqrt(o.spec_T_ref)));
+    p.spec_lo = (float)o.spec_lo;
+    p.spec_inv_width = o.spec_bins > 0 ? (float)(o.spec_bins / (o.spec_hi - o.spec_lo)) : 0.f;
+    p.hubble = (float)o.hubble_kms_per_cell; p.hubble_eps = (float)o.hubble_eps; p.v_max = (float)o.v_max_kms;
+    p.peel_on = o.peel_on ? 1 : 0;
+    size_t cube_elems = 0;
+    if (p.peel_on) {
+        if (o.peel_nx <= 0 || o.peel_ny <= 0 || o.peel_nv <= 0 || !(o.peel_v_hi > o.peel_v_lo) || !(o.peel_width_cells > 0) || !(o.tau_peel_max > 0))
+            return fail(ctx, THOR_ERR_ARG, "thor_run: bad peel options");
+        const double n2 = o.k_obs[0] * o.k_obs[0] + o.k_obs[1] * o.k_obs[1] + o.k_obs[2] * o.k_obs[2];
+        if (!(n2 > 0)) return fail(ctx, THOR_ERR_ARG, "thor_run: k_obs is zero");
+        double k[3], h[3] = {1, 0, 0}, i1[3], i2[3];
+        for (int i = 0; i < 3; ++i) k[i] = o.k_obs[i] / std::sqrt(n2);
+        // image-plane basis: helper axis = x unless k_obs is closest to x, then y
+        if (std::fabs(k[0]) > std::fabs(k[1]) && std::fabs(k[0]) > std::fabs(k[2])) { h[0] = 0; h[1] = 1; }
+        const double hk = h[0] * k[0] + h[1] * k[1] + h[2] * k[2];
+        double m2 = 0;
+        for (int i = 0; i < 3; ++i) { i1[i] = h[i] - hk * k[i]; m2 += i1[i] * i1[i]; }
+        for (int i = 0; i < 3; ++i) i1[i] /= std::sqrt(m2);
+        i2[0] = k[1] * i1[2] - k[2] * i1[1]; i2[1] = k[2] * i1[0] - k[0] * i1[2]; i2[2] = k[0] * i1[1] - k[1] * i1[0];
+        for (int i = 0; i < 3; ++i) { p.kobs[i] = (float)k[i]; p.img1[i] = (float)i1[i]; p.img2[i] = (float)i2[i]; }
+        p.peel_nx = o.peel_nx; p.peel_ny = o.peel_ny; p.peel_nv = o.peel_nv;
+        p.peel_v_lo = (float)o.peel_v_lo;
+        p.peel_inv_dv = (float)(o.peel_nv / (o.peel_v_hi - o.peel_v_lo));
+        p.peel_inv_width = (float)(1.0 / o.peel_width_cells);
+        p.tau_peel_max = (float)o.tau_peel_max;
+        cube_elems = (size_t)o.peel_nx * o.peel_ny * o.peel_nv;
+    }
+    p.id_offset = o.photon_id_offset; p.n_photons = n_photons; p.seed = seed; p.max_scatter = o.max_scatter;
+    CU(cudaSetDevice(ctx->device));
+    const bool keep = o.accumulate && ctx->have_run;
+    if (cube_elems != ctx->cube_elems) {
+        if (ctx->d_cube) { cudaFree(ctx->d_cube); ctx->d_cube = nullptr; }
+        ctx->cube_elems = 0;
+        if (cube_elems) {
+            CU(cudaMalloc(&ctx->d_cube, cube_elems * sizeof(unsigned long long)));
+            CU(cudaMemsetAsync(ctx->d_cube, 0, cube_elems * sizeof(unsigned long long), ctx->stream));
+            ctx->cube_elems = cube_elems;
+        }
+    } else if (cube_elems && !keep) {
+        CU(cudaMemsetAsync(ctx->d_cube, 0, cube_elems * sizeof(unsigned long long), ctx->stream));
+    }
+    if (o.raw_output && n_photons > 0) {
+        if (ctx->raw_cap < n_photons) {
+            if (ctx->d_raw) { cudaFree(ctx->d_raw); ctx->d_raw = nullptr; }
+            ctx->raw_cap = 0;
+            CU(cudaMalloc(&ctx->d_raw, (size_t)n_photons * sizeof(thor::RawRecord)));
+            ctx->raw_cap = (size_t)n_photons;
+        }
+        p.raw = ctx->d_raw;
+    }
+    if (keep) CU(cudaMemsetAsync(ctx->d_small, 0, sizeof(unsigned long long), ctx->stream));
+    else CU(cudaMemsetAsync(ctx->d_small, 0, SMALL_TOTAL * sizeof(unsigned long long), ctx->stream));
+    p.next_photon = ctx->d_small + SMALL_NEXT;
+    p.counters = ctx->d_small + SMALL_COUNTERS;
+    p.nscat_hist = ctx->d_small + SMALL_HIST;
+    p.spectrum = ctx->d_small + SMALL_SPEC;
+    p.cube = ctx->d_cube;
+    ctx->have_run = false;
+    CU(cudaEventRecord(ctx->ev0, ctx->stream));
+    if (n_photons > 0) CU(thor::launch_walk(p, ctx->n_sm, ctx->stream, &ctx->last_blocks));
+    CU(cudaEventRecord(ctx->ev1, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    CU(cudaEventElapsedTime(&ctx->last_ms, ctx->ev0, ctx->ev1));
+    ctx->last = o; ctx->last_n = n_photons; ctx->have_run = true;
+    return THOR_OK;
+}
+
+extern "C" thor_status thor_last_run_ms(const thor_ctx* ctx, float* ms) {
+    if (!ctx || !ms) return fail(nullptr, THOR_ERR_ARG, "thor_last_run_ms: NULL argument");
+    if (!ctx->have_run) return fail(const_cast<thor_ctx*>(ctx), THOR_ERR_STATE, "thor_last_run_ms: no run yet");
+    *ms = ctx->last_ms;
+    return THOR_OK;
+}
+
+extern "C" thor_status thor_tally_get(thor_ctx* ctx, int kind, void* dst, size_t dst_bytes, size_t* needed) {
+    if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_tally_get: ctx is NULL");
+    if (!ctx->have_run) return fail(ctx, THOR_ERR_STATE, "thor_tally_get: no completed run");
+    const bool dev_dst = (kind & THOR_TALLY_DEVICE_DST) != 0;
+    const int k = kind & ~THOR_TALLY_DEVICE_DST;
+    const void* src = nullptr;
+    size_t bytes = 0;
+    switch (k) {
+        case THOR_TALLY_SPECTRUM:
+            src = ctx->d_small + SMALL_SPEC; bytes = ((size_t)ctx->last.spec_bins + 2) * 8; break;
+        case THOR_TALLY_NSCAT_HIST: src = ctx->d_small + SMALL_HIST; bytes = 64 * 8; break;
+        case THOR_TALLY_COUNTERS: src = ctx->d_small + SMALL_COUNTERS; bytes = (size_t)thor::N_COUNTERS * 8; break;
+        case THOR_TALLY_CUBE:
+            if (!ctx->last.peel_on || !ctx->d_cube) return fail(ctx, THOR_ERR_STATE, "thor_tally_get: the last run had no peel-off");
+            src = ctx->d_cube; bytes = ctx->cube_elems * 8; break;
+        case THOR_TALLY_RAW:
+            if (!ctx->last.raw_output || !ctx->d_raw) return fail(ctx, THOR_ERR_STATE, "thor_tally_get: the last run kept no raw records");
+            src = ctx->d_raw; bytes = (size_t)ctx->last_n * sizeof(thor::RawRecord); break;
+        default: return fail(ctx, THOR_ERR_ARG, "thor_tally_get: unknown tally kind");
+    }
+    if (needed) *needed = bytes;
+    if (!dst) return THOR_OK;
+    if (dst_bytes < bytes) return fail(ctx, THOR_ERR_ARG, "thor_tally_get: dst_bytes too small");
+    if (bytes == 0) return THOR_OK;
+    CU(cudaSetDevice(ctx->device));
+    if (k == THOR_TALLY_CUBE && !dev_dst) {
+        // fixed point -> double on the host
+        std::vector<unsigned long long> tmp;
+        try { tmp.resize(ctx->cube_elems); } catch (...) { return fail(ctx, THOR_ERR_OOM, "thor_tally_get: host allocation failed"); }
+        CU(cudaMemcpyAsync(tmp.data(), src, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        double* d = static_cast<double*>(dst);
+        for (size_t i = 0; i < ctx->cube_elems; ++i) d[i] = (double)tmp[i] / thor::CUBE_FIXED_SCALE;
+        return THOR_OK;
+    }
+    CU(cudaMemcpyAsync(dst, src, bytes, dev_dst ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return THOR_OK;
+}

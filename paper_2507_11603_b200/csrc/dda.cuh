@@ -1,0 +1,108 @@
+// a4 DDA cell march — the paper's `query`: "index of the next cell, the pathlength to that cell",
+// propagation "from cell face to cell face".  The paper prints no traversal algorithm; this is the
+// specification of DESIGN.md §DDA, in fp32 with every multiply/add/subtract/divide rounded on its own
+// (__fmul_rn / __fadd_rn / __fsub_rn / __fdiv_rn are never contracted into FMAs), so that the sequence of cells is
+// bit-exact against any IEEE-754 implementation of the same specification.
+//
+// State: integer cell c, in-cell offset f in the CLOSED interval [0,1] (cell units), direction k, inv = 1/k.
+//   per axis: k == 0 or frozen axis -> t = +inf; else face = (k > 0 ? 1 : 0), t = (face - f) * inv
+//   exit axis: x if t_x <= t_y and t_x <= t_z, else y if t_y <= t_z, else z; segment length = t_exit
+//   other axes: f = clamp(f + len * k, 0, 1);  exit axis: f = (k > 0 ? 0 : 1), c += sign(k), wrap or leave.
+// A periodic axis of extent 1 is "frozen": treated as infinite, its offset never changes.
+#pragma once
+#include <cstdint>
+#include <math_constants.h>
+
+namespace thor {
+
+struct GridDims {
+    int nx, ny, nz;
+    unsigned periodic;   // bit 0,1,2 = x,y,z
+    unsigned frozen;     // bit 0,1,2: periodic with extent 1
+};
+
+struct Ray {
+    int cx, cy, cz;
+    float fx, fy, fz;
+    float kx, ky, kz;
+    float ix, iy, iz;    // 1/k (IEEE division)
+};
+
+__device__ __forceinline__ void ray_set_direction(Ray& r, float kx, float ky, float kz) {
+    r.kx = kx; r.ky = ky; r.kz = kz;
+    r.ix = __fdiv_rn(1.0f, kx); r.iy = __fdiv_rn(1.0f, ky); r.iz = __fdiv_rn(1.0f, kz);
+}
+
+__device__ __forceinline__ float dda_t_axis(float f, float k, float inv, bool frozen) {
+    const float face = k > 0.0f ? 1.0f : 0.0f;
+    const float t = __fmul_rn(__fsub_rn(face, f), inv);
+    return (k == 0.0f || frozen) ? CUDART_INF_F : t;
+}
+
+// Distance to the next face; returns the exit axis (0,1,2).
+__device__ __forceinline__ int dda_next_face(const Ray& r, const GridDims& g, float& len) {
+    const float tx = dda_t_axis(r.fx, r.kx, r.ix, g.frozen & 1u);
+    const float ty = dda_t_axis(r.fy, r.ky, r.iy, g.frozen & 2u);
+    const float tz = dda_t_axis(r.fz, r.kz, r.iz, g.frozen & 4u);
+    int ex;
+    if (tx <= ty && tx <= tz) { ex = 0; len = tx; }
+    else if (ty <= tz) { ex = 1; len = ty; }
+    else { ex = 2; len = tz; }
+    return ex;
+}
+
+__device__ __forceinline__ float dda_move(float f, float s, float k) {
+    const float nf = __fadd_rn(f, __fmul_rn(s, k));
+    return fminf(fmaxf(nf, 0.0f), 1.0f);
+}
+
+// Move a distance s (<= distance to the next face) inside the current cell.
+__device__ __forceinline__ void dda_advance_within(Ray& r, const GridDims& g, float s) {
+    if (!(g.frozen & 1u)) r.fx = dda_move(r.fx, s, r.kx);
+    if (!(g.frozen & 2u)) r.fy = dda_move(r.fy, s, r.ky);
+    if (!(g.frozen & 4u)) r.fz = dda_move(r.fz, s, r.kz);
+}
+
+// Cross the face found by dda_next_face.  Returns false if the ray left the grid through a non-periodic face.
+__device__ __forceinline__ bool dda_cross(Ray& r, const GridDims& g, int ex, float len) {
+    if (ex != 0 && !(g.frozen & 1u)) r.fx = dda_move(r.fx, len, r.kx);
+    if (ex != 1 && !(g.frozen & 2u)) r.fy = dda_move(r.fy, len, r.ky);
+    if (ex != 2 && !(g.frozen & 4u)) r.fz = dda_move(r.fz, len, r.kz);
+    const float ke = ex == 0 ? r.kx : ex == 1 ? r.ky : r.kz;
+    const int n = ex == 0 ? g.nx : ex == 1 ? g.ny : g.nz;
+    const int s = ke > 0.0f ? 1 : -1;
+    const float fe = s > 0 ? 0.0f : 1.0f;
+    int c = (ex == 0 ? r.cx : ex == 1 ? r.cy : r.cz) + s;
+    bool inside = true;
+    if (c < 0 || c >= n) {
+        if (g.periodic & (1u << ex)) c = c < 0 ? n - 1 : 0;
+        else inside = false;
+    }
+    if (inside) {
+        if (ex == 0) { r.cx = c; r.fx = fe; }
+        else if (ex == 1) { r.cy = c; r.fy = fe; }
+        else { r.cz = c; r.fz = fe; }
+    }
+    return inside;
+}
+
+// Position in cell units -> (cell, offset): cell = floor(pos) clamped to [0, n-1], f = pos - cell clamped to [0,1]
+// (reading A20: a source exactly on a face belongs to the upper cell with f = 0).
+__device__ __forceinline__ void dda_locate_axis(float pos, int n, int& c, float& f) {
+    int ci = (int)pos;
+    ci = min(max(ci, 0), n - 1);
+    c = ci;
+    f = fminf(fmaxf(__fsub_rn(pos, (float)ci), 0.0f), 1.0f);
+}
+
+__device__ __forceinline__ void dda_locate(Ray& r, const GridDims& g, float px, float py, float pz) {
+    dda_locate_axis(px, g.nx, r.cx, r.fx);
+    dda_locate_axis(py, g.ny, r.cy, r.fy);
+    dda_locate_axis(pz, g.nz, r.cz, r.fz);
+}
+
+__device__ __forceinline__ int64_t dda_linear(const Ray& r, const GridDims& g) {
+    return ((int64_t)r.cz * g.ny + r.cy) * (int64_t)g.nx + r.cx;
+}
+
+}  // namespace thor

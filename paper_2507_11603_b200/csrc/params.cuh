@@ -1,0 +1,75 @@
+// Kernel-side parameter block of the walk (filled by api.cu from thor_grid_create / thor_sources_set / thor_opts).
+#pragma once
+#include <cstdint>
+#include "dda.cuh"
+
+namespace thor {
+
+// Lyα atomic constants, CGS (textbook values; the paper prints none of them).
+// Definitions of x, u, v_th: PAPER.md:107.
+struct LyaConstants {
+    double c_vth;   // v_th [km/s]      = c_vth sqrt(T)        (sqrt(2 k_B / m_H) 1e-5)
+    double c_a;     // a                = c_a / sqrt(T)        (A21 lambda0 / (4 pi sqrt(2 k_B / m_H)))
+    double c_sig;   // sigma_0 [cm^2]   = c_sig / sqrt(T)      (f12 sqrt(pi) e^2 lambda0 / (m_e c sqrt(2 k_B / m_H)))
+};
+
+inline LyaConstants lya_constants() {
+    const double kB = 1.380649e-16, mH = 1.6735575e-24, c = 2.99792458e10, e = 4.80320471e-10, me = 9.1093837e-28;
+    const double lambda0 = 1215.67e-8, f12 = 0.4162, A21 = 6.265e8, pi = 3.14159265358979323846;
+    const double s = __builtin_sqrt(2.0 * kB / mH);          // cm/s per sqrt(K)
+    LyaConstants k;
+    k.c_vth = s * 1e-5;
+    k.c_a = A21 * lambda0 / (4.0 * pi * s);
+    k.c_sig = f12 * __builtin_sqrt(pi) * e * e * lambda0 / (me * c * s);
+    return k;
+}
+
+enum : int { CT_ESCAPED = 0, CT_ABSORBED, CT_TERMINATED, CT_CAPPED, CT_SCATTERINGS, CT_CROSSINGS, CT_REJ_ITERS,
+             CT_PEEL_RAYS, CT_PEEL_CELLS, N_COUNTERS };
+
+struct RawRecord { float V; uint32_t nscat; int32_t status; float kx, ky, kz; };
+
+constexpr double CUBE_FIXED_SCALE = 4294967296.0;   // peel weights are summed as round(w 2^32) in uint64
+
+struct WalkParams {
+    GridDims g;
+    const float* __restrict__ nHI;
+    const float* __restrict__ T;
+    const float* __restrict__ vx;
+    const float* __restrict__ vy;
+    const float* __restrict__ vz;
+    const float* __restrict__ kdust;     // nullptr = no dust
+    float sig_cell;      // c_sig * cell_cm: kappa_line per cell length = n * sig_cell * rsqrt(T) * H(a,x)
+    float c_a, c_vth, inv_c_vth;
+    float cell_cm;
+    // sources
+    long long n_src;
+    const float* __restrict__ src_pos;   // [n][3]
+    const float* __restrict__ src_sigma; // [n]
+    const double* __restrict__ src_cdf;  // [n], normalised cumulative luminosity, last = 1
+    // opts
+    int phase_core, phase_wing, phase_frame;
+    float phase_split_x;
+    int core_skip_mode;
+    float x_crit;
+    int spec_mode, spec_bins;
+    float spec_inv_vth_ref;              // 1 / v_th(spec_T_ref)
+    float spec_lo, spec_inv_width;       // bin = floor((val - lo) * inv_width), inv_width = bins / (hi - lo)
+    float hubble, hubble_eps, v_max;
+    int peel_on;
+    float kobs[3], img1[3], img2[3];
+    int peel_nx, peel_ny, peel_nv;
+    float peel_v_lo, peel_inv_dv;        // iv = floor((dv - lo) * inv_dv)
+    float peel_inv_width;                // 1 / peel_width_cells
+    float tau_peel_max;
+    unsigned long long id_offset, n_photons, seed, max_scatter;
+    // work distribution + tallies (device)
+    unsigned long long* next_photon;     // a14: global atomic photon counter
+    unsigned long long* spectrum;        // [spec_bins + 2]
+    unsigned long long* nscat_hist;      // [64]
+    unsigned long long* counters;        // [N_COUNTERS]
+    unsigned long long* cube;            // [ny][nx][nv] fixed point, or nullptr
+    RawRecord* raw;                      // [n_photons] or nullptr
+};
+
+}  // namespace thor

@@ -1,0 +1,53 @@
+// a1 RNG — Philox4x32-10 keyed on (seed, photon id, draw index); BASELINE.json north_star, reading A16.
+// (The paper uses xoshiro128++ per work-item; the north star replaces it by a counter-based RNG.)
+//   key     = (seed lo, seed hi)
+//   counter = (block lo, block hi, id lo, id hi),  block = draw >> 2,  word = draw & 3
+// which is cuRAND's curand_init(seed, subsequence = id, offset = 0) + curand4() layout.
+#pragma once
+#include <cstdint>
+
+namespace thor {
+
+struct U4 { uint32_t x, y, z, w; };
+
+__device__ __forceinline__ U4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                            uint32_t k1) {
+    constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
+        const uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += W0; k1 += W1;                       // bumped after the round == before every round but the first
+    }
+    return U4{c0, c1, c2, c3};
+}
+
+// u32 -> uniform in the open interval (0,1): ((r >> 8) + 0.5) 2^-24, exact in fp32 (reading A8).
+__device__ __forceinline__ float u01(uint32_t r) { return ((float)(r >> 8) + 0.5f) * 5.9604644775390625e-8f; }
+
+// One packet's draw stream.  Four cached words + the draw index; draw d is word d & 3 of block d >> 2.
+struct Stream {
+    uint32_t k0, k1, id_lo, id_hi;
+    uint32_t w0, w1, w2, w3;
+    uint64_t d;
+
+    __device__ __forceinline__ void init(uint64_t seed, uint64_t id) {
+        k0 = (uint32_t)seed; k1 = (uint32_t)(seed >> 32); id_lo = (uint32_t)id; id_hi = (uint32_t)(id >> 32);
+        d = 0;
+    }
+    __device__ __forceinline__ uint32_t next_u32() {
+        const uint32_t lane = (uint32_t)d & 3u;
+        if (lane == 0u) {
+            const uint64_t blk = d >> 2;
+            const U4 r = philox4x32_10((uint32_t)blk, (uint32_t)(blk >> 32), id_lo, id_hi, k0, k1);
+            w0 = r.x; w1 = r.y; w2 = r.z; w3 = r.w;
+        }
+        ++d;
+        return lane == 0u ? w0 : lane == 1u ? w1 : lane == 2u ? w2 : w3;
+    }
+    __device__ __forceinline__ float uniform() { return u01(next_u32()); }
+};
+
+}  // namespace thor

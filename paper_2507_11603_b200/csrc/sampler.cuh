@@ -1,0 +1,154 @@
+// a8-a10: random variates of one scattering event (§2.3.1, §3.4).
+//   u_par  : Eq. 6, f(u) ∝ e^{-u^2} / ((x-u)^2 + a^2), by rejection.
+//   u_perp : Eq. 5, each component ∝ e^{-u^2} (variance 1/2, reading A5), with the
+//            left-truncated magnitude of core-skipping (reading A7).
+//   mu     : isotropic or dipole phase function.
+//
+// u_par envelope (own design).  Eq. 10 splits the u axis once, at u0, and
+// bounds e^{-u^2} by a constant on each side; Eq. 6 is sampled exactly for any split (reading A2).  Here the axis
+// is split up to twice, 0 <= u1 <= u0 < x (x >= 0 by the symmetry f(u;-x) = f(-u;x)), with w = x - u:
+//   A  u <= u1      bound e^{-u^2} L(u1),       L(u) = 1/((x-u)^2 + a^2);  propose u ~ N(0,1/2), a draw above u1 is a
+//                   rejection; accept with L(u)/L(u1).                     mass sqrt(pi) L(u1)
+//   B  u1 < u <= u0 bound e^{-u1^2} / w^2;  propose 1/w uniform in (1/w1, 1/w0); accept with
+//                   e^{u1^2 - u^2} w^2/(w^2 + a^2).                        mass e^{-u1^2} (1/w0 - 1/w1)
+//   C  u > u0       bound e^{-u0^2} L(u);   propose psi = atan2(a, w) uniform in (psi0, pi), u = x - a cot(psi);
+//                   accept with e^{u0^2 - u^2}.                            mass e^{-u0^2} (pi - psi0)/a
+// Piece A (the Gaussian bulk of non-resonant atoms) exists for x >= 1.5; below that B runs from u = -inf with
+// u1^2 := 0 (that is Eq. 10's left piece with a 1/w^2 proposal); for x < 0.05 only C is left (plain Lorentzian).
+// B is written in w, not in the angle, because atan((u-x)/a) + pi/2 cancels catastrophically in fp32 when w >> a.
+// Split rules (any value is exact; these are within ~10 % of the acceptance optimum, 0.2 worst case near x_cw,
+// -> 0.9 in the far wing where Eq. 10 alone falls below 0.1):
+//   u1 = min(sqrt(ln x + 1.4), x - 0.4),  delta0 = sqrt(a e^{x^2 - u1^2} / (2 pi x)),  delta = delta0/(1 + x delta0),
+//   u0 = min(x - delta, sqrt(ln(pi x^2 / a) + 2)).
+#pragma once
+#include "philox.cuh"
+
+namespace thor {
+
+constexpr float PI_F = 3.14159265358979323846f;
+constexpr float SQRT_PI_F = 1.77245385090551602730f;
+
+struct UparEnvelope {
+    float xa, a, a2;
+    float u1, u1sq, u0, u0sq;
+    float inv_w0, inv_w1;     // 1/(x-u0), 1/(x-u1) (0 when B starts at -inf)
+    float L1inv;              // (x-u1)^2 + a^2
+    float psi0;
+    float mA, mAB, mTot;      // cumulative masses
+};
+
+__device__ __forceinline__ UparEnvelope upar_envelope(float a, float xa) {
+    UparEnvelope e;
+    e.xa = xa; e.a = a; e.a2 = a * a;
+    if (xa < 0.05f) {                       // C only, uref = 0
+        e.u1 = 0.f; e.u1sq = 0.f; e.u0 = 0.f; e.u0sq = 0.f; e.inv_w0 = 0.f; e.inv_w1 = 0.f; e.L1inv = 1.f;
+        e.psi0 = 0.f; e.mA = 0.f; e.mAB = 0.f; e.mTot = PI_F / a;
+        return e;
+    }
+    const bool useA = xa >= 1.5f;
+    float u1 = useA ? fminf(sqrtf(__logf(xa) + 1.4f), xa - 0.4f) : 0.f;
+    const float u1sq_rule = u1 * u1;
+    const float q = a * __expf(fminf(xa * xa - u1sq_rule, 40.f)) / (2.f * PI_F * xa);
+    const float d0 = sqrtf(q);
+    const float delta = d0 / (1.f + xa * d0);
+    const float ucap = sqrtf(__logf(PI_F * fmaxf(xa * xa, 1.f) / a) + 2.f);
+    const float u0 = fmaxf(fminf(xa - delta, ucap), 0.f);
+    u1 = fminf(u1, u0);
+    e.u0 = u0; e.u0sq = u0 * u0;
+    e.u1 = u1; e.u1sq = useA ? u1 * u1 : 0.f;
+    const float w0 = xa - u0, w1 = xa - u1;
+    e.inv_w0 = 1.f / w0;
+    e.inv_w1 = useA ? 1.f / w1 : 0.f;
+    e.L1inv = w1 * w1 + e.a2;
+    e.psi0 = atan2f(a, w0);
+    e.mA = useA ? SQRT_PI_F / e.L1inv : 0.f;
+    const float mB = __expf(-e.u1sq) * (e.inv_w0 - e.inv_w1);
+    const float mC = __expf(-e.u0sq) * (PI_F - e.psi0) / a;
+    e.mAB = e.mA + mB;
+    e.mTot = e.mAB + mC;
+    return e;
+}
+
+// One proposal + accept test.  Returns true and sets u (for x >= 0) on acceptance.
+__device__ __forceinline__ bool upar_try(const UparEnvelope& e, Stream& rng, float& u) {
+    const float r1 = rng.uniform() * e.mTot;
+    const float r2 = rng.uniform();
+    const float r3 = rng.uniform();
+    if (r1 < e.mA) {
+        const float r4 = rng.uniform();
+        const float uu = sqrtf(-__logf(r2)) * cospif(2.f * r3);
+        const float w = e.xa - uu;
+        u = uu;
+        return uu <= e.u1 && r4 * (w * w + e.a2) <= e.L1inv;
+    } else if (r1 < e.mAB) {
+        const float iw = fmaf(r2, e.inv_w0 - e.inv_w1, e.inv_w1);
+        const float w = 1.f / iw;
+        const float uu = e.xa - w;
+        const float w2 = w * w;
+        u = uu;
+        return r3 * (w2 + e.a2) <= __expf(e.u1sq - uu * uu) * w2;
+    } else {
+        const float psi = fmaf(r2, PI_F - e.psi0, e.psi0);
+        float s, c;
+        sincosf(psi, &s, &c);
+        const float uu = e.xa - e.a * c / s;
+        u = uu;
+        return r3 <= __expf(e.u0sq - uu * uu);
+    }
+}
+
+__device__ __forceinline__ float sample_upar(float a, float x, Stream& rng, uint32_t& iters) {
+    const UparEnvelope e = upar_envelope(a, fabsf(x));
+    float u;
+    do { ++iters; } while (!upar_try(e, rng, u));
+    return x < 0.f ? -u : u;
+}
+
+// Eq. 5 in polar form: magnitude m = sqrt(-ln r1) (or sqrt(x_crit^2 - ln r1) when |x_in| < x_crit),
+// angle 2 pi r2.
+__device__ __forceinline__ void sample_uperp(float x_in, float x_crit, Stream& rng, float& up1, float& up2) {
+    const float r1 = rng.uniform(), r2 = rng.uniform();
+    const float shift = fabsf(x_in) < x_crit ? x_crit * x_crit : 0.f;
+    const float m = sqrtf(shift - __logf(r1));
+    float s, c;
+    sincospif(2.f * r2, &s, &c);
+    up1 = m * c; up2 = m * s;
+}
+
+// Dipole p(mu) = 3/8 (1 + mu^2): the CDF (mu^3 + 3 mu + 4)/8 = r gives mu^3 + 3 mu - 2B = 0, B = 4r - 2, with the
+// real root mu = cbrt(B + sqrt(B^2+1)) - cbrt(sqrt(B^2+1) - B)  (Cardano).
+__device__ __forceinline__ float dipole_mu(float r) {
+    const float B = fmaf(4.f, r, -2.f);
+    const float s = sqrtf(fmaf(B, B, 1.f));
+    // cancellation-free: with p = cbrt(s + |B|), mu = sign(B) (p - 1/p)
+    const float p = cbrtf(s + fabsf(B));
+    const float m = p - 1.f / p;
+    return B < 0.f ? -m : m;
+}
+
+// phase: 0 isotropic, 1 dipole, 2 = 1/3 isotropic + 2/3 dipole, one extra draw for the mix.
+__device__ __forceinline__ float sample_mu(int phase, Stream& rng, bool& is_dipole) {
+    int ph = phase;
+    if (phase == 2) ph = rng.uniform() < (1.f / 3.f) ? 0 : 1;
+    is_dipole = ph == 1;
+    const float r = rng.uniform();
+    const float mu = is_dipole ? dipole_mu(r) : fmaf(2.f, r, -1.f);
+    return fminf(fmaxf(mu, -1.f), 1.f);
+}
+
+// Orthonormal basis (e1, e2) perpendicular to the unit vector k: helper axis = the axis of the smallest |k| component.
+__device__ __forceinline__ void ortho_basis(float kx, float ky, float kz, float e1[3], float e2[3]) {
+    const float ax = fabsf(kx), ay = fabsf(ky), az = fabsf(kz);
+    float hx = 0.f, hy = 0.f, hz = 0.f;
+    if (ax <= ay && ax <= az) hx = 1.f; else if (ay <= az) hy = 1.f; else hz = 1.f;
+    const float hk = hx * kx + hy * ky + hz * kz;
+    float x = hx - hk * kx, y = hy - hk * ky, z = hz - hk * kz;
+    const float inv = rsqrtf(x * x + y * y + z * z);
+    x *= inv; y *= inv; z *= inv;
+    e1[0] = x; e1[1] = y; e1[2] = z;
+    e2[0] = ky * z - kz * y;
+    e2[1] = kz * x - kx * z;
+    e2[2] = kx * y - ky * x;
+}
+
+}  // namespace thor

@@ -1,0 +1,118 @@
+// The walk kernel: steps a1-a14 of DESIGN.md §Path (§3.4, Fig. 1) in one persistent
+// launch.  One lane = one photon packet; finished lanes are refilled from a global atomic photon counter
+// (warp-aggregated, a14); the warp alternates between a MARCH phase (one DDA cell step + gather + Voigt optical
+// depth for every marching lane) and a SCATTER phase (u_par rejection, u_perp, phase function, Eq. 7 for every lane
+// that reached its interaction site), so that lanes execute the same phase together.
+// Escape tallies go to shared-memory histograms flushed once per block with global atomics (a13).
+#pragma once
+#include "params.cuh"
+#include "philox.cuh"
+#include "voigt.cuh"
+#include "sampler.cuh"
+
+namespace thor {
+
+enum : int { LS_IDLE = 0, LS_MARCH = 1, LS_SCATTER = 2, LS_OUT = 3 };
+
+struct CellProps { float n, T, vx, vy, vz, kd; };
+
+// a5 cell gather: SoA fp32 fields through the read-only path.
+__device__ __forceinline__ CellProps fetch_cell(const WalkParams& p, int64_t i) {
+    CellProps c;
+    c.n = __ldg(p.nHI + i); c.T = __ldg(p.T + i);
+    c.vx = __ldg(p.vx + i); c.vy = __ldg(p.vy + i); c.vz = __ldg(p.vz + i);
+    c.kd = p.kdust ? __ldg(p.kdust + i) * p.cell_cm : 0.f;
+    return c;
+}
+
+// Derived per-cell quantities (one MUFU.RSQ): a, 1/v_th, v_th, n sigma_0 cell_cm.
+struct CellDerived { float a, vth, inv_vth, nsig; };
+__device__ __forceinline__ CellDerived derive_cell(const WalkParams& p, const CellProps& c) {
+    CellDerived d;
+    const float rs = rsqrtf(c.T);
+    d.a = p.c_a * rs;
+    d.inv_vth = p.inv_c_vth * rs;
+    d.vth = p.c_vth * (c.T * rs);
+    d.nsig = c.n > 0.f ? c.n * p.sig_cell * rs : 0.f;
+    return d;
+}
+
+// a6/a7: optical depth of one segment of length len (cell units) starting at velocity offset V0, or the distance
+// s_hit at which tau_need is reached (linear within the step).  Without Hubble drift: kappa len.
+// With drift Hc (km/s per cell length): sub-steps per reading A12 — n_sub = 1 if min|x| over the segment > 6 else
+// ceil(|dV| / (eps v_th)), midpoint rule.  Returns true on interaction; k_line/k_tot are the opacities there.
+__device__ __forceinline__ bool integrate_segment(const WalkParams& p, const float2* s_tab, const CellProps& c,
+                                                  const CellDerived& d, float V0, float vk, float len, float tau_need,
+                                                  float& tau_out, float& s_hit, float& k_line, float& k_tot) {
+    tau_out = 0.f; s_hit = 0.f; k_line = 0.f; k_tot = 0.f;
+    if (c.n <= 0.f && c.kd <= 0.f) return false;
+    const float Hc = p.hubble;
+    int nsub = 1;
+    if (Hc != 0.f && c.n > 0.f && len > 0.f) {
+        const float xa = (V0 - vk) * d.inv_vth, xb = (V0 - Hc * len - vk) * d.inv_vth;
+        const float minabs = xa * xb <= 0.f ? 0.f : fminf(fabsf(xa), fabsf(xb));
+        if (minabs <= 6.f) {
+            const float q = ceilf(fabsf(Hc * len) * d.inv_vth / p.hubble_eps);
+            nsub = q < 1.f ? 1 : (q > 1e6f ? 1000000 : (int)q);
+        }
+    }
+    const float ds = len / (float)nsub;
+    float tau = 0.f;
+    for (int j = 0; j < nsub; ++j) {
+        const float Vmid = V0 - Hc * ((float)j + 0.5f) * ds;
+        const float kl = c.n > 0.f ? d.nsig * voigt_H(s_tab, d.a, (Vmid - vk) * d.inv_vth) : 0.f;
+        const float kt = kl + c.kd;
+        const float dtau = kt * ds;
+        if (tau + dtau >= tau_need && kt > 0.f) {
+            s_hit = fminf((float)j * ds + (tau_need - tau) / kt, len);
+            k_line = kl; k_tot = kt;
+            tau_out = tau_need;
+            return true;
+        }
+        tau += dtau;
+    }
+    tau_out = tau;
+    return false;
+}
+
+// a12 peel-off: w = P^ exp(-tau_obs), tau_obs integrated from `at` along k_obs to the box face at
+// velocity offset V_o by the same march (a4-a6), dropped beyond tau_peel_max (reading A13); added to
+// (pixel of the starting point projected perpendicular to k_obs, spectral bin of dv = -V at the box face).
+__device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, const Ray& at, float V_o, float phat,
+                                      uint32_t& n_cells) {
+    const float px0 = (float)at.cx + at.fx - 0.5f * (float)p.g.nx;
+    const float py0 = (float)at.cy + at.fy - 0.5f * (float)p.g.ny;
+    const float pz0 = (float)at.cz + at.fz - 0.5f * (float)p.g.nz;
+    const float px = ((px0 * p.img1[0] + py0 * p.img1[1] + pz0 * p.img1[2]) * p.peel_inv_width + 0.5f) * (float)p.peel_nx;
+    const float py = ((px0 * p.img2[0] + py0 * p.img2[1] + pz0 * p.img2[2]) * p.peel_inv_width + 0.5f) * (float)p.peel_ny;
+    if (!(px >= 0.f && px < (float)p.peel_nx && py >= 0.f && py < (float)p.peel_ny)) return;
+    Ray r = at;
+    ray_set_direction(r, p.kobs[0], p.kobs[1], p.kobs[2]);
+    float tau = 0.f, V = V_o;
+    for (;;) {
+        float len;
+        const int ex = dda_next_face(r, p.g, len);
+        const CellProps c = fetch_cell(p, dda_linear(r, p.g));
+        const CellDerived d = derive_cell(p, c);
+        const float vk = c.vx * r.kx + c.vy * r.ky + c.vz * r.kz;
+        float dtau, s_hit, kl, kt;
+        integrate_segment(p, s_tab, c, d, V, vk, len, 3.0e38f, dtau, s_hit, kl, kt);
+        tau += dtau;
+        V -= p.hubble * len;
+        ++n_cells;
+        if (tau > p.tau_peel_max) return;
+        // peel rays leave through the first box face they meet, periodic or not
+        const float ke = ex == 0 ? r.kx : ex == 1 ? r.ky : r.kz;
+        const int cn = (ex == 0 ? r.cx : ex == 1 ? r.cy : r.cz) + (ke > 0.f ? 1 : -1);
+        const int nn = ex == 0 ? p.g.nx : ex == 1 ? p.g.ny : p.g.nz;
+        if (cn < 0 || cn >= nn) break;
+        dda_cross(r, p.g, ex, len);
+    }
+    const int iv = (int)floorf((-V - p.peel_v_lo) * p.peel_inv_dv);
+    if (iv < 0 || iv >= p.peel_nv) return;
+    const float w = phat * __expf(-tau);
+    const unsigned long long q = (unsigned long long)__float2ull_rn(w * (float)CUBE_FIXED_SCALE);
+    if (q) atomicAdd(p.cube + ((size_t)(int)py * p.peel_nx + (int)px) * p.peel_nv + iv, q);
+}
+
+}  // namespace thor
