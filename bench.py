@@ -1,0 +1,297 @@
+"""bench.py — throughput of the Lyα random walk (the whole hot path, DESIGN.md §Path rows a1-a14) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload shell|sphere|slab|turb|web] [--impl reference]
+
+A "step" is one thor_run over one batch of packets of the workload: BASELINE.json configs[1] (expanding dusty shell,
+128^3 grid, 1e6 packets) by default.  value = scatterings/s over the timed steps (whole job, all ranks), with
+packets/s and cell crossings/s beside it; inputs are resident in HBM when the timed region starts.  `e2e` is the same
+metric through the C-ABI with HOST buffers (grid + sources copied host->device, tallies copied back, all inside the
+timed region).  `roofline` is the issue-slot ("alu") roofline of the walk kernel; `cpu_baseline`
+is the fp64 oracle timed on this box's host cores on a bounded sample of the same workload.
+
+N > 1 (torchrun): the path shards by photon id: every rank walks its own id range of the
+same size on its own replica of the grid (weak scaling), and the tallies are summed with one NCCL all-reduce.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+from paper_2507_11603_b200 import workloads as W
+
+# Issue-slot roofline constants: algorithmic thread-instructions per unit of work, counted
+# once from ncu (smsp__thread_inst_executed.sum of the walk kernel regressed on its scattering / crossing counters;
+# profiles/r01_walk_inst_per_unit.md) — fixed numbers, so a slower kernel cannot raise its own roofline fraction.
+INST_PER_SCATTERING = 640.0
+INST_PER_CROSSING = 110.0
+N_SM, SCHEDULERS_PER_SM, LANES = 148, 4, 32
+
+
+def make_workload(name, n_photons=None):
+    if name == "shell":      # BASELINE.json configs[1]
+        w = W.expanding_shell(n=128, n_photons=1_000_000)
+    elif name == "sphere":   # configs[0] scaled to fill the GPU (same physics, more packets), tau0 = 1e4
+        w = W.static_sphere(n=32, tau0=1e4, T=10.0, n_photons=200_000)
+    elif name == "slab":     # configs[2]
+        w = W.static_slab(n_photons=1_000_000)
+    elif name == "turb":     # configs[3] at 256^3
+        w = W.turbulent_box(n=256, n_src=1 << 16, n_photons=100_000, peel_pix=256, peel_bins=400)
+        w["opts"]["max_scatter"] = 100_000
+    elif name == "web":      # configs[4] at 512^3
+        w = W.cosmic_web(n=512, n_src=1 << 18, n_photons=1_000_000, map_pix=2048)
+    else:
+        raise SystemExit(f"unknown workload {name}")
+    if n_photons:
+        w["n_photons"] = int(n_photons)
+    return w
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML every 100 ms while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz, self._stop_evt = index, [], set(), None, threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap", nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            self._stop_evt.wait(0.1)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return dict(sm_mhz=med, sm_max_mhz=self.max_mhz, reasons=sorted(self.reasons), samples=len(self.samples))
+
+
+def oracle_sample(w, budget_s, chunk):
+    """Times the oracle, as it stands, single-threaded, on photon ids [0, k*chunk) of the workload until budget_s
+    seconds of CPU work are spent.  Returns (scatterings, packets, crossings, seconds)."""
+    from oracle import thor_oracle
+    thor_oracle.build()
+    scat = pk = cross = 0
+    secs = 0.0
+    off = 0
+    while secs < budget_s:
+        r = thor_oracle.run(w["grid"], w["sources"], dict(w["opts"], photon_id_offset=off), chunk, w["seed"],
+                            want_raw=False)
+        secs += r["seconds"]
+        scat += r["counters"]["scatterings"]
+        cross += r["counters"]["cell_crossings"]
+        pk += chunk
+        off += chunk
+    return scat, pk, cross, secs
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle, as it stands, on the box's host cores, same config / metric / unit; each step a
+    bounded sample of the workload (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    chunk = max(1, min(w["n_photons"], args.ref_chunk))
+    for _ in range(args.warmup):
+        oracle_sample(w, 0.0, max(1, chunk // 10))
+    scat = pk = 0
+    secs = 0.0
+    for _ in range(args.steps):
+        s, p, _, t = oracle_sample(w, args.ref_budget, chunk)
+        scat += s
+        pk += p
+        secs += t
+    v = scat / secs
+    sample = f"{pk} packets (ids 0..) of {w['n_photons']} per step x {args.steps} steps, single thread, fp64"
+    print(json.dumps({
+        "impl": "reference", "metric": "lya_scatterings_per_sec", "value": v, "unit": "scatterings/s",
+        "packets_per_sec": pk / secs, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": w["name"], "n_photons_per_step": pk // args.steps},
+        "cpu_baseline": {"value": v, "unit": "scatterings/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "scatterings/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="shell")
+    ap.add_argument("--n-photons", type=int, default=0)
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--ref-budget", type=float, default=10.0, help="seconds of oracle work per reference step")
+    ap.add_argument("--ref-chunk", type=int, default=500)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    w = make_workload(args.workload, args.n_photons)
+    if args.impl == "reference":
+        return run_reference(args, w)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2507_11603_b200.csrc import build as cuda_build
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank == 0:
+        cuda_build.build()
+    from paper_2507_11603_b200 import thor
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist.barrier()
+    thor.lib()
+    n = w["n_photons"]
+    opts = dict(w["opts"], raw_output=0)
+    ctx = thor.Context.from_workload(w["grid"])                    # fields resident in HBM before the timed region
+    ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    spec_dev = torch.zeros(opts["spec_bins"] + 2, dtype=torch.int64, device="cuda")
+    cnt_dev = torch.zeros(len(thor.COUNTER_NAMES), dtype=torch.int64, device="cuda")
+
+    def step(i):
+        # rank r walks photon ids [r n, (r+1) n) of step i's seed; tallies summed over ranks (the one exchange step)
+        ctx.run(n, w["seed"] + i, dict(opts, photon_id_offset=rank * n))
+        ctx.tally_to_device(thor.TALLY_SPECTRUM, spec_dev)
+        ctx.tally_to_device(thor.TALLY_COUNTERS, cnt_dev)
+        if world > 1:
+            dist.all_reduce(spec_dev)
+            dist.all_reduce(cnt_dev)
+        return ctx.last_run_ms()
+
+    for i in range(args.warmup):
+        step(-1 - i)
+    sampler = ClockSampler(local)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kern_ms, totals = [], np.zeros(len(thor.COUNTER_NAMES), np.int64)
+    for i in range(args.steps):
+        flush.zero_()                                              # flush L2 between timed iterations (untimed)
+        ev[i][0].record()
+        kern_ms.append(step(i))
+        ev[i][1].record()
+        totals += cnt_dev.cpu().numpy()                            # already summed over ranks
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop()
+    step_ms = sum(a.elapsed_time(b) for a, b in ev)
+    t = torch.tensor([step_ms, sum(kern_ms)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    step_ms, kernel_ms = float(t[0]), float(t[1])
+    c = dict(zip(thor.COUNTER_NAMES, (int(v) for v in totals)))
+    packets = c["escaped"] + c["absorbed"] + c["terminated"] + c["capped"]
+    assert packets == n * world * args.steps, (packets, n, world, args.steps)
+    secs = step_ms * 1e-3
+    value = c["scatterings"] / secs
+
+    out = {
+        "metric": "lya_scatterings_per_sec", "value": value, "unit": "scatterings/s",
+        "packets_per_sec": packets / secs, "cell_crossings_per_sec": (c["cell_crossings"] + c["peel_cells"]) / secs,
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w["name"], "baseline_config": args.workload, "grid": [w["grid"]["nx"], w["grid"]["ny"], w["grid"]["nz"]],
+                   "n_photons_per_step_per_gpu": n, "parallelism": f"photon-id shards x{world}, grid replicated",
+                   "l2": "flushed between timed iterations (256 MB memset)",
+                   "scatterings_per_packet": c["scatterings"] / packets,
+                   "rejection_iters_per_scattering": c["rejection_iters"] / max(1, c["scatterings"])},
+        "clocks": clocks, "gpu_launches": args.steps * 1,
+        "counters": c,
+    }
+    # ---- roofline of the dominant (only) kernel: issue-slot bound (grid is L2-resident)
+    inst = INST_PER_SCATTERING * c["scatterings"] + INST_PER_CROSSING * (c["cell_crossings"] + c["peel_cells"])
+    sm_hz = 1e6 * (clocks["sm_max_mhz"] or 1965.0)
+    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    peak = n_sm * SCHEDULERS_PER_SM * LANES * sm_hz * world
+    achieved = inst / (kernel_ms * 1e-3)
+    out["roofline"] = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "G thread-inst/s",
+                       "frac": achieved / peak, "traffic": None,
+                       "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_hz / 1e6:.0f} MHz (clocks.max.sm), derived in DESIGN.md",
+                       "kernel": "walk_kernel", "kernel_ms_per_launch": kernel_ms / args.steps,
+                       "inst_per_scattering": INST_PER_SCATTERING, "inst_per_crossing": INST_PER_CROSSING}
+    ctx.close()
+
+    # ---- e2e: the same step through the C-ABI with HOST buffers; H2D of grid + sources and D2H of tallies are timed
+    if not args.no_e2e:
+        fields = [k for k in ("nHI", "T", "vx", "vy", "vz", "kdust") if w["grid"].get(k) is not None]
+        h2d = sum(w["grid"][k].nbytes for k in fields) + sum(np.asarray(w["sources"][k]).nbytes for k in ("pos", "lum", "sigma"))
+        d2h = (opts["spec_bins"] + 2 + 64 + len(thor.COUNTER_NAMES)) * 8
+        e_scat, e_secs = 0, 0.0
+        for i in range(-1, args.steps):                             # one untimed warm-up pass
+            if world > 1:
+                dist.barrier()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            cx = thor.Context.from_workload(w["grid"], host=True)
+            cx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
+            cx.run(n, w["seed"] + max(i, 0), dict(opts, photon_id_offset=rank * n))
+            cx.spectrum(); cx.nscat_hist()
+            cc = cx.counters()
+            cx.close()
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            tt = torch.tensor([dt, float(cc["scatterings"])], dtype=torch.float64, device="cuda")
+            if world > 1:
+                mx = tt.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+                dist.all_reduce(tt)
+                tt[0] = mx[0]
+            if i >= 0:
+                e_secs += float(tt[0]); e_scat += float(tt[1])
+        out["e2e"] = {"value": e_scat / e_secs, "unit": "scatterings/s", "h2d_bytes_per_step": int(h2d),
+                      "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e_secs / args.steps,
+                      "timing": "host wall clock around create(host arrays)+sources_set+run+tally_get+destroy, device synchronised on both sides, max over ranks"}
+
+    # ---- cpu_baseline: the oracle on a bounded sample, rank 0 at N = 1 only
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        chunk = max(1, min(n, args.ref_chunk))
+        s, p, _, t = oracle_sample(w, args.cpu_budget, chunk)
+        out["cpu_baseline"] = {"value": s / t, "unit": "scatterings/s", "cores": 1, "kind": "oracle",
+                               "packets_per_sec": p / t,
+                               "sample": f"photon ids [0, {p}) of the same workload and seed, single thread, fp64, {t:.1f} s"}
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()

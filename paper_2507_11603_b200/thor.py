@@ -188,6 +188,15 @@ class Context:
         assert need.value == out.nbytes, (need.value, out.nbytes)
         return out
 
+    def tally_to_device(self, kind, tensor):
+        """Copies tally `kind` into a CUDA tensor (THOR_TALLY_DEVICE_DST): no host round trip (multi-GPU reduce)."""
+        nbytes = tensor.numel() * tensor.element_size()
+        need = C.c_size_t()
+        _check(lib().thor_tally_get(self._ctx, kind | TALLY_DEVICE_DST, C.c_void_p(tensor.data_ptr()), nbytes,
+                                    C.byref(need)), self._ctx)
+        assert need.value == nbytes, (need.value, nbytes)
+        return tensor
+
     def spectrum(self):
         return self._get(TALLY_SPECTRUM, np.uint64, self._opts.spec_bins + 2)
 

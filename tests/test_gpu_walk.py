@@ -267,7 +267,7 @@ def test_dust_only_escape_fraction(thor):
     w = dict(grid=grid, sources=src, opts=dict(spec_bins=10, spec_lo=-1.0, spec_hi=1.0), n_photons=n, seed=4)
     g = thor.run_workload(w)
     _conserved(g, n)
-    k = np.abs(g["raw"][["kx", "ky", "kz"]].view(np.float32).reshape(-1, 3)).astype(np.float64)
+    k = np.abs(np.stack([g["raw"]["kx"], g["raw"]["ky"], g["raw"]["kz"]], 1)).astype(np.float64)
     chord = (N / 2) / k.max(axis=1)
     expect = np.exp(-kd_per_cell * chord).mean()          # directions are isotropic for absorbed and escaped alike
     f = g["counters"]["escaped"] / n

@@ -195,3 +195,97 @@ def test_hubble_drift_gunn_peterson(oracle):
     # halving eps changes nothing within noise (the midpoint rule has converged)
     res2 = oracle.run(w["grid"], w["sources"], dict(opts, hubble_eps=0.05), n, seed=5)
     assert abs(res2["nscat_hist"][0] / n - p) < 4.5 * math.sqrt(p * (1 - p) / n)
+
+
+# ---------------------------------------------------------------- P12: peel-off (next-event estimator)
+def _peel_opts(base, k_obs, nv=40, v=100.0, pix=8, width=16.0):
+    return dict(base, peel_on=1, k_obs=k_obs, peel_nx=pix, peel_ny=pix, peel_nv=nv, peel_v_lo=-v, peel_v_hi=v,
+                peel_width_cells=width, tau_peel_max=30.0)
+
+
+def test_peel_thin_limit_and_pixel_mapping(oracle):
+    """No gas: every packet contributes exactly P^ = 1 at emission, at the pixel of the source
+    projected perpendicular to k_obs and in the spectral bin of the emitted frequency.  For k_obs = +z the image
+    axes are (x, y)."""
+    n = 5000
+    w = W.static_sphere(n=16, tau0=0.0, T=1e4, n_photons=n)
+    src = dict(pos=np.array([[3.2, 12.7, 5.0]], np.float32), lum=np.ones(1, np.float32), sigma=np.zeros(1, np.float32))
+    res = oracle.run(w["grid"], src, _peel_opts(w["opts"], (0.0, 0.0, 1.0), nv=4, v=10.0), n, seed=3)
+    assert res["counters"]["peel_rays"] == n and res["counters"]["scatterings"] == 0
+    cube = res["cube"]
+    assert cube.sum() == pytest.approx(n, rel=1e-12)
+    iy, ix, iv = np.unravel_index(cube.argmax(), cube.shape)
+    assert (ix, iy, iv) == (int(3.2 / 2), int(12.7 / 2), 2) and cube[iy, ix, iv] == pytest.approx(n, rel=1e-12)
+
+
+@pytest.mark.parametrize("phase", [0, 1])
+def test_peel_matches_escapes_into_cone(oracle, phase):
+    """The next-event-estimator identity: the peel-off spectrum toward k_obs equals, in expectation, the spectrum of
+    the packets that escape into a small cone about k_obs times 4 pi / dOmega.  Few-scattering sphere (tau0 = 5) in
+    uniform bulk motion, so that frequencies depend on direction (v.k_obs shift), with the isotropic (P^ = 1) and the
+    dipole (P^ = 3/4 (1 + mu^2)) weights.  A wrong weight, a peel from the wrong frequency / frame, a missing
+    e^{-tau_obs} or a missing emission-time contribution each break it."""
+    n = 400_000
+    w = W.static_sphere(n=16, tau0=5.0, T=1e4, n_photons=n)
+    g = w["grid"]
+    ko = np.array([0.3, -0.5, 0.8])
+    ko /= np.linalg.norm(ko)
+    v = 50.0 * ko                    # along k_obs: v.k varies only to second order over the cone (50 (1 - cos) km/s)
+    grid = dict(g, vx=np.full_like(g["vx"], v[0]), vy=np.full_like(g["vy"], v[1]), vz=np.full_like(g["vz"], v[2]))
+    nv, vr = 12, 120.0
+    opts = _peel_opts(dict(w["opts"], phase_core=phase, phase_wing=phase), tuple(ko), nv=nv, v=vr, pix=4, width=40.0)
+    res = oracle.run(grid, w["sources"], opts, n, seed=11)
+    _conserved(res, n)
+    raw = res["raw"]
+    cosang = raw["kx"] * ko[0] + raw["ky"] * ko[1] + raw["kz"] * ko[2]
+    cmin = 0.96
+    cone = raw[cosang > cmin]
+    frac = (1 - cmin) / 2
+    h_cone, _ = np.histogram(-cone["V"].astype(float), bins=nv, range=(-vr, vr))
+    peel = res["cube"].sum(axis=(0, 1))
+    assert peel.sum() == pytest.approx(len(cone) / frac, rel=0.04)
+    expect = h_cone / frac
+    sig = np.sqrt(h_cone + 1.0) / frac + np.sqrt(1.5 * peel + 1.0)
+    z = np.abs(peel - expect) / sig
+    assert z.max() < 4.5, (z, peel, expect)
+    # the line is shifted by v.k_obs in dv = -V (bulk motion toward the observer = blueshift = negative dv)
+    centres = np.linspace(-vr, vr, nv + 1)[:-1] + vr / nv
+    assert abs((peel * centres).sum() / peel.sum() + 50.0) < 2.0
+    # the dipole weight changes the angular distribution of singly scattered light, not the total (sphere): both ~ n
+    assert peel.sum() == pytest.approx(n, rel=0.01)
+
+
+def test_peel_phase_function_weight(oracle):
+    """The peel weight carries the phase function toward the observer.  A small optically thin blob
+    far from the source along +x is lit almost head-on (k_in ~ +x), so singly scattered light toward an observer at
+    mu = k_in.k_obs has weight P^(mu): isotropic 1, dipole 3/4 (1 + mu^2).  Observers at +y (mu ~ 0) and at 45 degrees
+    in the x-y plane (mu ~ 0.707) therefore see scattered totals in the ratio 1 (isotropic) or 0.75/1.125 = 2/3
+    (dipole).  The walks are identical in both runs (peel-off consumes no random numbers, reading A16); the direct
+    contribution is exactly one per packet because neither sight line from the source crosses the blob."""
+    n = 1_000_000
+    N = 16
+    shape = (N, N, N)
+    T = 1e4
+    nHI = np.zeros(shape, np.float32)
+    tau_cell = 0.05
+    nHI[6:10, 6:10, 12:14] = tau_cell / (oracle.sigma0_cm2(T) * W.PC_CM)          # [z, y, x]
+    z = np.zeros(shape, np.float32)
+    grid = dict(nx=N, ny=N, nz=N, periodic=(0, 0, 0), cell_cm=W.PC_CM, nHI=nHI, T=np.full(shape, T, np.float32),
+                vx=z, vy=z, vz=z, kdust=None)
+    src = dict(pos=np.array([[2.0, 8.0, 8.0]], np.float32), lum=np.ones(1, np.float32), sigma=np.zeros(1, np.float32))
+    s = 1 / math.sqrt(2)
+    out = {}
+    for phase in (0, 1):
+        for name, ko in (("perp", (0.0, 1.0, 0.0)), ("fwd45", (s, s, 0.0))):
+            opts = _peel_opts(dict(spec_bins=10, spec_lo=-100.0, spec_hi=100.0, spec_mode=1, phase_core=phase,
+                                   phase_wing=phase), ko, nv=1, v=1e4, pix=1, width=64.0)
+            res = oracle.run(grid, src, opts, n, seed=5)
+            assert res["counters"]["peel_rays"] == n + res["counters"]["scatterings"]
+            out[phase, name] = (res["cube"].sum() - n, res["counters"]["scatterings"])
+    n_scat = out[0, "perp"][1]
+    assert n_scat > 500 and out[0, "fwd45"][1] == n_scat             # same walk for both observers
+    # isotropic: every scattering contributes 1 minus up to ~10 % of self-absorption on the way out of the blob
+    assert 0.88 * n_scat < out[0, "perp"][0] <= n_scat
+    assert out[0, "perp"][0] / out[0, "fwd45"][0] == pytest.approx(1.0, abs=0.03)
+    assert out[1, "perp"][0] / out[1, "fwd45"][0] == pytest.approx(2.0 / 3.0, abs=0.03)
+    assert 0.88 * 0.75 * out[1, "perp"][1] < out[1, "perp"][0] <= 0.76 * out[1, "perp"][1]
