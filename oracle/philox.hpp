@@ -32,9 +32,10 @@ inline Philox4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
     return Philox4{{c0, c1, c2, c3}};
 }
 
-// u32 -> uniform in the OPEN interval (0,1): ((r >> 8) + 0.5) * 2^-24 (reading A8; exact in fp32 and fp64).
+// u32 -> uniform in the OPEN interval (0,1): ((r >> 9) + 0.5) * 2^-23 (reading A8).  23 bits, not 24: k + 1/2 with
+// k < 2^23 fits a 24-bit significand, so the same value is exact in fp32 and in fp64.
 // The paper offers R in [0,1) and 1-R in (0,1]; the open interval keeps -ln(u) finite both ways.
-inline double u32_to_uniform(uint32_t r) { return ((double)(r >> 8) + 0.5) * (1.0 / 16777216.0); }
+inline double u32_to_uniform(uint32_t r) { return ((double)(r >> 9) + 0.5) * (1.0 / 8388608.0); }
 
 // One packet's stream: draw d of photon `id` under `seed`.
 class DrawStream {

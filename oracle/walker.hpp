@@ -126,13 +126,13 @@ inline SegmentOut integrate_segment(const Grid& g, const CellProps& p, double V0
     }
     const double ds = len / nsub;
     for (int j = 0; j < nsub; ++j) {
-        const double Vmid = V0 - Hc * (j + 0.5) * ds;
+        const double Vmid = Hc != 0.0 ? V0 - Hc * (j + 0.5) * ds : V0;   // no 0 * inf when ds = +inf (reading A24)
         const double kl = kappa_line(g, p, Vmid, k);
         const double kt = kl + kdust;
         const double dtau = kt * ds;
         if (o.tau + dtau >= tau_need && kt > 0.0) {
             o.hit = true;
-            o.s_hit = j * ds + (tau_need - o.tau) / kt;       // linear within the step
+            o.s_hit = (j ? j * ds : 0.0) + (tau_need - o.tau) / kt;       // linear within the step
             if (o.s_hit > len) o.s_hit = len;
             o.k_line = kl;
             o.tau = tau_need;
@@ -213,6 +213,7 @@ private:
         for (;;) {
             double len;
             const int ex = dda_next_face(r, g_.dims, len);
+            if (std::isinf(len)) return;                      // reading A24: never reaches a box face -> dropped
             const CellProps cp = fetch_cell(g_, r.c);
             const SegmentOut so = integrate_segment(g_, cp, V, kobs_, len, 1e300, o_.hubble_kms_per_cell, o_.hubble_eps);
             tau += so.tau;
@@ -271,9 +272,12 @@ private:
                 so = integrate_segment(g_, cp, V, k, len, tau_target - tau_acc, Hc, o_.hubble_eps);
                 if (so.hit) {
                     dda_advance_within(ray, g_.dims, so.s_hit);
-                    V -= Hc * so.s_hit;
+                    if (Hc != 0.0) V -= Hc * so.s_hit;
                     break;
                 }
+                // Reading A24: a ray parallel to every non-frozen axis has an infinite segment; if it did not
+                // interact there (empty cell, or a drifting frequency) it can neither leave nor be followed: capped.
+                if (std::isinf(len)) { status = ST_CAPPED; done = true; break; }
                 tau_acc += so.tau;
                 V -= Hc * len;
                 res.counters[CT_CROSSINGS]++;

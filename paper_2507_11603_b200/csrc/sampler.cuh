@@ -100,7 +100,8 @@ __device__ __forceinline__ bool upar_try(const UparEnvelope& e, Stream& rng, flo
 __device__ __forceinline__ float sample_upar(float a, float x, Stream& rng, uint32_t& iters) {
     const UparEnvelope e = upar_envelope(a, fabsf(x));
     float u;
-    do { ++iters; } while (!upar_try(e, rng, u));
+    uint32_t guard = 0;                      // fail-safe: acceptance is >= ~0.15 everywhere, 2^20 rejections cannot
+    do { ++iters; } while (!upar_try(e, rng, u) && ++guard < (1u << 20));   // happen unless x is NaN; never hang
     return x < 0.f ? -u : u;
 }
 

@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(WALK_THREADS, 2) walk_kernel(const __grid_cons
             const bool hit = integrate_segment(p, sh.voigt, c, d, V, vk, len, tau_rem, dtau, s_hit, kl, kt);
             if (hit) {
                 dda_advance_within(ray, p.g, s_hit);
-                V -= p.hubble * s_hit;
+                if (p.hubble != 0.f) V -= p.hubble * s_hit;
                 // a7 interaction kind: dust with probability kappa_dust / kappa_total
                 bool absorbed = false;
                 if (p.kdust) absorbed = rng.uniform() * kt < c.kd;
@@ -127,6 +127,11 @@ __global__ void __launch_bounds__(WALK_THREADS, 2) walk_kernel(const __grid_cons
                     }
                     state = LS_SCATTER;
                 }
+            } else if (!(len < CUDART_INF_F)) {
+                // reading A24: infinite segment (ray parallel to every non-frozen axis) without interaction: the
+                // packet can neither leave nor be followed -> capped
+                tally_finish(p, sh, CT_CAPPED, V, nscat, crossings, rej_iters, id, ray.kx, ray.ky, ray.kz);
+                state = LS_IDLE;
             } else {
                 tau_rem -= dtau;
                 V -= p.hubble * len;
@@ -182,7 +187,7 @@ __global__ void __launch_bounds__(WALK_THREADS, 2) walk_kernel(const __grid_cons
                 if (p.v_max > 0.f && fabsf(V) > p.v_max) {
                     tally_finish(p, sh, CT_TERMINATED, V, nscat, crossings, rej_iters, id, nx, ny, nz);
                     state = LS_IDLE;
-                } else if (p.max_scatter && nscat >= p.max_scatter) {
+                } else if ((p.max_scatter && nscat >= p.max_scatter) || !(fabsf(V) <= 3.0e38f)) {   // cap, or fail-safe: non-finite V
                     tally_finish(p, sh, CT_CAPPED, V, nscat, crossings, rej_iters, id, nx, ny, nz);
                     state = LS_IDLE;
                 } else {

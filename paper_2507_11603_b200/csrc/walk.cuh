@@ -59,12 +59,12 @@ __device__ __forceinline__ bool integrate_segment(const WalkParams& p, const flo
     const float ds = len / (float)nsub;
     float tau = 0.f;
     for (int j = 0; j < nsub; ++j) {
-        const float Vmid = V0 - Hc * ((float)j + 0.5f) * ds;
+        const float Vmid = Hc != 0.f ? V0 - Hc * ((float)j + 0.5f) * ds : V0;   // no 0 * inf when ds = +inf (A24)
         const float kl = c.n > 0.f ? d.nsig * voigt_H(s_tab, d.a, (Vmid - vk) * d.inv_vth) : 0.f;
         const float kt = kl + c.kd;
         const float dtau = kt * ds;
         if (tau + dtau >= tau_need && kt > 0.f) {
-            s_hit = fminf((float)j * ds + (tau_need - tau) / kt, len);
+            s_hit = fminf((j ? (float)j * ds : 0.f) + (tau_need - tau) / kt, len);
             k_line = kl; k_tot = kt;
             tau_out = tau_need;
             return true;
@@ -92,6 +92,7 @@ __device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, 
     for (;;) {
         float len;
         const int ex = dda_next_face(r, p.g, len);
+        if (!(len < CUDART_INF_F)) return;                    // reading A24: never reaches a box face -> dropped
         const CellProps c = fetch_cell(p, dda_linear(r, p.g));
         const CellDerived d = derive_cell(p, c);
         const float vk = c.vx * r.kx + c.vy * r.ky + c.vz * r.kz;

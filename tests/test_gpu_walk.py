@@ -59,7 +59,11 @@ def _statistical_parity(g, o, n_g, n_o, spec_scale=1.0):
     """g, o: result dicts with raw records; the two sides may hold different packet counts."""
     eg = g["raw"][g["raw"]["status"] != 1]
     eo = o["raw"][o["raw"]["status"] != 1]
-    assert stats.ks_2samp(eg["V"], eo["V"]).pvalue > 0.01
+    if len(eg) > 1 and len(eo) > 1:
+        assert stats.ks_2samp(eg["V"], eo["V"]).pvalue > 0.01
+    else:                                                   # nothing escapes (all absorbed): compare final V instead
+        assert len(eg) == len(eo) == 0
+        assert stats.ks_2samp(g["raw"]["V"], o["raw"]["V"]).pvalue > 0.01
     assert stats.ks_2samp(g["raw"]["nscat"], o["raw"]["nscat"]).pvalue > 0.01
     mg, mo = g["raw"]["nscat"].astype(np.float64), o["raw"]["nscat"].astype(np.float64)
     se = math.sqrt(mg.var() / n_g + mo.var() / n_o)
@@ -362,3 +366,33 @@ def test_multi_source_selection(thor):
     assert abs(f0 - 1 / 8) < 4 * math.sqrt(1 / 8 * 7 / 8 / n)
     var = (3 * 100.0 + 4 * 900.0) / 8
     assert abs(V.var() - var) < 0.03 * var
+
+
+def test_infinite_segments(thor, oracle):
+    """Reading A24 on the GPU.  (i) The packet that exposed it: seed 2^64 - 1, photon id 528744 of config 3 is emitted
+    with k_z = 0 exactly, an infinite in-plane segment; it must interact at l* = tau / kappa and walk on, not spin
+    on 0 * inf = NaN.  (ii) A fully periodic 1 x 1 x 1 cell (every segment infinite): dusty gas absorbs every packet,
+    with the same zero-scattering fraction as the oracle; an empty cell caps every packet."""
+    w = W.static_slab(n_photons=64)
+    ctx = thor.Context.from_workload(w["grid"])
+    try:
+        ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
+        ctx.run(64, (1 << 64) - 1, dict(w["opts"], raw_output=1, photon_id_offset=528744 - 10))
+        raw, c = ctx.raw(), ctx.counters()
+        assert c["escaped"] == 64 and np.all(np.isfinite(raw["V"])) and raw["nscat"][10] > 0
+    finally:
+        ctx.close()
+    n = 20_000
+    one = lambda v: np.full((1, 1, 1), v, np.float32)
+    T, tau_cell = 1e4, 3.0
+    grid = dict(nx=1, ny=1, nz=1, periodic=(1, 1, 1), cell_cm=W.PC_CM, nHI=one(tau_cell / (oracle.sigma0_cm2(T) * W.PC_CM)),
+                T=one(T), vx=one(0), vy=one(0), vz=one(0), kdust=one(0.5 / W.PC_CM))
+    src = dict(pos=np.array([[0.5, 0.5, 0.5]], np.float32), lum=np.ones(1, np.float32), sigma=np.zeros(1, np.float32))
+    wl = dict(grid=grid, sources=src, opts=dict(spec_bins=10, spec_lo=-50.0, spec_hi=50.0), n_photons=n, seed=2)
+    g = thor.run_workload(wl)
+    o = oracle.run(grid, src, wl["opts"], n, 2)
+    _conserved(g, n)
+    assert g["counters"]["absorbed"] == n and g["counters"]["cell_crossings"] == 0
+    _statistical_parity(g, o, n, n)
+    g = thor.run_workload(dict(wl, grid=dict(grid, nHI=one(0), kdust=None), n_photons=100))
+    assert g["counters"]["capped"] == 100 and g["counters"]["scatterings"] == 0

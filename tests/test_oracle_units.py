@@ -40,9 +40,13 @@ def test_draw_stream_layout(oracle):
 
 
 def test_uniform_mapping_open_interval(oracle):
-    assert oracle.u32_to_uniform(0) == 0.5 / 2 ** 24
-    assert oracle.u32_to_uniform(0xFFFFFFFF) == 1.0 - 0.5 / 2 ** 24
-    assert oracle.u32_to_uniform(0x80000000) == (2 ** 23 + 0.5) / 2 ** 24
+    assert oracle.u32_to_uniform(0) == 0.5 / 2 ** 23
+    assert oracle.u32_to_uniform(0xFFFFFFFF) == 1.0 - 0.5 / 2 ** 23
+    assert oracle.u32_to_uniform(0x80000000) == (2 ** 22 + 0.5) / 2 ** 23
+    # every value is representable in fp32 (so the CUDA path can form exactly the same uniforms)
+    for r in (0, 0x1FF, 0x200, 0x7FFFFFFF, 0x80000000, 0xFFFFFE00, 0xFFFFFFFF):
+        u = oracle.u32_to_uniform(r)
+        assert float(np.float32(u)) == u and 0.0 < u < 1.0
     u = np.array([oracle.u32_to_uniform(int(r)) for r in oracle.draws_u32(1, 0, 4000)])
     assert stats.kstest(u, stats.uniform(0, 1).cdf).pvalue > 1e-3
 

@@ -289,3 +289,32 @@ def test_peel_phase_function_weight(oracle):
     assert out[0, "perp"][0] / out[0, "fwd45"][0] == pytest.approx(1.0, abs=0.03)
     assert out[1, "perp"][0] / out[1, "fwd45"][0] == pytest.approx(2.0 / 3.0, abs=0.03)
     assert 0.88 * 0.75 * out[1, "perp"][1] < out[1, "perp"][0] <= 0.76 * out[1, "perp"][1]
+
+
+def test_infinite_segments_in_a_slab(oracle):
+    """Reading A24.  In the 1 x 1 x nz slab (x, y periodic with extent 1: infinite) a ray with k_z = 0 has an infinite
+    segment.  In gas it interacts at l* = tau / kappa like any other ray (no NaN from 0 * inf); in an empty slab it can
+    never leave and is counted as capped.  k_z = 0 is forced here by a dipole-free trick: a source in a 1 x 1 x 1
+    fully periodic cell has no finite face at all, so EVERY ray is infinite."""
+    n = 2000
+    shape = (1, 1, 1)
+    one = lambda v: np.full(shape, v, np.float32)
+    T = 1e4
+    tau_cell = 3.0
+    grid = dict(nx=1, ny=1, nz=1, periodic=(1, 1, 1), cell_cm=W.PC_CM, nHI=one(tau_cell / (oracle.sigma0_cm2(T) * W.PC_CM)),
+                T=one(T), vx=one(0), vy=one(0), vz=one(0), kdust=one(0.5 / W.PC_CM))
+    src = dict(pos=np.array([[0.5, 0.5, 0.5]], np.float32), lum=np.ones(1, np.float32), sigma=np.zeros(1, np.float32))
+    opts = dict(spec_bins=10, spec_lo=-50.0, spec_hi=50.0)
+    res = oracle.run(grid, src, opts, n, seed=2)
+    _conserved(res, n)
+    # an infinite uniform dusty medium: every packet is eventually absorbed, after a finite number of scatterings
+    assert res["counters"]["absorbed"] == n and res["counters"]["cell_crossings"] == 0
+    assert np.all(np.isfinite(res["raw"]["V"]))
+    # per interaction P(dust) = kd / (kd + n sigma H(x)); at line centre that is 0.5 / (0.5 + 3 H(a,0))
+    p0 = 0.5 / (0.5 + tau_cell * oracle.voigt_H(oracle.voigt_a(T), 0.0).item())
+    f0 = np.mean(res["raw"]["nscat"] == 0)
+    assert abs(f0 - p0) < 4 * math.sqrt(p0 * (1 - p0) / n)
+    # empty medium: nothing to interact with, no face to leave through -> capped
+    empty = dict(grid, nHI=one(0), kdust=None)
+    res = oracle.run(empty, src, opts, 50, seed=2)
+    assert res["counters"]["capped"] == 50 and res["counters"]["scatterings"] == 0
