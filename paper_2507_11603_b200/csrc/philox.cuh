@@ -51,4 +51,23 @@ struct Stream {
     __device__ __forceinline__ float uniform() { return u01(next_u32()); }
 };
 
+// The walk kernel's view of the same stream: whole counter blocks.  next4() returns draws 4b..4b+3 of the packet as
+// uniforms and advances b, so every lane of a warp runs the ten rounds at the same program point (the per-draw
+// Stream above regenerates its block on a different call in every lane: 4 of 32 lanes active, 40 % of all issued
+// instructions in the round-1 profile).  Draws a step does not need are skipped, never reused.
+struct BlockRng {
+    uint32_t id_lo, id_hi, b_lo, b_hi;
+
+    __device__ __forceinline__ void init(uint64_t id) {
+        id_lo = (uint32_t)id; id_hi = (uint32_t)(id >> 32); b_lo = 0u; b_hi = 0u;
+    }
+    __device__ __forceinline__ unsigned long long id() const { return ((unsigned long long)id_hi << 32) | id_lo; }
+    __device__ __forceinline__ float4 next4(uint32_t k0, uint32_t k1) {
+        const U4 r = philox4x32_10(b_lo, b_hi, id_lo, id_hi, k0, k1);
+        b_lo += 1u;
+        b_hi += (b_lo == 0u);
+        return make_float4(u01(r.x), u01(r.y), u01(r.z), u01(r.w));
+    }
+};
+
 }  // namespace thor

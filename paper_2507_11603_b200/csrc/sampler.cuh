@@ -14,7 +14,8 @@
 //   C  u > u0       bound e^{-u0^2} L(u);   propose psi = atan2(a, w) uniform in (psi0, pi), u = x - a cot(psi);
 //                   accept with e^{u0^2 - u^2}.                            mass e^{-u0^2} (pi - psi0)/a
 // Piece A (the Gaussian bulk of non-resonant atoms) exists for x >= 1.5; below that B runs from u = -inf with
-// u1^2 := 0 (that is Eq. 10's left piece with a 1/w^2 proposal); for x < 0.05 only C is left (plain Lorentzian).
+// u1^2 := 0 (that is Eq. 10's left piece with a 1/w^2 proposal); for x < 0.3 only C is left (plain Lorentzian,
+// acceptance H(a,x) >= 0.9, and no envelope to set up in the line centre where most scatterings happen).
 // B is written in w, not in the angle, because atan((u-x)/a) + pi/2 cancels catastrophically in fp32 when w >> a.
 // Split rules (any value is exact; these are within ~10 % of the acceptance optimum, 0.2 worst case near x_cw,
 // -> 0.9 in the far wing where Eq. 10 alone falls below 0.1):
@@ -30,19 +31,21 @@ constexpr float SQRT_PI_F = 1.77245385090551602730f;
 
 struct UparEnvelope {
     float xa, a, a2;
-    float u1, u1sq, u0, u0sq;
+    float u1, u1sq, u0sq;
     float inv_w0, inv_w1;     // 1/(x-u0), 1/(x-u1) (0 when B starts at -inf)
     float L1inv;              // (x-u1)^2 + a^2
-    float psi0;
+    float psi0pi;             // atan2(a, x-u0) / pi
     float mA, mAB, mTot;      // cumulative masses
 };
+
+constexpr float UPAR_X_LORENTZ = 0.3f;    // below this a plain Lorentzian proposal accepts with H(a,x) >= 0.9
 
 __device__ __forceinline__ UparEnvelope upar_envelope(float a, float xa) {
     UparEnvelope e;
     e.xa = xa; e.a = a; e.a2 = a * a;
-    if (xa < 0.05f) {                       // C only, uref = 0
-        e.u1 = 0.f; e.u1sq = 0.f; e.u0 = 0.f; e.u0sq = 0.f; e.inv_w0 = 0.f; e.inv_w1 = 0.f; e.L1inv = 1.f;
-        e.psi0 = 0.f; e.mA = 0.f; e.mAB = 0.f; e.mTot = PI_F / a;
+    if (xa < UPAR_X_LORENTZ) {              // C only, u0 = 0: no set-up cost in the line centre
+        e.u1 = 0.f; e.u1sq = 0.f; e.u0sq = 0.f; e.inv_w0 = 0.f; e.inv_w1 = 0.f; e.L1inv = 1.f;
+        e.psi0pi = 0.f; e.mA = 0.f; e.mAB = 0.f; e.mTot = 1.f;
         return e;
     }
     const bool useA = xa >= 1.5f;
@@ -54,61 +57,63 @@ __device__ __forceinline__ UparEnvelope upar_envelope(float a, float xa) {
     const float ucap = sqrtf(__logf(PI_F * fmaxf(xa * xa, 1.f) / a) + 2.f);
     const float u0 = fmaxf(fminf(xa - delta, ucap), 0.f);
     u1 = fminf(u1, u0);
-    e.u0 = u0; e.u0sq = u0 * u0;
+    e.u0sq = u0 * u0;
     e.u1 = u1; e.u1sq = useA ? u1 * u1 : 0.f;
     const float w0 = xa - u0, w1 = xa - u1;
     e.inv_w0 = 1.f / w0;
     e.inv_w1 = useA ? 1.f / w1 : 0.f;
     e.L1inv = w1 * w1 + e.a2;
-    e.psi0 = atan2f(a, w0);
+    e.psi0pi = atan2f(a, w0) * (1.f / PI_F);
     e.mA = useA ? SQRT_PI_F / e.L1inv : 0.f;
     const float mB = __expf(-e.u1sq) * (e.inv_w0 - e.inv_w1);
-    const float mC = __expf(-e.u0sq) * (PI_F - e.psi0) / a;
+    const float mC = __expf(-e.u0sq) * (PI_F * (1.f - e.psi0pi)) / a;
     e.mAB = e.mA + mB;
     e.mTot = e.mAB + mC;
     return e;
 }
 
-// One proposal + accept test.  Returns true and sets u (for x >= 0) on acceptance.
-__device__ __forceinline__ bool upar_try(const UparEnvelope& e, Stream& rng, float& u) {
-    const float r1 = rng.uniform() * e.mTot;
-    const float r2 = rng.uniform();
-    const float r3 = rng.uniform();
-    if (r1 < e.mA) {
-        const float r4 = rng.uniform();
-        const float uu = sqrtf(-__logf(r2)) * cospif(2.f * r3);
-        const float w = e.xa - uu;
+// One proposal + accept test from four uniforms.  Returns true and sets u (for x >= 0) on acceptance.
+__device__ __forceinline__ bool upar_try(const UparEnvelope& e, const float4 r, float& u) {
+    const float r1 = r.x * e.mTot;
+    if (r1 >= e.mAB) {                                   // C: Lorentzian peak and beyond
+        const float t = fmaf(r.y, 1.f - e.psi0pi, e.psi0pi);
+        float s, c;
+        sincospif(t, &s, &c);
+        const float uu = e.xa - e.a * c / s;
         u = uu;
-        return uu <= e.u1 && r4 * (w * w + e.a2) <= e.L1inv;
-    } else if (r1 < e.mAB) {
-        const float iw = fmaf(r2, e.inv_w0 - e.inv_w1, e.inv_w1);
+        return r.z <= __expf(e.u0sq - uu * uu);
+    } else if (r1 >= e.mA) {                             // B
+        const float iw = fmaf(r.y, e.inv_w0 - e.inv_w1, e.inv_w1);
         const float w = 1.f / iw;
         const float uu = e.xa - w;
         const float w2 = w * w;
         u = uu;
-        return r3 * (w2 + e.a2) <= __expf(e.u1sq - uu * uu) * w2;
-    } else {
-        const float psi = fmaf(r2, PI_F - e.psi0, e.psi0);
-        float s, c;
-        sincosf(psi, &s, &c);
-        const float uu = e.xa - e.a * c / s;
+        return r.z * (w2 + e.a2) <= __expf(e.u1sq - uu * uu) * w2;
+    } else {                                             // A: Gaussian bulk
+        const float uu = sqrtf(-__logf(r.y)) * cospif(2.f * r.z);
+        const float w = e.xa - uu;
         u = uu;
-        return r3 <= __expf(e.u0sq - uu * uu);
+        return uu <= e.u1 && r.w * (w * w + e.a2) <= e.L1inv;
     }
 }
 
-__device__ __forceinline__ float sample_upar(float a, float x, Stream& rng, uint32_t& iters) {
+// One counter block per iteration; every lane of the warp generates its block at the same program point.
+__device__ __forceinline__ float sample_upar(float a, float x, BlockRng& rng, uint32_t k0, uint32_t k1,
+                                             uint32_t& iters) {
     const UparEnvelope e = upar_envelope(a, fabsf(x));
     float u;
-    uint32_t guard = 0;                      // fail-safe: acceptance is >= ~0.15 everywhere, 2^20 rejections cannot
-    do { ++iters; } while (!upar_try(e, rng, u) && ++guard < (1u << 20));   // happen unless x is NaN; never hang
+    uint32_t guard = 0;                      // fail-safe: acceptance is >= ~0.2 everywhere, 2^20 rejections cannot
+    bool ok;                                 // happen unless x is NaN; never hang the GPU
+    do {
+        ++iters;
+        ok = upar_try(e, rng.next4(k0, k1), u);
+    } while (!ok && ++guard < (1u << 20));
     return x < 0.f ? -u : u;
 }
 
 // Eq. 5 in polar form: magnitude m = sqrt(-ln r1) (or sqrt(x_crit^2 - ln r1) when |x_in| < x_crit),
 // angle 2 pi r2.
-__device__ __forceinline__ void sample_uperp(float x_in, float x_crit, Stream& rng, float& up1, float& up2) {
-    const float r1 = rng.uniform(), r2 = rng.uniform();
+__device__ __forceinline__ void sample_uperp(float x_in, float x_crit, float r1, float r2, float& up1, float& up2) {
     const float shift = fabsf(x_in) < x_crit ? x_crit * x_crit : 0.f;
     const float m = sqrtf(shift - __logf(r1));
     float s, c;
@@ -127,12 +132,11 @@ __device__ __forceinline__ float dipole_mu(float r) {
     return B < 0.f ? -m : m;
 }
 
-// phase: 0 isotropic, 1 dipole, 2 = 1/3 isotropic + 2/3 dipole, one extra draw for the mix.
-__device__ __forceinline__ float sample_mu(int phase, Stream& rng, bool& is_dipole) {
+// phase: 0 isotropic, 1 dipole, 2 = 1/3 isotropic + 2/3 dipole; r_mix decides the mix, r gives mu.
+__device__ __forceinline__ float sample_mu(int phase, float r_mix, float r, bool& is_dipole) {
     int ph = phase;
-    if (phase == 2) ph = rng.uniform() < (1.f / 3.f) ? 0 : 1;
+    if (phase == 2) ph = r_mix < (1.f / 3.f) ? 0 : 1;
     is_dipole = ph == 1;
-    const float r = rng.uniform();
     const float mu = is_dipole ? dipole_mu(r) : fmaf(2.f, r, -1.f);
     return fminf(fmaxf(mu, -1.f), 1.f);
 }

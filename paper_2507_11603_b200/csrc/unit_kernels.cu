@@ -76,16 +76,18 @@ __global__ void unit_scatter_kernel(float a, float x_in, float x_crit, int phase
                                     long long n, float* u_par, float* x_out, float* k_out, uint32_t* iters) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    Stream rng;
-    rng.init(seed, id0 + (uint64_t)i);
+    BlockRng rng;
+    rng.init(id0 + (uint64_t)i);
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     uint32_t it = 0;
-    const float upar = sample_upar(a, x_in, rng, it);
+    const float4 s1 = rng.next4(k0, k1), s2 = rng.next4(k0, k1);        // same draw layout as walk_kernel
+    const float upar = sample_upar(a, x_in, rng, k0, k1, it);
     float up1, up2;
-    sample_uperp(x_in, x_crit, rng, up1, up2);
+    sample_uperp(x_in, x_crit, s1.w, s2.x, up1, up2);
     bool dip;
-    const float mu = sample_mu(phase, rng, dip);
+    const float mu = sample_mu(phase, s2.z, s1.y, dip);
     float sph, cph;
-    sincospif(2.f * rng.uniform(), &sph, &cph);
+    sincospif(2.f * s1.z, &sph, &cph);
     float e1[3], e2[3];
     ortho_basis(0.f, 0.f, 1.f, e1, e2);
     const float st = sqrtf(fmaxf(0.f, 1.f - mu * mu));

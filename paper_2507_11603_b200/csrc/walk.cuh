@@ -14,45 +14,61 @@ namespace thor {
 
 enum : int { LS_IDLE = 0, LS_MARCH = 1, LS_SCATTER = 2, LS_OUT = 3 };
 
-struct CellProps { float n, T, vx, vy, vz, kd; };
+// a5 cell gather + derived per-cell quantities (one MUFU.RSQ): SoA fp32 fields through the read-only path.  A packet
+// keeps the Cell of the cell it is in (registers) until it crosses a face: in optically thick cells a packet
+// scatters thousands of times between crossings and re-gathers nothing.
+struct Cell {
+    float a;         // Voigt parameter
+    float vth;       // km/s
+    float inv_vth;
+    float nsig;      // n sigma_0(T) cell_cm: line-centre optical depth per cell length (0 in empty cells)
+    float kd;        // dust absorption optical depth per cell length
+    float vx, vy, vz;
+};
 
-// a5 cell gather: SoA fp32 fields through the read-only path.
-__device__ __forceinline__ CellProps fetch_cell(const WalkParams& p, int64_t i) {
-    CellProps c;
-    c.n = __ldg(p.nHI + i); c.T = __ldg(p.T + i);
+__device__ __forceinline__ Cell load_cell(const WalkParams& p, int64_t i) {
+    Cell c;
+    const float n = __ldg(p.nHI + i), T = __ldg(p.T + i);
     c.vx = __ldg(p.vx + i); c.vy = __ldg(p.vy + i); c.vz = __ldg(p.vz + i);
     c.kd = p.kdust ? __ldg(p.kdust + i) * p.cell_cm : 0.f;
+    const float rs = rsqrtf(T);
+    c.a = p.c_a * rs;
+    c.inv_vth = p.inv_c_vth * rs;
+    c.vth = p.c_vth * (T * rs);
+    c.nsig = n > 0.f ? n * p.sig_cell * rs : 0.f;
     return c;
-}
-
-// Derived per-cell quantities (one MUFU.RSQ): a, 1/v_th, v_th, n sigma_0 cell_cm.
-struct CellDerived { float a, vth, inv_vth, nsig; };
-__device__ __forceinline__ CellDerived derive_cell(const WalkParams& p, const CellProps& c) {
-    CellDerived d;
-    const float rs = rsqrtf(c.T);
-    d.a = p.c_a * rs;
-    d.inv_vth = p.inv_c_vth * rs;
-    d.vth = p.c_vth * (c.T * rs);
-    d.nsig = c.n > 0.f ? c.n * p.sig_cell * rs : 0.f;
-    return d;
 }
 
 // a6/a7: optical depth of one segment of length len (cell units) starting at velocity offset V0, or the distance
 // s_hit at which tau_need is reached (linear within the step).  Without Hubble drift: kappa len.
 // With drift Hc (km/s per cell length): sub-steps per reading A12 — n_sub = 1 if min|x| over the segment > 6 else
-// ceil(|dV| / (eps v_th)), midpoint rule.  Returns true on interaction; k_line/k_tot are the opacities there.
-__device__ __forceinline__ bool integrate_segment(const WalkParams& p, const float2* s_tab, const CellProps& c,
-                                                  const CellDerived& d, float V0, float vk, float len, float tau_need,
-                                                  float& tau_out, float& s_hit, float& k_line, float& k_tot) {
-    tau_out = 0.f; s_hit = 0.f; k_line = 0.f; k_tot = 0.f;
-    if (c.n <= 0.f && c.kd <= 0.f) return false;
+// ceil(|dV| / (eps v_th)), midpoint rule.  Returns true on interaction; k_tot is the opacity there.
+template <bool HUBBLE>
+__device__ __forceinline__ bool integrate_segment(const WalkParams& p, const float2* s_tab, const Cell& c, float V0,
+                                                  float vk, float len, float tau_need, float& tau_out, float& s_hit,
+                                                  float& k_tot) {
+    tau_out = 0.f; s_hit = 0.f; k_tot = 0.f;
+    if (c.nsig <= 0.f && c.kd <= 0.f) return false;
+    if (!HUBBLE) {
+        const float kl = c.nsig > 0.f ? c.nsig * voigt_H(s_tab, c.a, (V0 - vk) * c.inv_vth) : 0.f;
+        const float kt = kl + c.kd;
+        const float dtau = kt * len;
+        if (dtau >= tau_need && kt > 0.f) {
+            s_hit = fminf(tau_need / kt, len);
+            k_tot = kt;
+            tau_out = tau_need;
+            return true;
+        }
+        tau_out = dtau;
+        return false;
+    }
     const float Hc = p.hubble;
     int nsub = 1;
-    if (Hc != 0.f && c.n > 0.f && len > 0.f) {
-        const float xa = (V0 - vk) * d.inv_vth, xb = (V0 - Hc * len - vk) * d.inv_vth;
+    if (Hc != 0.f && c.nsig > 0.f && len > 0.f) {
+        const float xa = (V0 - vk) * c.inv_vth, xb = (V0 - Hc * len - vk) * c.inv_vth;
         const float minabs = xa * xb <= 0.f ? 0.f : fminf(fabsf(xa), fabsf(xb));
         if (minabs <= 6.f) {
-            const float q = ceilf(fabsf(Hc * len) * d.inv_vth / p.hubble_eps);
+            const float q = ceilf(fabsf(Hc * len) * c.inv_vth / p.hubble_eps);
             nsub = q < 1.f ? 1 : (q > 1e6f ? 1000000 : (int)q);
         }
     }
@@ -60,12 +76,12 @@ __device__ __forceinline__ bool integrate_segment(const WalkParams& p, const flo
     float tau = 0.f;
     for (int j = 0; j < nsub; ++j) {
         const float Vmid = Hc != 0.f ? V0 - Hc * ((float)j + 0.5f) * ds : V0;   // no 0 * inf when ds = +inf (A24)
-        const float kl = c.n > 0.f ? d.nsig * voigt_H(s_tab, d.a, (Vmid - vk) * d.inv_vth) : 0.f;
+        const float kl = c.nsig > 0.f ? c.nsig * voigt_H(s_tab, c.a, (Vmid - vk) * c.inv_vth) : 0.f;
         const float kt = kl + c.kd;
         const float dtau = kt * ds;
         if (tau + dtau >= tau_need && kt > 0.f) {
             s_hit = fminf((j ? (float)j * ds : 0.f) + (tau_need - tau) / kt, len);
-            k_line = kl; k_tot = kt;
+            k_tot = kt;
             tau_out = tau_need;
             return true;
         }
@@ -78,6 +94,7 @@ __device__ __forceinline__ bool integrate_segment(const WalkParams& p, const flo
 // a12 peel-off: w = P^ exp(-tau_obs), tau_obs integrated from `at` along k_obs to the box face at
 // velocity offset V_o by the same march (a4-a6), dropped beyond tau_peel_max (reading A13); added to
 // (pixel of the starting point projected perpendicular to k_obs, spectral bin of dv = -V at the box face).
+template <bool HUBBLE>
 __device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, const Ray& at, float V_o, float phat,
                                       uint32_t& n_cells) {
     const float px0 = (float)at.cx + at.fx - 0.5f * (float)p.g.nx;
@@ -93,13 +110,12 @@ __device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, 
         float len;
         const int ex = dda_next_face(r, p.g, len);
         if (!(len < CUDART_INF_F)) return;                    // reading A24: never reaches a box face -> dropped
-        const CellProps c = fetch_cell(p, dda_linear(r, p.g));
-        const CellDerived d = derive_cell(p, c);
+        const Cell c = load_cell(p, dda_linear(r, p.g));
         const float vk = c.vx * r.kx + c.vy * r.ky + c.vz * r.kz;
-        float dtau, s_hit, kl, kt;
-        integrate_segment(p, s_tab, c, d, V, vk, len, 3.0e38f, dtau, s_hit, kl, kt);
+        float dtau, s_hit, kt;
+        integrate_segment<HUBBLE>(p, s_tab, c, V, vk, len, 3.0e38f, dtau, s_hit, kt);
         tau += dtau;
-        V -= p.hubble * len;
+        if (HUBBLE) V -= p.hubble * len;
         ++n_cells;
         if (tau > p.tau_peel_max) return;
         // peel rays leave through the first box face they meet, periodic or not
