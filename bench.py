@@ -39,7 +39,7 @@ def make_workload(name, n_photons=None):
     if name == "shell":      # BASELINE.json configs[1]
         w = W.expanding_shell(n=128, n_photons=1_000_000)
     elif name == "sphere":   # configs[0] scaled to fill the GPU (same physics, more packets), tau0 = 1e4
-        w = W.static_sphere(n=32, tau0=1e4, T=10.0, n_photons=200_000)
+        w = W.static_sphere(n=32, tau0=1e4, T=10.0, n_photons=1_000_000)
     elif name == "slab":     # configs[2]
         w = W.static_slab(n_photons=1_000_000)
     elif name == "turb":     # configs[3] at 256^3

@@ -8,7 +8,10 @@ SOURCES = ["api.cu", "walk.cu", "unit_kernels.cu"]
 DEPS = SOURCES + ["walk.cuh", "params.cuh", "philox.cuh", "dda.cuh", "voigt.cuh", "voigt_table.inc", "sampler.cuh",
                   os.path.join("..", "..", "include", "thor.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--shared",
-              "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-cudart", "shared"]
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-cudart", "shared",
+              # approximate (2 ulp) division and square root for the samplers; the DDA and Voigt use explicit
+              # __fdiv_rn / __fmul_rn / __fadd_rn / __frcp_rn intrinsics, which these flags do not touch
+              "-prec-div=false", "-prec-sqrt=false"]
 
 
 def build(force=False, verbose=False):

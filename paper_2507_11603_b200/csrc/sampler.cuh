@@ -29,43 +29,52 @@ namespace thor {
 constexpr float PI_F = 3.14159265358979323846f;
 constexpr float SQRT_PI_F = 1.77245385090551602730f;
 
+// The envelope of one scattering, kept in registers while the packet is in its rejection trials (walk_kernel runs
+// ONE trial per loop iteration for every lane that still needs one, instead of an inner loop the whole warp waits on).
 struct UparEnvelope {
-    float xa, a, a2;
-    float u1, u1sq, u0sq;
+    float xa;                 // |x_in|
+    float u1, u0sq;
     float inv_w0, inv_w1;     // 1/(x-u0), 1/(x-u1) (0 when B starts at -inf)
-    float L1inv;              // (x-u1)^2 + a^2
-    float psi0pi;             // atan2(a, x-u0) / pi
+    float psi0pi;             // atan(a / (x-u0)) / pi
     float mA, mAB, mTot;      // cumulative masses
 };
 
 constexpr float UPAR_X_LORENTZ = 0.3f;    // below this a plain Lorentzian proposal accepts with H(a,x) >= 0.9
 
+// atan(y) for 0 <= y <= 0.5 (4.7e-8 relative): y P(y^2), minimax fit; atanf beyond (a / w0 > 0.5 needs a > 0.02).
+__device__ __forceinline__ float atan_small(float y) {
+    if (y > 0.5f) return atanf(y);
+    const float z = y * y;
+    const float pz = fmaf(z, fmaf(z, fmaf(z, fmaf(z, fmaf(z, -5.201264606e-02f, 1.019391841e-01f), -1.418004712e-01f),
+                                          1.999438943e-01f), -3.333322389e-01f), 9.999999966e-01f);
+    return y * pz;
+}
+
 __device__ __forceinline__ UparEnvelope upar_envelope(float a, float xa) {
     UparEnvelope e;
-    e.xa = xa; e.a = a; e.a2 = a * a;
+    e.xa = xa;
     if (xa < UPAR_X_LORENTZ) {              // C only, u0 = 0: no set-up cost in the line centre
-        e.u1 = 0.f; e.u1sq = 0.f; e.u0sq = 0.f; e.inv_w0 = 0.f; e.inv_w1 = 0.f; e.L1inv = 1.f;
+        e.u1 = 0.f; e.u0sq = 0.f; e.inv_w0 = 0.f; e.inv_w1 = 0.f;
         e.psi0pi = 0.f; e.mA = 0.f; e.mAB = 0.f; e.mTot = 1.f;
         return e;
     }
     const bool useA = xa >= 1.5f;
     float u1 = useA ? fminf(sqrtf(__logf(xa) + 1.4f), xa - 0.4f) : 0.f;
-    const float u1sq_rule = u1 * u1;
-    const float q = a * __expf(fminf(xa * xa - u1sq_rule, 40.f)) / (2.f * PI_F * xa);
+    const float q = a * __expf(fminf(xa * xa - u1 * u1, 40.f)) / (2.f * PI_F * xa);
     const float d0 = sqrtf(q);
     const float delta = d0 / (1.f + xa * d0);
-    const float ucap = sqrtf(__logf(PI_F * fmaxf(xa * xa, 1.f) / a) + 2.f);
-    const float u0 = fmaxf(fminf(xa - delta, ucap), 0.f);
+    float u0 = xa - delta;
+    if (useA) u0 = fminf(u0, sqrtf(__logf(PI_F * xa * xa / a) + 2.f));   // the cap never binds below x = 1.5
+    u0 = fmaxf(u0, 0.f);
     u1 = fminf(u1, u0);
     e.u0sq = u0 * u0;
-    e.u1 = u1; e.u1sq = useA ? u1 * u1 : 0.f;
+    e.u1 = u1;
     const float w0 = xa - u0, w1 = xa - u1;
     e.inv_w0 = 1.f / w0;
     e.inv_w1 = useA ? 1.f / w1 : 0.f;
-    e.L1inv = w1 * w1 + e.a2;
-    e.psi0pi = atan2f(a, w0) * (1.f / PI_F);
-    e.mA = useA ? SQRT_PI_F / e.L1inv : 0.f;
-    const float mB = __expf(-e.u1sq) * (e.inv_w0 - e.inv_w1);
+    e.psi0pi = atan_small(a * e.inv_w0) * (1.f / PI_F);
+    e.mA = useA ? SQRT_PI_F / (w1 * w1 + a * a) : 0.f;
+    const float mB = __expf(-u1 * u1) * (e.inv_w0 - e.inv_w1);
     const float mC = __expf(-e.u0sq) * (PI_F * (1.f - e.psi0pi)) / a;
     e.mAB = e.mA + mB;
     e.mTot = e.mAB + mC;
@@ -73,13 +82,14 @@ __device__ __forceinline__ UparEnvelope upar_envelope(float a, float xa) {
 }
 
 // One proposal + accept test from four uniforms.  Returns true and sets u (for x >= 0) on acceptance.
-__device__ __forceinline__ bool upar_try(const UparEnvelope& e, const float4 r, float& u) {
+__device__ __forceinline__ bool upar_try(const UparEnvelope& e, float a, const float4 r, float& u) {
     const float r1 = r.x * e.mTot;
+    const float a2 = a * a;
     if (r1 >= e.mAB) {                                   // C: Lorentzian peak and beyond
         const float t = fmaf(r.y, 1.f - e.psi0pi, e.psi0pi);
         float s, c;
         sincospif(t, &s, &c);
-        const float uu = e.xa - e.a * c / s;
+        const float uu = e.xa - a * c / s;
         u = uu;
         return r.z <= __expf(e.u0sq - uu * uu);
     } else if (r1 >= e.mA) {                             // B
@@ -88,16 +98,16 @@ __device__ __forceinline__ bool upar_try(const UparEnvelope& e, const float4 r, 
         const float uu = e.xa - w;
         const float w2 = w * w;
         u = uu;
-        return r.z * (w2 + e.a2) <= __expf(e.u1sq - uu * uu) * w2;
+        return r.z * (w2 + a2) <= __expf(e.u1 * e.u1 - uu * uu) * w2;
     } else {                                             // A: Gaussian bulk
         const float uu = sqrtf(-__logf(r.y)) * cospif(2.f * r.z);
-        const float w = e.xa - uu;
+        const float w = e.xa - uu, w1 = e.xa - e.u1;
         u = uu;
-        return uu <= e.u1 && r.w * (w * w + e.a2) <= e.L1inv;
+        return uu <= e.u1 && r.w * (w * w + a2) <= w1 * w1 + a2;
     }
 }
 
-// One counter block per iteration; every lane of the warp generates its block at the same program point.
+// Whole rejection loop for one variate (unit kernel); one counter block per trial.
 __device__ __forceinline__ float sample_upar(float a, float x, BlockRng& rng, uint32_t k0, uint32_t k1,
                                              uint32_t& iters) {
     const UparEnvelope e = upar_envelope(a, fabsf(x));
@@ -106,7 +116,7 @@ __device__ __forceinline__ float sample_upar(float a, float x, BlockRng& rng, ui
     bool ok;                                 // happen unless x is NaN; never hang the GPU
     do {
         ++iters;
-        ok = upar_try(e, rng.next4(k0, k1), u);
+        ok = upar_try(e, a, rng.next4(k0, k1), u);
     } while (!ok && ++guard < (1u << 20));
     return x < 0.f ? -u : u;
 }

@@ -5,8 +5,18 @@
 
 namespace thor {
 
-constexpr int WALK_THREADS = 256;
+#ifndef THOR_WALK_THREADS
+#define THOR_WALK_THREADS 256
+#endif
+#ifndef THOR_WALK_MIN_CTAS
+#define THOR_WALK_MIN_CTAS 3
+#endif
+#ifndef THOR_FINISH_MIN_LANES
+#define THOR_FINISH_MIN_LANES 24
+#endif
+constexpr int WALK_THREADS = THOR_WALK_THREADS;
 constexpr int MAX_SPEC_BINS = 4096;
+constexpr int FINISH_MIN_LANES = THOR_FINISH_MIN_LANES;
 
 struct BlockTallies {
     float2 voigt[VOIGT_NODES];
@@ -35,7 +45,7 @@ __device__ __forceinline__ void tally_finish(const WalkParams& p, BlockTallies& 
 }
 
 template <bool HUBBLE, bool PEEL>
-__global__ void __launch_bounds__(WALK_THREADS, 2) walk_kernel(const __grid_constant__ WalkParams p) {
+__global__ void __launch_bounds__(WALK_THREADS, PEEL ? 2 : THOR_WALK_MIN_CTAS) walk_kernel(const __grid_constant__ WalkParams p) {
     __shared__ BlockTallies sh;
     voigt_table_load(sh.voigt);
     for (int i = threadIdx.x; i < N_COUNTERS; i += blockDim.x) sh.counters[i] = 0ull;
@@ -50,7 +60,10 @@ __global__ void __launch_bounds__(WALK_THREADS, 2) walk_kernel(const __grid_cons
     BlockRng rng;
     Cell cell;                                                // the cell the packet is in (valid unless `stale`)
     bool stale = true;
-    float V = 0.f, tau_rem = 0.f, hit_kt = 0.f;
+    float V = 0.f, tau_rem = 0.f, hit_kt = 0.f, x_in = 0.f, upar = 0.f;
+    UparEnvelope env;
+    env.mTot = -1.f;
+    uint32_t trials = 0;
     uint32_t nscat = 0, crossings = 0, rej_iters = 0, peel_rays = 0, peel_cells = 0;
     bool more = true;                                         // warp-uniform: photon counter not yet exhausted
 
@@ -107,7 +120,10 @@ __global__ void __launch_bounds__(WALK_THREADS, 2) walk_kernel(const __grid_cons
                 dda_advance_within(ray, p.g, s_hit);
                 if (HUBBLE) { if (p.hubble != 0.f) V -= p.hubble * s_hit; }
                 hit_kt = kt;
-                state = LS_SCATTER;
+                x_in = (V - vk) * cell.inv_vth;
+                env.mTot = -1.f;                                  // envelope not built yet
+                trials = 0u;
+                state = LS_TRIAL;
             } else if (!(len < CUDART_INF_F)) {
                 // reading A24: infinite segment (ray parallel to every non-frozen axis) without interaction: the
                 // packet can neither leave nor be followed -> capped
@@ -128,16 +144,29 @@ __global__ void __launch_bounds__(WALK_THREADS, 2) walk_kernel(const __grid_cons
             }
         }
 
-        // ---- a7-a11: interact.  Deferred while most lanes are still marching, so that scatterers run together ----
-        const unsigned want = __ballot_sync(0xffffffffu, state == LS_SCATTER);
-        const unsigned still = __ballot_sync(0xffffffffu, state == LS_MARCH);
-        if (!(want | still)) {
+        // ---- a8: ONE rejection trial of u_par for every lane that needs one.  No inner loop: a
+        // lane whose trial is rejected tries again in the next iteration, alongside the lanes that arrive from the
+        // march, instead of the whole warp waiting for its slowest lane (the paper's "largest source of thread
+        // divergence"; E[max of 32 iterations]/E[iterations] = 2.1-4.2) ----
+        if (state == LS_TRIAL) {
+            if (env.mTot < 0.f) env = upar_envelope(cell.a, fabsf(x_in));
+            ++rej_iters;
+            float u;
+            const bool ok = upar_try(env, cell.a, rng.next4(k0, k1), u);
+            // fail-safe: acceptance is >= ~0.2 everywhere; 2^20 rejections cannot happen unless x is NaN
+            if (ok || ++trials >= (1u << 20)) { upar = x_in < 0.f ? -u : u; state = LS_FINISH; }
+        }
+
+        // ---- a7, a9-a12: finish the interaction.  The most expensive section: deferred until enough lanes want it ----
+        const unsigned fin = __ballot_sync(0xffffffffu, state == LS_FINISH);
+        const unsigned busy = __ballot_sync(0xffffffffu, state == LS_MARCH || state == LS_TRIAL);
+        if (!(fin | busy)) {
             if (!more) break;
             continue;
         }
-        if (want && (__popc(want) >= __popc(still) || __popc(want) >= 8)) {
-            if (state == LS_SCATTER) {
-                // draws of this event: (tau, mu, phi, perp1), (perp2, dust, mix, -); u_par takes one block per trial
+        if (fin && (__popc(fin) >= __popc(busy) || __popc(fin) >= FINISH_MIN_LANES)) {
+            if (state == LS_FINISH) {
+                // draws of this event: (tau, mu, phi, perp1), (perp2, dust, mix, -)
                 const float4 s1 = rng.next4(k0, k1), s2 = rng.next4(k0, k1);
                 // a7 interaction kind: dust with probability kappa_dust / kappa_total
                 if (p.kdust && s2.y * hit_kt < cell.kd) {
@@ -145,14 +174,12 @@ __global__ void __launch_bounds__(WALK_THREADS, 2) walk_kernel(const __grid_cons
                     state = LS_IDLE;
                 } else {
                     const float kx = ray.kx, ky = ray.ky, kz = ray.kz;
-                    const float x_in = (V - (cell.vx * kx + cell.vy * ky + cell.vz * kz)) * cell.inv_vth;
                     float x_crit = 0.f;
                     if (p.core_skip_mode == 1) x_crit = p.x_crit;
                     else if (p.core_skip_mode == 2) {              // local: a tau_0 over half a cell (reading A7)
                         const float atau = cell.a * cell.nsig * 0.5f;
                         x_crit = atau >= 1.f ? 0.2f * cbrtf(atau) : 0.f;
                     }
-                    const float upar = sample_upar(cell.a, x_in, rng, k0, k1, rej_iters);
                     float up1, up2;
                     sample_uperp(x_in, x_crit, s1.w, s2.x, up1, up2);
                     const float xsel = p.phase_frame == 0 ? fabsf(x_in - upar) : fabsf(x_in);

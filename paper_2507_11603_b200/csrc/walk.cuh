@@ -12,7 +12,7 @@
 
 namespace thor {
 
-enum : int { LS_IDLE = 0, LS_MARCH = 1, LS_SCATTER = 2, LS_OUT = 3 };
+enum : int { LS_IDLE = 0, LS_MARCH = 1, LS_TRIAL = 2, LS_FINISH = 3, LS_OUT = 4 };
 
 // a5 cell gather + derived per-cell quantities (one MUFU.RSQ): SoA fp32 fields through the read-only path.  A packet
 // keeps the Cell of the cell it is in (registers) until it crosses a face: in optically thick cells a packet
