@@ -25,8 +25,10 @@ __device__ __forceinline__ U4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c
 }
 
 // u32 -> uniform in the open interval (0,1): ((r >> 9) + 0.5) 2^-23 (reading A8).  23 bits: k + 1/2 with k < 2^23 is
-// exact in fp32 (24 bits would round k + 1/2 to even for k >= 2^23 and could return exactly 0.5 or 1.0).
-__device__ __forceinline__ float u01(uint32_t r) { return ((float)(r >> 9) + 0.5f) * 1.1920928955078125e-7f; }
+// exact in fp32 (24 bits would round k + 1/2 to even for k >= 2^23 and could return exactly 0.5 or 1.0).  Formed
+// without an int->float conversion: the bits 0x3F800000 | k are the float 1 + k 2^-23, and subtracting 1 - 2^-24
+// (representable) leaves (k + 1/2) 2^-23 exactly.
+__device__ __forceinline__ float u01(uint32_t r) { return __uint_as_float((r >> 9) | 0x3F800000u) - 0.99999994039535522f; }
 
 // One packet's draw stream.  Four cached words + the draw index; draw d is word d & 3 of block d >> 2.
 struct Stream {

@@ -19,8 +19,9 @@
 // B is written in w, not in the angle, because atan((u-x)/a) + pi/2 cancels catastrophically in fp32 when w >> a.
 // Split rules (any value is exact; these are within ~10 % of the acceptance optimum, 0.2 worst case near x_cw,
 // -> 0.9 in the far wing where Eq. 10 alone falls below 0.1):
-//   u1 = min(sqrt(ln x + 1.4), x - 0.4),  delta0 = sqrt(a e^{x^2 - u1^2} / (2 pi x)),  delta = delta0/(1 + x delta0),
+//   u1 = min(1.9 + 0.03 x, x - 0.45),  delta0 = sqrt(a e^{x^2 - u1^2} / (2 pi x)),  delta = delta0/(1 + x delta0),
 //   u0 = min(x - delta, sqrt(ln(pi x^2 / a) + 2)).
+// Piece A's bound is exponentially tilted (see upar_envelope): the proposal is N(beta, 1/2), not N(0, 1/2).
 #pragma once
 #include "philox.cuh"
 
@@ -33,13 +34,24 @@ constexpr float SQRT_PI_F = 1.77245385090551602730f;
 // ONE trial per loop iteration for every lane that still needs one, instead of an inner loop the whole warp waits on).
 struct UparEnvelope {
     float xa;                 // |x_in|
-    float u1, u0sq;
+    float u1, u0sq, beta;
     float inv_w0, inv_w1;     // 1/(x-u0), 1/(x-u1) (0 when B starts at -inf)
     float psi0pi;             // atan(a / (x-u0)) / pi
     float mA, mAB, mTot;      // cumulative masses
 };
 
 constexpr float UPAR_X_LORENTZ = 0.3f;    // below this a plain Lorentzian proposal accepts with H(a,x) >= 0.9
+constexpr float UPAR_U_MIN = -4.5f;       // left end of piece A (see below)
+constexpr float TWO_PI_F = 6.28318530717958647692f;
+
+// sin / cos of the uniform random angle 2 pi r, r in (0,1): MUFU.SIN/COS on the reduced argument 2 pi (r - 1/2) in
+// (-pi, pi), negated (a half-turn); absolute error ~5e-7, far below the 2^-23 grain of r.
+__device__ __forceinline__ void sincos_uniform(float r, float& s, float& c) {
+    float s1, c1;
+    __sincosf(TWO_PI_F * (r - 0.5f), &s1, &c1);
+    s = -s1; c = -c1;
+}
+__device__ __forceinline__ float cos_uniform(float r) { return -__cosf(TWO_PI_F * (r - 0.5f)); }
 
 // atan(y) for 0 <= y <= 0.5 (4.7e-8 relative): y P(y^2), minimax fit; atanf beyond (a / w0 > 0.5 needs a > 0.02).
 __device__ __forceinline__ float atan_small(float y) {
@@ -50,19 +62,28 @@ __device__ __forceinline__ float atan_small(float y) {
     return y * pz;
 }
 
+// Piece A with an exponentially tilted bound.  On u <= u1 the Lorentzian factor L(u) = 1/((x-u)^2 + a^2) grows with
+// u; Eq. 10's constant bound L(u1) wastes a factor (x/(x-u1))^2 on the bulk of the Gaussian.  ln L is convex in u,
+// so with s = u1 - u, f(s) = ln(L(u1)/L(u)) is concave with f(0) = 0 and f(s) >= s f(s_max)/s_max on [0, s_max]:
+//     L(u) <= L(u1) exp(2 beta (u - u1)),   beta = f(s_max) / (2 s_max),   u in [UPAR_U_MIN, u1],  s_max = u1 - UPAR_U_MIN.
+// e^{-u^2} e^{2 beta u} is a Gaussian of mean beta: propose u ~ N(beta, 1/2), reject outside [UPAR_U_MIN, u1], accept
+// with L(u) / (L(u1) e^{2 beta (u - u1)}).  Mass sqrt(pi) L(u1) e^{beta^2 - 2 beta u1}.  Acceptance in the wings rises
+// from 0.25-0.55 to 0.5-0.8 (x = 4 ... 8).  The Gaussian mass left of UPAR_U_MIN is < 1e-9 of the piece: below the
+// 2^-23 grain of the uniform that picks the piece, so no separate piece can ever be selected for it.
 __device__ __forceinline__ UparEnvelope upar_envelope(float a, float xa) {
     UparEnvelope e;
     e.xa = xa;
     if (xa < UPAR_X_LORENTZ) {              // C only, u0 = 0: no set-up cost in the line centre
-        e.u1 = 0.f; e.u0sq = 0.f; e.inv_w0 = 0.f; e.inv_w1 = 0.f;
+        e.u1 = 0.f; e.u0sq = 0.f; e.beta = 0.f; e.inv_w0 = 0.f; e.inv_w1 = 0.f;
         e.psi0pi = 0.f; e.mA = 0.f; e.mAB = 0.f; e.mTot = 1.f;
         return e;
     }
     const bool useA = xa >= 1.5f;
-    float u1 = useA ? fminf(sqrtf(__logf(xa) + 1.4f), xa - 0.4f) : 0.f;
-    const float q = a * __expf(fminf(xa * xa - u1 * u1, 40.f)) / (2.f * PI_F * xa);
+    const float a2 = a * a;
+    float u1 = useA ? fminf(fmaf(0.03f, xa, 1.9f), xa - 0.45f) : 0.f;
+    const float q = a * __expf(fminf(xa * xa - u1 * u1, 40.f)) / (TWO_PI_F * xa);
     const float d0 = sqrtf(q);
-    const float delta = d0 / (1.f + xa * d0);
+    const float delta = d0 / fmaf(xa, d0, 1.f);
     float u0 = xa - delta;
     if (useA) u0 = fminf(u0, sqrtf(__logf(PI_F * xa * xa / a) + 2.f));   // the cap never binds below x = 1.5
     u0 = fmaxf(u0, 0.f);
@@ -71,12 +92,19 @@ __device__ __forceinline__ UparEnvelope upar_envelope(float a, float xa) {
     e.u1 = u1;
     const float w0 = xa - u0, w1 = xa - u1;
     e.inv_w0 = 1.f / w0;
-    e.inv_w1 = useA ? 1.f / w1 : 0.f;
     e.psi0pi = atan_small(a * e.inv_w0) * (1.f / PI_F);
-    e.mA = useA ? SQRT_PI_F / (w1 * w1 + a * a) : 0.f;
-    const float mB = __expf(-u1 * u1) * (e.inv_w0 - e.inv_w1);
     const float mC = __expf(-e.u0sq) * (PI_F * (1.f - e.psi0pi)) / a;
-    e.mAB = e.mA + mB;
+    if (useA) {
+        const float smax = u1 - UPAR_U_MIN, ws = w1 + smax;
+        const float L1inv = fmaf(w1, w1, a2);
+        e.inv_w1 = 1.f / w1;
+        e.beta = __logf(fmaf(ws, ws, a2) / L1inv) / (2.f * smax);
+        e.mA = SQRT_PI_F * __expf(e.beta * (e.beta - 2.f * u1)) / L1inv;
+        e.mAB = fmaf(__expf(-u1 * u1), e.inv_w0 - e.inv_w1, e.mA);
+    } else {
+        e.inv_w1 = 0.f; e.beta = 0.f; e.mA = 0.f;
+        e.mAB = e.inv_w0;
+    }
     e.mTot = e.mAB + mC;
     return e;
 }
@@ -99,11 +127,12 @@ __device__ __forceinline__ bool upar_try(const UparEnvelope& e, float a, const f
         const float w2 = w * w;
         u = uu;
         return r.z * (w2 + a2) <= __expf(e.u1 * e.u1 - uu * uu) * w2;
-    } else {                                             // A: Gaussian bulk
-        const float uu = sqrtf(-__logf(r.y)) * cospif(2.f * r.z);
+    } else {                                             // A: Gaussian bulk, tilted bound
+        const float uu = fmaf(sqrtf(-__logf(r.y)), cos_uniform(r.z), e.beta);
         const float w = e.xa - uu, w1 = e.xa - e.u1;
         u = uu;
-        return uu <= e.u1 && r.w * (w * w + a2) <= w1 * w1 + a2;
+        return uu >= UPAR_U_MIN && uu <= e.u1 &&
+               r.w * fmaf(w, w, a2) * __expf(2.f * e.beta * (uu - e.u1)) <= fmaf(w1, w1, a2);
     }
 }
 
@@ -127,7 +156,7 @@ __device__ __forceinline__ void sample_uperp(float x_in, float x_crit, float r1,
     const float shift = fabsf(x_in) < x_crit ? x_crit * x_crit : 0.f;
     const float m = sqrtf(shift - __logf(r1));
     float s, c;
-    sincospif(2.f * r2, &s, &c);
+    sincos_uniform(r2, s, c);
     up1 = m * c; up2 = m * s;
 }
 

@@ -87,7 +87,7 @@ __global__ void unit_scatter_kernel(float a, float x_in, float x_crit, int phase
     bool dip;
     const float mu = sample_mu(phase, s2.z, s1.y, dip);
     float sph, cph;
-    sincospif(2.f * s1.z, &sph, &cph);
+    sincos_uniform(s1.z, sph, cph);
     float e1[3], e2[3];
     ortho_basis(0.f, 0.f, 1.f, e1, e2);
     const float st = sqrtf(fmaxf(0.f, 1.f - mu * mu));

@@ -86,9 +86,9 @@ __global__ void __launch_bounds__(WALK_THREADS, PEEL ? 2 : THOR_WALK_MIN_CTAS) w
                     while (lo < hi) { const long long mid = (lo + hi) >> 1; if (us < p.src_cdf[mid]) hi = mid; else lo = mid + 1; }
                     const float mu0 = fmaf(2.f, e1.y, -1.f);      // isotropic direction (reading A22)
                     float sp, cp;
-                    sincospif(2.f * e1.z, &sp, &cp);
+                    sincos_uniform(e1.z, sp, cp);
                     const float st0 = sqrtf(fmaxf(0.f, 1.f - mu0 * mu0));
-                    const float gauss = sqrtf(-2.f * __logf(e1.w)) * cospif(2.f * e2.x);
+                    const float gauss = sqrtf(-2.f * __logf(e1.w)) * cos_uniform(e2.x);
                     dda_locate(ray, p.g, p.src_pos[3 * lo], p.src_pos[3 * lo + 1], p.src_pos[3 * lo + 2]);
                     ray_set_direction(ray, st0 * cp, st0 * sp, mu0);
                     cell = load_cell(p, dda_linear(ray, p.g));
@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(WALK_THREADS, PEEL ? 2 : THOR_WALK_MIN_CTAS) w
                     bool is_dipole;
                     const float mu = sample_mu(phase, s2.z, s1.y, is_dipole);
                     float sph, cph;
-                    sincospif(2.f * s1.z, &sph, &cph);
+                    sincos_uniform(s1.z, sph, cph);
                     float e1[3], e2[3];
                     ortho_basis(kx, ky, kz, e1, e2);
                     if (PEEL) {                                   // a12, before adopting k'
