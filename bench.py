@@ -168,7 +168,7 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if rank == 0:
         cuda_build.build()
-    from paper_2507_11603_b200 import thor
+    from paper_2507_11603_b200 import shard, thor
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
     torch.cuda.set_device(local)
     if world > 1:
@@ -188,9 +188,7 @@ def main():
         ctx.run(n, w["seed"] + i, dict(opts, photon_id_offset=rank * n))
         ctx.tally_to_device(thor.TALLY_SPECTRUM, spec_dev)
         ctx.tally_to_device(thor.TALLY_COUNTERS, cnt_dev)
-        if world > 1:
-            dist.all_reduce(spec_dev)
-            dist.all_reduce(cnt_dev)
+        shard.allreduce_tallies([spec_dev, cnt_dev])               # no-op at N = 1
         return ctx.last_run_ms()
 
     for i in range(args.warmup):
