@@ -33,6 +33,21 @@ __device__ __forceinline__ void ray_set_direction(Ray& r, float kx, float ky, fl
     r.ix = __fdiv_rn(1.0f, kx); r.iy = __fdiv_rn(1.0f, ky); r.iz = __fdiv_rn(1.0f, kz);
 }
 
+// Direction now, reciprocals later: a packet that scatters deep inside a cell never needs them (walk_kernel).
+__device__ __forceinline__ void ray_set_k(Ray& r, float kx, float ky, float kz) { r.kx = kx; r.ky = ky; r.kz = kz; }
+__device__ __forceinline__ void ray_set_inv(Ray& r) {
+    r.ix = __fdiv_rn(1.0f, r.kx); r.iy = __fdiv_rn(1.0f, r.ky); r.iz = __fdiv_rn(1.0f, r.kz);
+}
+
+// Distance from the in-cell position to the nearest face of the cell in ANY direction (frozen axes have none): a
+// lower bound of the segment length dda_next_face would return, at the cost of six min operations.
+__device__ __forceinline__ float dda_min_face_distance(const Ray& r, const GridDims& g) {
+    const float dx = (g.frozen & 1u) ? CUDART_INF_F : fminf(r.fx, 1.0f - r.fx);
+    const float dy = (g.frozen & 2u) ? CUDART_INF_F : fminf(r.fy, 1.0f - r.fy);
+    const float dz = (g.frozen & 4u) ? CUDART_INF_F : fminf(r.fz, 1.0f - r.fz);
+    return fminf(dx, fminf(dy, dz));
+}
+
 __device__ __forceinline__ float dda_t_axis(float f, float k, float inv, bool frozen) {
     const float face = k > 0.0f ? 1.0f : 0.0f;
     const float t = __fmul_rn(__fsub_rn(face, f), inv);

@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(WALK_THREADS, PEEL ? 2 : THOR_WALK_MIN_CTAS) w
     Ray ray;
     BlockRng rng;
     Cell cell;                                                // the cell the packet is in (valid unless `stale`)
-    bool stale = true;
+    bool stale = true, inv_ok = false;                        // inv_ok: 1/k of the current direction is in `ray`
     float V = 0.f, tau_rem = 0.f, hit_kt = 0.f, x_in = 0.f, upar = 0.f;
     UparEnvelope env;
     env.mTot = -1.f;
@@ -90,7 +90,8 @@ __global__ void __launch_bounds__(WALK_THREADS, PEEL ? 2 : THOR_WALK_MIN_CTAS) w
                     const float st0 = sqrtf(fmaxf(0.f, 1.f - mu0 * mu0));
                     const float gauss = sqrtf(-2.f * __logf(e1.w)) * cos_uniform(e2.x);
                     dda_locate(ray, p.g, p.src_pos[3 * lo], p.src_pos[3 * lo + 1], p.src_pos[3 * lo + 2]);
-                    ray_set_direction(ray, st0 * cp, st0 * sp, mu0);
+                    ray_set_k(ray, st0 * cp, st0 * sp, mu0);
+                    inv_ok = false;
                     cell = load_cell(p, dda_linear(ray, p.g));
                     stale = false;
                     const float dV = p.src_sigma[lo] * gauss;     // Gaussian line in the gas frame (reading A10)
@@ -110,12 +111,31 @@ __global__ void __launch_bounds__(WALK_THREADS, PEEL ? 2 : THOR_WALK_MIN_CTAS) w
 
         // ---- a4-a7: one cell step for every marching lane ----
         if (state == LS_MARCH) {
-            float len;
-            const int ex = dda_next_face(ray, p.g, len);
             if (stale) { cell = load_cell(p, dda_linear(ray, p.g)); stale = false; }
             const float vk = cell.vx * ray.kx + cell.vy * ray.ky + cell.vz * ray.kz;
-            float dtau, s_hit, kt;
-            const bool hit = integrate_segment<HUBBLE>(p, sh.voigt, cell, V, vk, len, tau_rem, dtau, s_hit, kt);
+            bool hit = false;
+            float len = 0.f, dtau = 0.f, s_hit = 0.f, kt = 0.f;
+            int ex = 0;
+            if (!HUBBLE) {
+                // Piecewise-constant cell: the interaction lies at s = tau / kappa if that is inside the
+                // cell.  Deep in an optically thick cell s is far smaller than the distance to the nearest face, which
+                // bounds the segment length from below: no DDA step and no reciprocals of k are needed at all.
+                kt = cell_opacity(sh.voigt, cell, V, vk);
+                const float s = kt > 0.f ? tau_rem / kt : CUDART_INF_F;
+                if (kt > 0.f && s <= dda_min_face_distance(ray, p.g)) {
+                    hit = true; s_hit = s;
+                } else {
+                    if (!inv_ok) { ray_set_inv(ray); inv_ok = true; }
+                    ex = dda_next_face(ray, p.g, len);
+                    hit = kt > 0.f && s <= len;
+                    s_hit = s;
+                    dtau = kt * len;
+                }
+            } else {
+                if (!inv_ok) { ray_set_inv(ray); inv_ok = true; }
+                ex = dda_next_face(ray, p.g, len);
+                hit = integrate_segment<true>(p, sh.voigt, cell, V, vk, len, tau_rem, dtau, s_hit, kt);
+            }
             if (hit) {
                 dda_advance_within(ray, p.g, s_hit);
                 if (HUBBLE) { if (p.hubble != 0.f) V -= p.hubble * s_hit; }
@@ -207,7 +227,8 @@ __global__ void __launch_bounds__(WALK_THREADS, PEEL ? 2 : THOR_WALK_MIN_CTAS) w
                     nx *= inv; ny *= inv; nz *= inv;
                     // a11, Eq. 7, recoil dropped: x_out = x_in + u.(k_out - k_in)
                     const float x_out = x_in - upar + upar * mu + st * (up1 * cph + up2 * sph);
-                    ray_set_direction(ray, nx, ny, nz);
+                    ray_set_k(ray, nx, ny, nz);
+                    inv_ok = false;
                     V = x_out * cell.vth + cell.vx * nx + cell.vy * ny + cell.vz * nz;
                     ++nscat;
                     if (p.v_max > 0.f && fabsf(V) > p.v_max) {

@@ -91,6 +91,12 @@ __device__ __forceinline__ bool integrate_segment(const WalkParams& p, const flo
     return false;
 }
 
+// Total opacity per cell length at velocity offset V for direction cosine-weighted bulk velocity vk (no drift).
+__device__ __forceinline__ float cell_opacity(const float2* s_tab, const Cell& c, float V, float vk) {
+    const float kl = c.nsig > 0.f ? c.nsig * voigt_H(s_tab, c.a, (V - vk) * c.inv_vth) : 0.f;
+    return kl + c.kd;
+}
+
 // a12 peel-off: w = P^ exp(-tau_obs), tau_obs integrated from `at` along k_obs to the box face at
 // velocity offset V_o by the same march (a4-a6), dropped beyond tau_peel_max (reading A13); added to
 // (pixel of the starting point projected perpendicular to k_obs, spectral bin of dv = -V at the box face).
