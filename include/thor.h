@@ -37,6 +37,11 @@ typedef enum {
 #define THOR_PERIODIC_Y 0x20u
 #define THOR_PERIODIC_Z 0x40u
 #define THOR_GRID_NO_VALIDATE 0x100u /* skip the device-side scan for NaN / negative fields */
+#define THOR_GRID_PACK 0x200u     /* the library makes its OWN copy, re-laid-out as one 32-byte record per cell
+                                     {nHI, T, vx, vy, vz, kdust, 0, 0}: one DRAM sector per cell gather instead of
+                                     five or six.  Costs 32 B per cell of device memory; the caller's
+                                     arrays are not referenced after thor_grid_create returns.  Results are
+                                     bit-identical to the borrowed SoA layout. */
 
 /* The dataset (uniform Cartesian grid, fields constant per cell).  Six SoA fp32 arrays, dense
  * row-major [nz][ny][nx] (x fastest): nHI [cm^-3], T [K], vx, vy, vz [km/s], and kdust [cm^-1], the dust ABSORPTION

@@ -13,6 +13,8 @@
 
 namespace thor {
 cudaError_t launch_walk(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out);
+cudaError_t launch_pack_fields(const float* nHI, const float* T, const float* vx, const float* vy, const float* vz,
+                               const float* kdust, long long n, float4* out, cudaStream_t stream);
 cudaError_t launch_validate_fields(const float* nHI, const float* T, const float* vx, const float* vy, const float* vz,
                                    const float* kdust, long long n, unsigned* d_flags, cudaStream_t stream);
 }  // namespace thor
@@ -25,6 +27,8 @@ struct thor_ctx {
     long long n_cells = 0;
     const float* f[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // nHI, T, vx, vy, vz, kdust
     float* owned[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    float4* d_packed = nullptr;                 // THOR_GRID_PACK: the library's own one-sector-per-cell copy
+    bool has_dust = false;
     // sources
     long long n_src = 0;
     float* d_src_pos = nullptr;
@@ -87,6 +91,7 @@ extern "C" void thor_grid_destroy(thor_ctx* ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     for (float* p : ctx->owned) if (p) cudaFree(p);
+    if (ctx->d_packed) cudaFree(ctx->d_packed);
     if (ctx->d_src_pos) cudaFree(ctx->d_src_pos);
     if (ctx->d_src_sigma) cudaFree(ctx->d_src_sigma);
     if (ctx->d_src_cdf) cudaFree(ctx->d_src_cdf);
@@ -170,6 +175,17 @@ extern "C" thor_status thor_grid_create(thor_ctx** out, int nx, int ny, int nz, 
     } else {
         CU(cudaStreamSynchronize(ctx->stream));
     }
+    ctx->has_dust = kdust != nullptr;
+    if (flags & THOR_GRID_PACK) {
+        CU(cudaMalloc(&ctx->d_packed, (size_t)ctx->n_cells * 2 * sizeof(float4)));
+        CU(thor::launch_pack_fields(ctx->f[0], ctx->f[1], ctx->f[2], ctx->f[3], ctx->f[4], ctx->f[5], ctx->n_cells,
+                                    ctx->d_packed, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        for (int i = 0; i < 6; ++i) {            // the SoA arrays are no longer read: drop our copies / the borrow
+            if (ctx->owned[i]) { cudaFree(ctx->owned[i]); ctx->owned[i] = nullptr; }
+            ctx->f[i] = nullptr;
+        }
+    }
     guard.c = nullptr;
     *out = ctx;
     return THOR_OK;
@@ -235,6 +251,7 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     thor::WalkParams p{};
     p.g = ctx->g;
     p.nHI = ctx->f[0]; p.T = ctx->f[1]; p.vx = ctx->f[2]; p.vy = ctx->f[3]; p.vz = ctx->f[4]; p.kdust = ctx->f[5];
+    p.packed = ctx->d_packed; p.has_dust = ctx->has_dust ? 1 : 0;
     p.sig_cell = (float)(K.c_sig * ctx->cell_cm);
     p.c_a = (float)K.c_a; p.c_vth = (float)K.c_vth; p.inv_c_vth = (float)(1.0 / K.c_vth);
     p.cell_cm = (float)ctx->cell_cm;

@@ -39,6 +39,8 @@ struct WalkParams {
     const float* __restrict__ vy;
     const float* __restrict__ vz;
     const float* __restrict__ kdust;     // nullptr = no dust
+    const float4* __restrict__ packed;   // THOR_GRID_PACK: [cell][2] = {nHI, T, vx, vy}, {vz, kdust, 0, 0}: one 32-byte sector
+    int has_dust;                        // kdust was given (packed or not)
     float sig_cell;      // c_sig * cell_cm: kappa_line per cell length = n * sig_cell * rsqrt(T) * H(a,x)
     float c_a, c_vth, inv_c_vth;
     float cell_cm;

@@ -30,6 +30,22 @@ cudaError_t launch_validate_fields(const float* nHI, const float* T, const float
     return cudaGetLastError();
 }
 
+__global__ void pack_fields_kernel(const float* nHI, const float* T, const float* vx, const float* vy, const float* vz,
+                                   const float* kdust, long long n, float4* out) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        out[2 * i] = make_float4(nHI[i], T[i], vx[i], vy[i]);
+        out[2 * i + 1] = make_float4(vz[i], kdust ? kdust[i] : 0.f, 0.f, 0.f);
+    }
+}
+
+cudaError_t launch_pack_fields(const float* nHI, const float* T, const float* vx, const float* vy, const float* vz,
+                               const float* kdust, long long n, float4* out, cudaStream_t stream) {
+    long long blocks = (n + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    pack_fields_kernel<<<(unsigned)blocks, 256, 0, stream>>>(nHI, T, vx, vy, vz, kdust, n, out);
+    return cudaGetLastError();
+}
+
 __global__ void unit_philox_kernel(uint64_t seed, uint64_t id0, long long n_ids, int n_draws, uint32_t* out) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_ids) return;

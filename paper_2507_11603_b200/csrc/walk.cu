@@ -17,6 +17,10 @@ namespace thor {
 constexpr int WALK_THREADS = THOR_WALK_THREADS;
 constexpr int MAX_SPEC_BINS = 4096;
 constexpr int FINISH_MIN_LANES = THOR_FINISH_MIN_LANES;
+#ifndef THOR_REFILL_MIN_LANES
+#define THOR_REFILL_MIN_LANES 8
+#endif
+constexpr int REFILL_MIN_LANES = THOR_REFILL_MIN_LANES;
 
 struct BlockTallies {
     float2 voigt[VOIGT_NODES];
@@ -69,8 +73,10 @@ __global__ void __launch_bounds__(WALK_THREADS, PEEL ? 2 : THOR_WALK_MIN_CTAS) w
 
     for (;;) {
         // ---- a14 + a2/a3: refill idle lanes from the global photon counter, emit ----
+        // Refills are batched: emission is a chain of dependent loads (binary search of the source CDF, source cell
+        // gather) that stalls the whole warp, so it waits until REFILL_MIN_LANES lanes are idle (or nothing else runs).
         const unsigned idle = __ballot_sync(0xffffffffu, state == LS_IDLE);
-        if (idle && more) {
+        if (more && idle && (__popc(idle) >= REFILL_MIN_LANES || idle == __ballot_sync(0xffffffffu, state == LS_IDLE || state == LS_OUT))) {
             unsigned long long base = 0;
             if (lane == 0) base = atomicAdd(p.next_photon, (unsigned long long)__popc(idle));
             base = __shfl_sync(0xffffffffu, base, 0);
@@ -189,7 +195,7 @@ __global__ void __launch_bounds__(WALK_THREADS, PEEL ? 2 : THOR_WALK_MIN_CTAS) w
                 // draws of this event: (tau, mu, phi, perp1), (perp2, dust, mix, -)
                 const float4 s1 = rng.next4(k0, k1), s2 = rng.next4(k0, k1);
                 // a7 interaction kind: dust with probability kappa_dust / kappa_total
-                if (p.kdust && s2.y * hit_kt < cell.kd) {
+                if (p.has_dust && s2.y * hit_kt < cell.kd) {
                     tally_finish(p, sh, CT_ABSORBED, V, nscat, crossings, rej_iters, rng.id(), ray.kx, ray.ky, ray.kz);
                     state = LS_IDLE;
                 } else {

@@ -28,9 +28,16 @@ struct Cell {
 
 __device__ __forceinline__ Cell load_cell(const WalkParams& p, int64_t i) {
     Cell c;
-    const float n = __ldg(p.nHI + i), T = __ldg(p.T + i);
-    c.vx = __ldg(p.vx + i); c.vy = __ldg(p.vy + i); c.vz = __ldg(p.vz + i);
-    c.kd = p.kdust ? __ldg(p.kdust + i) * p.cell_cm : 0.f;
+    float n, T;
+    if (p.packed) {                     // one 32-byte sector per cell instead of five or six
+        const float4 q0 = __ldg(p.packed + 2 * i), q1 = __ldg(p.packed + 2 * i + 1);
+        n = q0.x; T = q0.y; c.vx = q0.z; c.vy = q0.w; c.vz = q1.x;
+        c.kd = q1.y * p.cell_cm;
+    } else {
+        n = __ldg(p.nHI + i); T = __ldg(p.T + i);
+        c.vx = __ldg(p.vx + i); c.vy = __ldg(p.vy + i); c.vz = __ldg(p.vz + i);
+        c.kd = p.kdust ? __ldg(p.kdust + i) * p.cell_cm : 0.f;
+    }
     const float rs = rsqrtf(T);
     c.a = p.c_a * rs;
     c.inv_vth = p.inv_c_vth * rs;

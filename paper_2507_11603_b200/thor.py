@@ -12,7 +12,7 @@ LIB_PATH = os.path.join(_HERE, "libthor_b200.so")
 
 STATUS = {0: "THOR_OK", 1: "THOR_ERR_ARG", 2: "THOR_ERR_STATE", 3: "THOR_ERR_OOM", 4: "THOR_ERR_CUDA",
           5: "THOR_ERR_UNSUPPORTED"}
-GRID_HOST, PERIODIC_X, PERIODIC_Y, PERIODIC_Z, GRID_NO_VALIDATE = 0x1, 0x10, 0x20, 0x40, 0x100
+GRID_HOST, PERIODIC_X, PERIODIC_Y, PERIODIC_Z, GRID_NO_VALIDATE, GRID_PACK = 0x1, 0x10, 0x20, 0x40, 0x100, 0x200
 TALLY_SPECTRUM, TALLY_NSCAT_HIST, TALLY_COUNTERS, TALLY_CUBE, TALLY_RAW, TALLY_DEVICE_DST = 0, 1, 2, 3, 4, 0x100
 COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "cell_crossings", "rejection_iters",
                  "peel_rays", "peel_cells"]
@@ -111,10 +111,10 @@ class Context:
     kept referenced here) or numpy float32 arrays (host=True: copied to the device by the library)."""
 
     def __init__(self, nx, ny, nz, cell_cm, nHI, T, vx, vy, vz, kdust=None, periodic=(0, 0, 0), host=False,
-                 validate=True):
+                 validate=True, pack=False):
         self._ctx = C.c_void_p()
         fields = [nHI, T, vx, vy, vz, kdust]
-        flags = _periodic_flags(periodic) | (0 if validate else GRID_NO_VALIDATE)
+        flags = _periodic_flags(periodic) | (0 if validate else GRID_NO_VALIDATE) | (GRID_PACK if pack else 0)
         if host:
             self._keep = [None if a is None else np.ascontiguousarray(a, np.float32) for a in fields]
             ptrs = [None if a is None else a.ctypes.data_as(C.c_void_p) for a in self._keep]
@@ -136,9 +136,11 @@ class Context:
             if a is not None and int(np.prod(a.shape)) != nx * ny * nz:
                 raise ValueError("field size does not match nx*ny*nz")
         _check(lib().thor_grid_create(C.byref(self._ctx), nx, ny, nz, float(cell_cm), *ptrs, flags, stream))
+        if pack:
+            self._keep = None              # THOR_GRID_PACK: the library holds its own copy; release ours
 
     @classmethod
-    def from_workload(cls, grid, host=False, device="cuda"):
+    def from_workload(cls, grid, host=False, device="cuda", pack=False):
         """grid: the dict made by paper_2507_11603_b200.workloads (numpy float32 fields)."""
         keys = ("nHI", "T", "vx", "vy", "vz", "kdust")
         if host:
@@ -148,7 +150,7 @@ class Context:
             arrs = [None if grid.get(k) is None else torch.from_numpy(np.ascontiguousarray(grid[k], np.float32)).to(device)
                     for k in keys]
         return cls(grid["nx"], grid["ny"], grid["nz"], grid["cell_cm"], *arrs,
-                   periodic=grid.get("periodic", (0, 0, 0)), host=host)
+                   periodic=grid.get("periodic", (0, 0, 0)), host=host, pack=pack)
 
     def close(self):
         if getattr(self, "_ctx", None) and self._ctx.value:
@@ -215,9 +217,9 @@ class Context:
         return self._get(TALLY_RAW, RAW_DTYPE, self._n)
 
 
-def run_workload(w, n_photons=None, host=False, raw=True, **opt_overrides):
+def run_workload(w, n_photons=None, host=False, raw=True, pack=False, **opt_overrides):
     """Convenience: build a Context from a workloads.* dict, run it, return the tallies as a dict."""
-    ctx = Context.from_workload(w["grid"], host=host)
+    ctx = Context.from_workload(w["grid"], host=host, pack=pack)
     try:
         ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
         n = w["n_photons"] if n_photons is None else n_photons
