@@ -30,9 +30,12 @@ from paper_2507_11603_b200 import workloads as W
 # Issue-slot roofline constants: algorithmic thread-instructions per unit of work, counted
 # once from ncu (smsp__thread_inst_executed.sum of the walk kernel regressed on its scattering / crossing counters;
 # profiles/r01_walk_inst_per_unit.md) — fixed numbers, so a slower kernel cannot raise its own roofline fraction.
-INST_PER_SCATTERING = 640.0
+INST_PER_SCATTERING = 630.0
 INST_PER_CROSSING = 110.0
 N_SM, SCHEDULERS_PER_SM, LANES = 148, 4, 32
+# dram__bytes_read.sum + dram__bytes_write.sum of walk_kernel per launch, from the ncu captures summarised in
+# profiles/r01_launches_bench_shell.md and profiles/r01_walk_kernel_v5_ncu.md (bench.py cannot measure this itself)
+TRAFFIC_BYTES_PER_LAUNCH = {"shell": 5.4e7, "sphere": 7.9e5, "slab": 1.8e5, "gather": 1.2677e11}
 
 
 def make_workload(name, n_photons=None):
@@ -47,6 +50,11 @@ def make_workload(name, n_photons=None):
         w["opts"]["max_scatter"] = 100_000
     elif name == "web":      # configs[4] at 512^3
         w = W.cosmic_web(n=512, n_src=1 << 18, n_photons=1_000_000, map_pix=2048)
+    elif name == "gather":   # the cell-gather regime of configs[4]: same 512^3 fields, optically thin (mean n_HI 1e-11), so
+        # packets stream through ~340 cells each and the walk is bound by the HBM gathers, not by scatterings
+        w = W.cosmic_web(n=512, n_src=1 << 16, n_photons=4_000_000, map_pix=2048, mean_n=1e-11)
+        w["opts"].update(peel_on=0, v_max_kms=0.0)
+        w["name"] = "cosmic_web_n512_thin_gather"
     else:
         raise SystemExit(f"unknown workload {name}")
     if n_photons:
@@ -155,6 +163,7 @@ def main():
     ap.add_argument("--ref-chunk", type=int, default=500)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--pack", type=int, default=-1, help="THOR_GRID_PACK (1/0); default: on for the gather workload")
     args = ap.parse_args()
     w = make_workload(args.workload, args.n_photons)
     if args.impl == "reference":
@@ -177,7 +186,8 @@ def main():
     thor.lib()
     n = w["n_photons"]
     opts = dict(w["opts"], raw_output=0)
-    ctx = thor.Context.from_workload(w["grid"])                    # fields resident in HBM before the timed region
+    pack = bool(args.pack) if args.pack >= 0 else args.workload in ("gather", "web", "turb")
+    ctx = thor.Context.from_workload(w["grid"], pack=pack)         # fields resident in HBM before the timed region
     ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     spec_dev = torch.zeros(opts["spec_bins"] + 2, dtype=torch.int64, device="cuda")
@@ -240,11 +250,30 @@ def main():
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     peak = n_sm * SCHEDULERS_PER_SM * LANES * sm_hz * world
     achieved = inst / (kernel_ms * 1e-3)
+    if args.workload == "gather":
+        # HBM roofline of the cell gather: 20 algorithmic bytes per crossing (n, T, vx, vy, vz)
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        hbm = float(peaks.get("hbm_gbs", 6650.0)) * world
+        gbs = 20.0 * (c["cell_crossings"] + c["peel_cells"]) / (kernel_ms * 1e-3) / 1e9
+        out["roofline_hbm"] = {"bound": "hbm", "achieved": gbs, "peak": hbm, "unit": "GB/s", "frac": gbs / hbm,
+                               "traffic": TRAFFIC_BYTES_PER_LAUNCH["gather"] if (pack and not args.n_photons) else None,
+                               "algorithmic_bytes_per_launch": 20.0 * (c["cell_crossings"] + c["peel_cells"]) / args.steps,
+                               "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks else "6650 GB/s (of fallback)",
+                               "bytes_per_crossing": 20, "layout": "packed 32 B/cell" if pack else "SoA 5 x 4 B/cell"}
+    out["config"]["layout"] = "packed 32 B/cell (THOR_GRID_PACK)" if pack else "SoA fp32, borrowed"
     out["roofline"] = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "G thread-inst/s",
-                       "frac": achieved / peak, "traffic": None,
+                       "frac": achieved / peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.workload) if not args.n_photons else None,
+                       "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01_*.md",
                        "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_hz / 1e6:.0f} MHz (clocks.max.sm), derived in DESIGN.md",
                        "kernel": "walk_kernel", "kernel_ms_per_launch": kernel_ms / args.steps,
                        "inst_per_scattering": INST_PER_SCATTERING, "inst_per_crossing": INST_PER_CROSSING}
+    if "roofline_hbm" in out:                                       # gather workload: the HBM roofline is the binding one
+        out["roofline_alu"] = out["roofline"]
+        out["roofline"] = out.pop("roofline_hbm")
     ctx.close()
 
     # ---- e2e: the same step through the C-ABI with HOST buffers; H2D of grid + sources and D2H of tallies are timed
@@ -258,7 +287,7 @@ def main():
                 dist.barrier()
             torch.cuda.synchronize()
             t0 = time.perf_counter()
-            cx = thor.Context.from_workload(w["grid"], host=True)
+            cx = thor.Context.from_workload(w["grid"], host=True, pack=pack)
             cx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
             cx.run(n, w["seed"] + max(i, 0), dict(opts, photon_id_offset=rank * n))
             cx.spectrum(); cx.nscat_hist()
