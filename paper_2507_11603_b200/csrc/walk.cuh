@@ -26,23 +26,37 @@ struct Cell {
     float vx, vy, vz;
 };
 
-__device__ __forceinline__ Cell load_cell(const WalkParams& p, int64_t i) {
+// The gather is issued as soon as the packet knows its next cell (right after the face crossing) and consumed one
+// loop iteration later: load_cell_raw leaves the raw fields in the Cell's own registers (n in nsig, T in a, kdust in
+// kd) and derive_cell turns them into the derived quantities at first use, so the loop control and the other stage
+// sections run in the shadow of the load.
+__device__ __forceinline__ Cell load_cell_raw(const WalkParams& p, int64_t i) {
     Cell c;
-    float n, T;
     if (p.packed) {                     // one 32-byte sector per cell instead of five or six
         const float4 q0 = __ldg(p.packed + 2 * i), q1 = __ldg(p.packed + 2 * i + 1);
-        n = q0.x; T = q0.y; c.vx = q0.z; c.vy = q0.w; c.vz = q1.x;
-        c.kd = q1.y * p.cell_cm;
+        c.nsig = q0.x; c.a = q0.y; c.vx = q0.z; c.vy = q0.w; c.vz = q1.x; c.kd = q1.y;
     } else {
-        n = __ldg(p.nHI + i); T = __ldg(p.T + i);
+        c.nsig = __ldg(p.nHI + i); c.a = __ldg(p.T + i);
         c.vx = __ldg(p.vx + i); c.vy = __ldg(p.vy + i); c.vz = __ldg(p.vz + i);
-        c.kd = p.kdust ? __ldg(p.kdust + i) * p.cell_cm : 0.f;
+        c.kd = p.kdust ? __ldg(p.kdust + i) : 0.f;
     }
+    c.vth = 0.f; c.inv_vth = 0.f;
+    return c;
+}
+
+__device__ __forceinline__ void derive_cell(const WalkParams& p, Cell& c) {
+    const float n = c.nsig, T = c.a;
     const float rs = rsqrtf(T);
+    c.kd = c.kd * p.cell_cm;
     c.a = p.c_a * rs;
     c.inv_vth = p.inv_c_vth * rs;
     c.vth = p.c_vth * (T * rs);
     c.nsig = n > 0.f ? n * p.sig_cell * rs : 0.f;
+}
+
+__device__ __forceinline__ Cell load_cell(const WalkParams& p, int64_t i) {
+    Cell c = load_cell_raw(p, i);
+    derive_cell(p, c);
     return c;
 }
 
