@@ -193,12 +193,15 @@ def main():
     spec_dev = torch.zeros(opts["spec_bins"] + 2, dtype=torch.int64, device="cuda")
     cnt_dev = torch.zeros(len(thor.COUNTER_NAMES), dtype=torch.int64, device="cuda")
 
+    feed_ms = []
+
     def step(i):
         # rank r walks photon ids [r n, (r+1) n) of step i's seed; tallies summed over ranks (the one exchange step)
         ctx.run(n, w["seed"] + i, dict(opts, photon_id_offset=rank * n))
         ctx.tally_to_device(thor.TALLY_SPECTRUM, spec_dev)
         ctx.tally_to_device(thor.TALLY_COUNTERS, cnt_dev)
         shard.allreduce_tallies([spec_dev, cnt_dev])               # no-op at N = 1
+        feed_ms.append(ctx.last_run_feed_ms())
         return ctx.last_run_ms()
 
     for i in range(args.warmup):
@@ -242,6 +245,11 @@ def main():
                    "scatterings_per_packet": c["scatterings"] / packets,
                    "rejection_iters_per_scattering": c["rejection_iters"] / max(1, c["scatterings"])},
         "clocks": clocks, "gpu_launches": args.steps * 1,
+        # how the kernel time splits: until the photon counter runs dry the walk is fed (throughput phase); after that
+        # the launch only drains the packets in flight, and lasts as long as its longest single packet
+        "phases": {"feed_ms_per_step": float(np.mean(feed_ms[-args.steps:])),
+                   "drain_ms_per_step": kernel_ms / args.steps - float(np.mean(feed_ms[-args.steps:])),
+                   "source": "device %globaltimer at kernel entry and when the photon counter is first found exhausted (thor_last_run_feed_ms)"},
         "counters": c,
     }
     # ---- roofline of the dominant (only) kernel: issue-slot bound (grid is L2-resident)

@@ -107,6 +107,11 @@ thor_status thor_run(thor_ctx *ctx, unsigned long long n_photons, unsigned long 
 /* Duration of the walk kernel of the last thor_run in milliseconds, from CUDA events on the context's stream. */
 thor_status thor_last_run_ms(const thor_ctx *ctx, float *ms);
 
+/* Time, in milliseconds from kernel entry (device %globaltimer), at which the photon counter of the last thor_run was
+ * first found exhausted: until then the walk is fed (throughput phase); the rest of thor_last_run_ms is the drain of
+ * the packets in flight, whose length is set by the longest single packet. */
+thor_status thor_last_run_feed_ms(const thor_ctx *ctx, float *ms);
+
 /* tallies */
 #define THOR_TALLY_SPECTRUM 0   /* uint64[spec_bins + 2]: bins, then underflow, overflow */
 #define THOR_TALLY_NSCAT_HIST 1 /* uint64[64]: bin 0: nscat = 0; bin b: 2^(b-1) <= nscat < 2^b */

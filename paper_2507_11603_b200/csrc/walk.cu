@@ -5,6 +5,12 @@
 
 namespace thor {
 
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
 #ifndef THOR_WALK_THREADS
 #define THOR_WALK_THREADS 256
 #endif
@@ -51,6 +57,7 @@ __device__ __forceinline__ void tally_finish(const WalkParams& p, BlockTallies& 
 template <bool HUBBLE, bool PEEL, int MIN_CTAS>
 __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __grid_constant__ WalkParams p) {
     __shared__ BlockTallies sh;
+    if (threadIdx.x == 0) atomicMin(p.t_start, global_timer_ns());
     voigt_table_load(sh.voigt);
     for (int i = threadIdx.x; i < N_COUNTERS; i += blockDim.x) sh.counters[i] = 0ull;
     for (int i = threadIdx.x; i < 64; i += blockDim.x) sh.nscat_hist[i] = 0u;
@@ -113,7 +120,11 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
                     state = LS_MARCH;
                 }
             }
-            if (__any_sync(0xffffffffu, state == LS_OUT)) more = false;
+            if (__any_sync(0xffffffffu, state == LS_OUT)) {
+                // the queue is empty: from here on the launch only drains the packets in flight
+                if (more && lane == 0) atomicMin(p.t_dry, global_timer_ns());
+                more = false;
+            }
         }
 
         // ---- a4-a7: one cell step for every marching lane ----

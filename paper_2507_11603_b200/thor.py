@@ -19,7 +19,7 @@ COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "
 RAW_DTYPE = np.dtype([("V", "<f4"), ("nscat", "<u4"), ("status", "<i4"), ("kx", "<f4"), ("ky", "<f4"), ("kz", "<f4")])
 
 EXPORTS = ["thor_grid_create", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run",
-           "thor_last_run_ms", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_dda_trace",
+           "thor_last_run_ms", "thor_last_run_feed_ms", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_dda_trace",
            "thor_unit_voigt", "thor_unit_scatter"]
 
 
@@ -67,6 +67,7 @@ def lib():
         L.thor_opts_default.restype = None
         L.thor_run.argtypes = [P, C.c_ulonglong, C.c_ulonglong, C.POINTER(Opts)]
         L.thor_last_run_ms.argtypes = [P, C.POINTER(f)]
+        L.thor_last_run_feed_ms.argtypes = [P, C.POINTER(f)]
         L.thor_tally_get.argtypes = [P, i32, P, C.c_size_t, C.POINTER(C.c_size_t)]
         L.thor_last_error.argtypes = [P]
         L.thor_last_error.restype = C.c_char_p
@@ -181,6 +182,11 @@ class Context:
     def last_run_ms(self):
         ms = C.c_float()
         _check(lib().thor_last_run_ms(self._ctx, C.byref(ms)), self._ctx)
+        return ms.value
+
+    def last_run_feed_ms(self):
+        ms = C.c_float()
+        _check(lib().thor_last_run_feed_ms(self._ctx, C.byref(ms)), self._ctx)
         return ms.value
 
     def _get(self, kind, dtype, shape):

@@ -339,6 +339,7 @@ def test_edge_cases(thor):
         assert sum(ctx.counters().values()) == 0 and int(ctx.spectrum().sum()) == 0
         ctx.run(1, 1, dict(w["opts"], raw_output=1))                # a single packet (one lane of one warp)
         assert sum(ctx.counters()[k] for k in ("escaped", "absorbed", "terminated", "capped")) == 1
+        assert 0.0 <= ctx.last_run_feed_ms() <= ctx.last_run_ms() + 1e-3   # feed phase lies inside the kernel time
         ctx.run(33, 1, dict(w["opts"], raw_output=1, max_scatter=3))   # ragged warp + cap
         c = ctx.counters()
         assert c["escaped"] + c["capped"] == 33 and c["capped"] > 0
