@@ -3,6 +3,17 @@
 // The Monte Carlo resonant-scattering random walk of PAPER.md §3.4 (Fig. 1), step by step, in
 // fp64, one packet at a time.  Numbered steps follow DESIGN.md §"Algorithm"; each cites the
 // passage it restates.  Readings of silent/ambiguous points are the A-numbers of DESIGN.md.
+//
+// Pins (tests/test_oracle_walk.py): Neufeld slab and Dijkstra sphere escape CDFs, E_2 unscattered fraction, thin
+// limit, dust-only escape fraction, interaction-kind probability, core-skip and Galilean invariance, Gunn-Peterson
+// depth under Hubble drift, peel-off (thin limit + pixel mapping, next-event-estimator identity, dipole weight
+// ratio), infinite segments, photon-number conservation.
+// PARITY UNPINNED: the scattering COUNT of a walk has no closed form in the paper or the literature quoted by it
+// (only "N_scat ∝ tau_0" at high tau_0), so the absolute number of scatterings per packet is checked
+// only for order of magnitude; and the paper's outflow-sphere, MgII and cosmological results (PAPER.md:326 right,
+// 358, Figs. 7-10) are figures without printed values.  Local core-skipping (mode 2, reading A7) is pinned only
+// through the global mode's invariance test; the sub-cell stepping criterion (A12) only through the Gunn-Peterson
+// depth.
 #pragma once
 #include <cstdint>
 #include <cmath>
