@@ -35,7 +35,7 @@ INST_PER_CROSSING = 110.0
 N_SM, SCHEDULERS_PER_SM, LANES = 148, 4, 32
 # dram__bytes_read.sum + dram__bytes_write.sum of walk_kernel per launch, from the ncu captures summarised in
 # profiles/r01_launches_bench_shell.md and profiles/r01_walk_kernel_v5_ncu.md (bench.py cannot measure this itself)
-TRAFFIC_BYTES_PER_LAUNCH = {"shell": 5.4e7, "sphere": 7.9e5, "slab": 1.8e5, "gather": 1.2677e11}
+TRAFFIC_BYTES_PER_LAUNCH = {"shell": 6.3e7, "sphere": 7.9e5, "slab": 1.8e5, "gather": 1.2677e11}
 
 
 def make_workload(name, n_photons=None):
