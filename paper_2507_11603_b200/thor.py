@@ -155,7 +155,9 @@ class Context:
 
     def close(self):
         if getattr(self, "_ctx", None) and self._ctx.value:
-            lib().thor_grid_destroy(self._ctx)
+            L = _lib                      # at interpreter shutdown the module globals may already be gone
+            if L is not None:
+                L.thor_grid_destroy(self._ctx)
             self._ctx = C.c_void_p()
         self._keep = None
 
