@@ -425,3 +425,36 @@ def test_packed_layout_is_bit_identical(thor):
             assert np.array_equal(a["spectrum"], b["spectrum"])
             if a["cube"] is not None:
                 assert np.array_equal(a["cube"], b["cube"])
+
+
+@pytest.mark.parametrize("which", ["shell", "slab"])
+def test_full_size_configs_properties(thor, which):
+    """BASELINE.json configs 2 and 3 at FULL size (128^3 shell / 256-cell slab, 1e6 packets), in the launch
+    configuration bench.py times (persistent grid of 444 CTAs).  The oracle cannot walk 1e10 scatterings, so: (i)
+    conservation and tally consistency; (ii) a packet's fate depends on (seed, photon id) only, not on what else is in
+    flight — the raw records of the first 3000 ids equal, bit for bit, those of a 3000-packet run (a far smaller
+    grid: 12 CTAs), which is the configuration the oracle parity tests above cover; (iii) the
+    feed/drain split lies inside the kernel time."""
+    w = W.expanding_shell(n=128, n_photons=1_000_000) if which == "shell" else W.static_slab(n_photons=1_000_000)
+    n = w["n_photons"]
+    ctx = thor.Context.from_workload(w["grid"])
+    try:
+        ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
+        ctx.run(n, w["seed"], dict(w["opts"], raw_output=1))
+        full = dict(spectrum=ctx.spectrum(), nscat_hist=ctx.nscat_hist(), counters=ctx.counters(), raw=ctx.raw())
+        assert 0.0 < ctx.last_run_feed_ms() <= ctx.last_run_ms()
+        _conserved(full, n)
+        k = 3000
+        ctx.run(k, w["seed"], dict(w["opts"], raw_output=1))
+        small = ctx.raw()
+        assert full["raw"][:k].tobytes() == small.tobytes()
+    finally:
+        ctx.close()
+    if which == "slab":
+        assert full["counters"]["escaped"] == n
+        ax = np.abs(full["raw"]["V"].astype(float)) / 12.845          # x at 1e4 K (recipe number)
+        atau = 4718.0
+        kk = math.sqrt(math.pi ** 3 / 54) / atau
+        assert stats.kstest(ax[::50], lambda x: 4 / math.pi * np.arctan(np.tanh(kk * x ** 3 / 2))).statistic < 0.05   # P4
+    else:
+        assert full["counters"]["absorbed"] > 0.85 * n
