@@ -180,19 +180,15 @@ __device__ __forceinline__ float sample_mu(int phase, float r_mix, float r, bool
     return fminf(fmaxf(mu, -1.f), 1.f);
 }
 
-// Orthonormal basis (e1, e2) perpendicular to the unit vector k: helper axis = the axis of the smallest |k| component.
+// Orthonormal basis (e1, e2) perpendicular to the unit vector k, branch-free (Duff et al. 2017 construction: with
+// sg = sign(kz), a = -1/(sg + kz), b = kx ky a:  e1 = (1 + sg kx^2 a, sg b, -sg kx),  e2 = (b, sg + ky^2 a, -ky)).
+// Any right-handed choice gives the same distribution of k' because the azimuth is uniform.
 __device__ __forceinline__ void ortho_basis(float kx, float ky, float kz, float e1[3], float e2[3]) {
-    const float ax = fabsf(kx), ay = fabsf(ky), az = fabsf(kz);
-    float hx = 0.f, hy = 0.f, hz = 0.f;
-    if (ax <= ay && ax <= az) hx = 1.f; else if (ay <= az) hy = 1.f; else hz = 1.f;
-    const float hk = hx * kx + hy * ky + hz * kz;
-    float x = hx - hk * kx, y = hy - hk * ky, z = hz - hk * kz;
-    const float inv = rsqrtf(x * x + y * y + z * z);
-    x *= inv; y *= inv; z *= inv;
-    e1[0] = x; e1[1] = y; e1[2] = z;
-    e2[0] = ky * z - kz * y;
-    e2[1] = kz * x - kx * z;
-    e2[2] = kx * y - ky * x;
+    const float sg = copysignf(1.f, kz);
+    const float a = -1.f / (sg + kz);
+    const float b = kx * ky * a;
+    e1[0] = fmaf(sg * kx, kx * a, 1.f); e1[1] = sg * b; e1[2] = -sg * kx;
+    e2[0] = b; e2[1] = fmaf(ky, ky * a, sg); e2[2] = -ky;
 }
 
 }  // namespace thor
