@@ -135,6 +135,20 @@ typedef struct thor_raw_record {
  * THOR_ERR_STATE if the last run did not produce that tally. */
 thor_status thor_tally_get(thor_ctx *ctx, int kind, void *dst, size_t dst_bytes, size_t *needed);
 
+/* Ray-tracing operators on the context's grid (PAPER.md 3.5; the same DDA, gather and Voigt function as the walk).
+ * org_xyz, dir_xyz: DEVICE float[n_rays][3], origins in cell units inside the grid and unit directions; each ray is
+ * marched to the first box face.  Outputs are DEVICE arrays, any may be NULL:
+ *   out_column[n_rays]     Int n_HI ds [cm^-2]                         (projection, PAPER.md 3.5.1 with q = n_HI, w = 1)
+ *   out_tmean[n_rays]      Int T n_HI ds / Int n_HI ds [K]              (weighted average Q / Q^, w = n_HI)
+ *   out_tau[n_rays][n_v]   tau(V_j), V_j = v_lo + (j + 1/2)(v_hi - v_lo)/n_v [km/s offset from line centre at the
+ *                          ray origin]: Eq. 11 (PAPER.md 3.5.2) with the gas frequency shifted by its line-of-sight
+ *                          velocity and the Hubble term hubble_kms_per_cell * s (s = path length in cells), dust
+ *                          absorption included.
+ * One kernel launch; synchronous.  THOR_ERR_ARG for NULL / empty inputs or a bad velocity axis. */
+thor_status thor_raytrace(thor_ctx *ctx, long long n_rays, const float *org_xyz, const float *dir_xyz,
+                          double hubble_kms_per_cell, int n_v, double v_lo, double v_hi, float *out_column,
+                          float *out_tmean, float *out_tau);
+
 /* Static-lifetime or context-owned text of the last error (ctx may be NULL for create-time errors). */
 const char *thor_last_error(const thor_ctx *ctx);
 

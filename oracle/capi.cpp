@@ -176,4 +176,49 @@ double orc_run(int nx, int ny, int nz, int px, int py, int pz, double cell_cm,
     return std::chrono::duration<double>(t1 - t0).count();
 }
 
+// Ray-tracing operators (PAPER.md 3.5), one ray at a time in fp64 on the DDA's fp64 twin: projection Q = Int q w ds
+// (PAPER.md 3.5.1: column density with q = n_HI, w = 1; weighted mean Q / Q^ with q = T, w = n_HI) and the absorption
+// spectrum of Eq. 11 (PAPER.md 3.5.2): tau(V_j) = Int n sigma(nu(s), T) ds, the gas seeing the frequency shifted by
+// its line-of-sight velocity and the Hubble term Hc * s (s in cells; midpoint of each face-to-face segment), with
+// piecewise-constant cells.  Rays run from their origin to the first box face.
+void orc_raytrace(int nx, int ny, int nz, double cell_cm, const float* nHI, const float* T, const float* vx,
+                  const float* vy, const float* vz, const float* kdust, int64_t n_rays, const float* org,
+                  const float* dir, double hubble, int n_v, double v_lo, double v_hi, double* out_column,
+                  double* out_tmean, double* out_tau) {
+    Grid g{{{nx, ny, nz}, {false, false, false}}, cell_cm, nHI, T, vx, vy, vz, kdust};
+    for (int64_t i = 0; i < n_rays; ++i) {
+        Ray<double> r;
+        const double pos[3] = {org[3 * i], org[3 * i + 1], org[3 * i + 2]};
+        dda_locate(r, g.dims, pos);
+        const double k[3] = {dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
+        r.set_direction(k);
+        double col = 0, tn = 0, s_path = 0;
+        if (out_tau) for (int j = 0; j < n_v; ++j) out_tau[i * n_v + j] = 0.0;
+        for (;;) {
+            double len;
+            const int ex = dda_next_face(r, g.dims, len);
+            if (std::isinf(len)) break;
+            const CellProps cp = fetch_cell(g, r.c);
+            col += cp.n * len;
+            tn += cp.n * cp.T * len;
+            if (out_tau && (cp.n > 0 || cp.kd > 0)) {
+                const double vgas = dot3(cp.v, k) + hubble * (s_path + 0.5 * len);
+                const double vth = vth_kms(cp.T), a = voigt_a(cp.T);
+                for (int j = 0; j < n_v; ++j) {
+                    const double V = v_lo + (j + 0.5) * (v_hi - v_lo) / n_v;
+                    const double kl = cp.n > 0 ? cp.n * sigma0_cm2(cp.T) * voigt_H(a, (V - vgas) / vth) * cell_cm : 0.0;
+                    out_tau[i * n_v + j] += (kl + cp.kd * cell_cm) * len;
+                }
+            }
+            s_path += len;
+            const int s = r.k[ex] > 0 ? 1 : -1;
+            const int cn = r.c[ex] + s;
+            if (cn < 0 || cn >= g.dims.n[ex]) break;
+            dda_cross(r, g.dims, ex, len);
+        }
+        if (out_column) out_column[i] = col * cell_cm;
+        if (out_tmean) out_tmean[i] = col > 0 ? tn / col : 0.0;
+    }
+}
+
 }  // extern "C"

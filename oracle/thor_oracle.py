@@ -85,6 +85,8 @@ def lib():
         L.orc_dipole_mu.argtypes = [d]
         L.orc_scatter_once.argtypes = [d, d, d, i32, u64, u64, i64, P, P]
         L.orc_dda_trace.argtypes = [i32] * 6 + [i64, P, P, i64, i32, P, P, P, P, P]
+        L.orc_raytrace.restype = None
+        L.orc_raytrace.argtypes = [i32, i32, i32, d] + [P] * 6 + [i64, P, P, d, i32, d, d, P, P, P]
         L.orc_run.restype = d
         L.orc_run.argtypes = [i32] * 6 + [d] + [P] * 6 + [i64, P, P, P, P, u64, u64] + [P] * 5
         _lib = L
@@ -211,3 +213,22 @@ def run(grid, sources, opts, n_photons, seed, want_raw=True):
                          _ptr(spectrum), _ptr(hist), _ptr(counters), _ptr(cube), _ptr(raw))
     return dict(spectrum=spectrum, nscat_hist=hist, counters=dict(zip(COUNTER_NAMES, (int(c) for c in counters))),
                 cube=cube, raw=raw, seconds=secs)
+
+
+def raytrace(grid, origins, dirs, n_v=0, v_lo=0.0, v_hi=1.0, hubble_kms_per_cell=0.0):
+    """Projection and absorption spectra along rays (PAPER.md 3.5.1-3.5.2, Eq. 11).  Returns dict(column, tmean[, tau])."""
+    f = lambda k: None if grid.get(k) is None else np.ascontiguousarray(grid[k], np.float32)
+    nHI, T, vx, vy, vz, kd = (f(k) for k in ("nHI", "T", "vx", "vy", "vz", "kdust"))
+    org = np.ascontiguousarray(origins, np.float32).reshape(-1, 3)
+    dr = np.ascontiguousarray(dirs, np.float32).reshape(-1, 3)
+    n = org.shape[0]
+    col = np.zeros(n, np.float64)
+    tm = np.zeros(n, np.float64)
+    tau = np.zeros((n, n_v), np.float64) if n_v > 0 else None
+    lib().orc_raytrace(int(grid["nx"]), int(grid["ny"]), int(grid["nz"]), float(grid["cell_cm"]), _ptr(nHI), _ptr(T),
+                       _ptr(vx), _ptr(vy), _ptr(vz), _ptr(kd), n, _ptr(org), _ptr(dr), float(hubble_kms_per_cell),
+                       int(n_v), float(v_lo), float(v_hi), _ptr(col), _ptr(tm), _ptr(tau))
+    out = dict(column=col, tmean=tm)
+    if tau is not None:
+        out["tau"] = tau
+    return out

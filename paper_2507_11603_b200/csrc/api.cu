@@ -13,6 +13,9 @@
 
 namespace thor {
 cudaError_t launch_walk(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out);
+cudaError_t launch_raytrace(const WalkParams& p, long long n_rays, const float* org, const float* dir, float hubble,
+                            int n_v, float v_lo, float dv, float* out_column, float* out_tmean, float* out_tau,
+                            cudaStream_t stream);
 cudaError_t launch_pack_fields(const float* nHI, const float* T, const float* vx, const float* vy, const float* vz,
                                const float* kdust, long long n, float4* out, cudaStream_t stream);
 cudaError_t launch_validate_fields(const float* nHI, const float* T, const float* vx, const float* vy, const float* vz,
@@ -335,6 +338,29 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
         if (t[1] != ~0ull && t[1] >= t[0]) ctx->last_feed_ms = (float)((double)(t[1] - t[0]) * 1e-6);
     }
     ctx->last = o; ctx->last_n = n_photons; ctx->have_run = true;
+    return THOR_OK;
+}
+
+extern "C" thor_status thor_raytrace(thor_ctx* ctx, long long n_rays, const float* org_xyz, const float* dir_xyz,
+                                     double hubble_kms_per_cell, int n_v, double v_lo, double v_hi, float* out_column,
+                                     float* out_tmean, float* out_tau) {
+    if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_raytrace: ctx is NULL");
+    if (n_rays <= 0 || !org_xyz || !dir_xyz) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: no rays");
+    if (!out_column && !out_tmean && !out_tau) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: no output requested");
+    if (out_tau && (n_v <= 0 || !(v_hi > v_lo))) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: bad velocity axis");
+    if (!std::isfinite(hubble_kms_per_cell)) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: bad Hubble term");
+    const thor::LyaConstants K = thor::lya_constants();
+    thor::WalkParams p{};
+    p.g = ctx->g;
+    p.nHI = ctx->f[0]; p.T = ctx->f[1]; p.vx = ctx->f[2]; p.vy = ctx->f[3]; p.vz = ctx->f[4]; p.kdust = ctx->f[5];
+    p.packed = ctx->d_packed; p.has_dust = ctx->has_dust ? 1 : 0;
+    p.sig_cell = (float)(K.c_sig * ctx->cell_cm);
+    p.c_a = (float)K.c_a; p.c_vth = (float)K.c_vth; p.inv_c_vth = (float)(1.0 / K.c_vth);
+    p.cell_cm = (float)ctx->cell_cm;
+    CU(cudaSetDevice(ctx->device));
+    CU(thor::launch_raytrace(p, n_rays, org_xyz, dir_xyz, (float)hubble_kms_per_cell, out_tau ? n_v : 0, (float)v_lo,
+                             out_tau ? (float)((v_hi - v_lo) / n_v) : 0.f, out_column, out_tmean, out_tau, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
     return THOR_OK;
 }
 

@@ -284,6 +284,63 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
         if (sh.spectrum[i]) atomicAdd(p.spectrum + i, (unsigned long long)sh.spectrum[i]);
 }
 
+// ---- ray-tracing operators on the same DDA + gather + Voigt (PAPER.md 3.5) ----
+// One thread per ray, marched from its origin to the first box face.  Projection (PAPER.md 3.5.1): Q = Int q w ds with
+// q = n_HI, w = 1 (column density, cm^-2) and q = T, w = n_HI (density-weighted temperature Q / Q^).  Absorption
+// spectrum (PAPER.md 3.5.2, Eq. 11): tau(V_j) = Int n sigma(nu(s), T) ds with the gas seeing the sight-line
+// frequency shifted by its line-of-sight velocity v.k and the Hubble term H s; piecewise-constant cells, midpoint of
+// each segment for the Hubble term.
+__global__ void raytrace_kernel(const __grid_constant__ WalkParams p, long long n_rays, const float* __restrict__ org,
+                                const float* __restrict__ dir, float hubble, int n_v, float v_lo, float dv,
+                                float* __restrict__ out_column, float* __restrict__ out_tmean, float* __restrict__ out_tau) {
+    __shared__ float2 s_tab[VOIGT_NODES];
+    voigt_table_load(s_tab);
+    __syncthreads();
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_rays) return;
+    Ray r;
+    dda_locate(r, p.g, org[3 * i], org[3 * i + 1], org[3 * i + 2]);
+    ray_set_direction(r, dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]);
+    float col = 0.f, tn = 0.f, s_path = 0.f;
+    float* tau = out_tau ? out_tau + i * n_v : nullptr;
+    if (tau) for (int j = 0; j < n_v; ++j) tau[j] = 0.f;
+    for (;;) {
+        float len;
+        const int ex = dda_next_face(r, p.g, len);
+        if (!(len < CUDART_INF_F)) break;
+        Cell c = load_cell_raw(p, dda_linear(r, p.g));
+        const float n = c.nsig, T = c.a;
+        col += n * len;
+        tn += n * T * len;
+        if (tau) {
+            derive_cell(p, c);
+            const float vgas = c.vx * r.kx + c.vy * r.ky + c.vz * r.kz + hubble * (s_path + 0.5f * len);
+            if (c.nsig > 0.f || c.kd > 0.f)
+                for (int j = 0; j < n_v; ++j) {
+                    const float V = v_lo + ((float)j + 0.5f) * dv;
+                    const float kl = c.nsig > 0.f ? c.nsig * voigt_H(s_tab, c.a, (V - vgas) * c.inv_vth) : 0.f;
+                    tau[j] += (kl + c.kd) * len;
+                }
+        }
+        s_path += len;
+        const float ke = ex == 0 ? r.kx : ex == 1 ? r.ky : r.kz;
+        const int cn = (ex == 0 ? r.cx : ex == 1 ? r.cy : r.cz) + (ke > 0.f ? 1 : -1);
+        const int nn = ex == 0 ? p.g.nx : ex == 1 ? p.g.ny : p.g.nz;
+        if (cn < 0 || cn >= nn) break;                        // rays end at the first box face, periodic or not
+        dda_cross(r, p.g, ex, len);
+    }
+    if (out_column) out_column[i] = col * p.cell_cm;
+    if (out_tmean) out_tmean[i] = col > 0.f ? tn / col : 0.f;
+}
+
+cudaError_t launch_raytrace(const WalkParams& p, long long n_rays, const float* org, const float* dir, float hubble,
+                            int n_v, float v_lo, float dv, float* out_column, float* out_tmean, float* out_tau,
+                            cudaStream_t stream) {
+    raytrace_kernel<<<(unsigned)((n_rays + 127) / 128), 128, 0, stream>>>(p, n_rays, org, dir, hubble, n_v, v_lo, dv,
+                                                                         out_column, out_tmean, out_tau);
+    return cudaGetLastError();
+}
+
 // Launch configuration: one persistent grid, blocks = SMs x resident blocks per SM.  The kernel is specialised at
 // compile time on (Hubble drift, peel-off) so that the common static, no-peel walk carries neither, and on the
 // register budget: 3 CTAs of 256 threads per SM (<= 80 registers) when the grid fits the 126 MB L2 and the walk is

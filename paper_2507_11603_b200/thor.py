@@ -19,7 +19,7 @@ COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "
 RAW_DTYPE = np.dtype([("V", "<f4"), ("nscat", "<u4"), ("status", "<i4"), ("kx", "<f4"), ("ky", "<f4"), ("kz", "<f4")])
 
 EXPORTS = ["thor_grid_create", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run",
-           "thor_last_run_ms", "thor_last_run_feed_ms", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_dda_trace",
+           "thor_last_run_ms", "thor_last_run_feed_ms", "thor_raytrace", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_dda_trace",
            "thor_unit_voigt", "thor_unit_scatter"]
 
 
@@ -68,6 +68,7 @@ def lib():
         L.thor_run.argtypes = [P, C.c_ulonglong, C.c_ulonglong, C.POINTER(Opts)]
         L.thor_last_run_ms.argtypes = [P, C.POINTER(f)]
         L.thor_last_run_feed_ms.argtypes = [P, C.POINTER(f)]
+        L.thor_raytrace.argtypes = [P, i64, P, P, d, i32, d, d, P, P, P]
         L.thor_tally_get.argtypes = [P, i32, P, C.c_size_t, C.POINTER(C.c_size_t)]
         L.thor_last_error.argtypes = [P]
         L.thor_last_error.restype = C.c_char_p
@@ -185,6 +186,24 @@ class Context:
         ms = C.c_float()
         _check(lib().thor_last_run_ms(self._ctx, C.byref(ms)), self._ctx)
         return ms.value
+
+    def raytrace(self, origins, dirs, n_v=0, v_lo=0.0, v_hi=1.0, hubble_kms_per_cell=0.0):
+        """Projection / absorption spectra along rays (thor_raytrace).  Returns dict(column, tmean[, tau])."""
+        import torch
+        org = torch.from_numpy(np.ascontiguousarray(origins, np.float32)).cuda()
+        dr = torch.from_numpy(np.ascontiguousarray(dirs, np.float32)).cuda()
+        n = org.shape[0]
+        col = torch.empty(n, dtype=torch.float32, device="cuda")
+        tm = torch.empty(n, dtype=torch.float32, device="cuda")
+        tau = torch.empty((n, n_v), dtype=torch.float32, device="cuda") if n_v > 0 else None
+        _check(lib().thor_raytrace(self._ctx, n, C.c_void_p(org.data_ptr()), C.c_void_p(dr.data_ptr()),
+                                   float(hubble_kms_per_cell), int(n_v), float(v_lo), float(v_hi),
+                                   C.c_void_p(col.data_ptr()), C.c_void_p(tm.data_ptr()),
+                                   C.c_void_p(tau.data_ptr()) if tau is not None else None), self._ctx)
+        out = dict(column=col.cpu().numpy(), tmean=tm.cpu().numpy())
+        if tau is not None:
+            out["tau"] = tau.cpu().numpy()
+        return out
 
     def last_run_feed_ms(self):
         ms = C.c_float()
