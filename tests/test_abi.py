@@ -56,6 +56,8 @@ def test_argument_errors_are_status_codes(thor):
     assert L.thor_run(None, 1, 1, None) == 1
     assert L.thor_tally_get(None, 0, None, 0, None) == 1
     assert L.thor_unit_voigt(0, p, p, p, None) == 1
+    assert L.thor_raytrace(None, 1, p, p, 0.0, 0, 0.0, 1.0, p, None, None) == 1
+    assert L.thor_last_run_feed_ms(None, None) == 1
     L.thor_grid_destroy(None)   # no-op
 
 
