@@ -193,7 +193,7 @@ def main():
     spec_dev = torch.zeros(opts["spec_bins"] + 2, dtype=torch.int64, device="cuda")
     cnt_dev = torch.zeros(len(thor.COUNTER_NAMES), dtype=torch.int64, device="cuda")
 
-    feed_ms = []
+    feed_ms, max_nscat = [], []
 
     def step(i):
         # rank r walks photon ids [r n, (r+1) n) of step i's seed; tallies summed over ranks (the one exchange step)
@@ -202,6 +202,7 @@ def main():
         ctx.tally_to_device(thor.TALLY_COUNTERS, cnt_dev)
         shard.allreduce_tallies([spec_dev, cnt_dev])               # no-op at N = 1
         feed_ms.append(ctx.last_run_feed_ms())
+        max_nscat.append(ctx.last_run_max_nscat())
         return ctx.last_run_ms()
 
     for i in range(args.warmup):
@@ -249,6 +250,9 @@ def main():
         # the launch only drains the packets in flight, and lasts as long as its longest single packet
         "phases": {"feed_ms_per_step": float(np.mean(feed_ms[-args.steps:])),
                    "drain_ms_per_step": kernel_ms / args.steps - float(np.mean(feed_ms[-args.steps:])),
+                   "longest_packet_scatterings": [int(v) for v in max_nscat[-args.steps:]],
+                   "drain_ns_per_scattering_of_longest_packet": float(np.mean([1e6 * (k - f) / max(1, m) for k, f, m in
+                                                                               zip(kern_ms, feed_ms[-args.steps:], max_nscat[-args.steps:])])),
                    "source": "device %globaltimer at kernel entry and when the photon counter is first found exhausted (thor_last_run_feed_ms)"},
         "counters": c,
     }

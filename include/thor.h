@@ -112,6 +112,10 @@ thor_status thor_last_run_ms(const thor_ctx *ctx, float *ms);
  * the packets in flight, whose length is set by the longest single packet. */
 thor_status thor_last_run_feed_ms(const thor_ctx *ctx, float *ms);
 
+/* Largest scattering count of any single packet of the last thor_run: the longest dependent chain, which bounds the
+ * drain phase from below. */
+thor_status thor_last_run_max_nscat(const thor_ctx *ctx, unsigned long long *n);
+
 /* tallies */
 #define THOR_TALLY_SPECTRUM 0   /* uint64[spec_bins + 2]: bins, then underflow, overflow */
 #define THOR_TALLY_NSCAT_HIST 1 /* uint64[64]: bin 0: nscat = 0; bin b: 2^(b-1) <= nscat < 2^b */

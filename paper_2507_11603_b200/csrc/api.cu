@@ -48,6 +48,7 @@ struct thor_ctx {
     thor_opts last{};
     unsigned long long last_n = 0;
     float last_ms = 0.f, last_feed_ms = 0.f;
+    unsigned long long last_max_nscat = 0;
     int last_blocks = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     std::string err;
@@ -56,7 +57,7 @@ struct thor_ctx {
 static thread_local std::string g_err;
 
 static constexpr size_t SMALL_NEXT = 0, SMALL_COUNTERS = 1, SMALL_HIST = SMALL_COUNTERS + thor::N_COUNTERS,
-                        SMALL_SPEC = SMALL_HIST + 64, SMALL_TIMES = SMALL_SPEC + 4096 + 2, SMALL_TOTAL = SMALL_TIMES + 2;
+                        SMALL_SPEC = SMALL_HIST + 64, SMALL_TIMES = SMALL_SPEC + 4096 + 2, SMALL_MAXN = SMALL_TIMES + 2, SMALL_TOTAL = SMALL_MAXN + 1;
 
 static thor_status fail(thor_ctx* c, thor_status s, const std::string& msg) {
     if (c) c->err = msg;
@@ -319,6 +320,8 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     CU(cudaMemsetAsync(ctx->d_small + SMALL_TIMES, 0xFF, 2 * sizeof(unsigned long long), ctx->stream));
     p.next_photon = ctx->d_small + SMALL_NEXT;
     p.t_start = ctx->d_small + SMALL_TIMES;
+    p.max_nscat = ctx->d_small + SMALL_MAXN;
+    CU(cudaMemsetAsync(ctx->d_small + SMALL_MAXN, 0, sizeof(unsigned long long), ctx->stream));
     p.t_dry = ctx->d_small + SMALL_TIMES + 1;
     p.counters = ctx->d_small + SMALL_COUNTERS;
     p.nscat_hist = ctx->d_small + SMALL_HIST;
@@ -332,10 +335,11 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     CU(cudaEventElapsedTime(&ctx->last_ms, ctx->ev0, ctx->ev1));
     ctx->last_feed_ms = 0.f;
     if (n_photons > 0) {
-        unsigned long long t[2] = {0, 0};
+        unsigned long long t[3] = {0, 0, 0};                    // t_start, t_dry, max_nscat are adjacent
         CU(cudaMemcpyAsync(t, ctx->d_small + SMALL_TIMES, sizeof t, cudaMemcpyDeviceToHost, ctx->stream));
         CU(cudaStreamSynchronize(ctx->stream));
         if (t[1] != ~0ull && t[1] >= t[0]) ctx->last_feed_ms = (float)((double)(t[1] - t[0]) * 1e-6);
+        ctx->last_max_nscat = t[2];
     }
     ctx->last = o; ctx->last_n = n_photons; ctx->have_run = true;
     return THOR_OK;
@@ -368,6 +372,13 @@ extern "C" thor_status thor_last_run_ms(const thor_ctx* ctx, float* ms) {
     if (!ctx || !ms) return fail(nullptr, THOR_ERR_ARG, "thor_last_run_ms: NULL argument");
     if (!ctx->have_run) return fail(const_cast<thor_ctx*>(ctx), THOR_ERR_STATE, "thor_last_run_ms: no run yet");
     *ms = ctx->last_ms;
+    return THOR_OK;
+}
+
+extern "C" thor_status thor_last_run_max_nscat(const thor_ctx* ctx, unsigned long long* n) {
+    if (!ctx || !n) return fail(nullptr, THOR_ERR_ARG, "thor_last_run_max_nscat: NULL argument");
+    if (!ctx->have_run) return fail(const_cast<thor_ctx*>(ctx), THOR_ERR_STATE, "thor_last_run_max_nscat: no run yet");
+    *n = ctx->last_max_nscat;
     return THOR_OK;
 }
 

@@ -67,6 +67,7 @@ struct WalkParams {
     unsigned long long id_offset, n_photons, seed, max_scatter;
     // work distribution + tallies (device)
     unsigned long long* next_photon;     // a14: global atomic photon counter
+    unsigned long long* max_nscat;       // max over packets of the scattering count (the longest dependent chain)
     unsigned long long* t_start;         // min over CTAs of %globaltimer at kernel entry (ns)
     unsigned long long* t_dry;           // min over warps of %globaltimer when the photon counter was found exhausted
     unsigned long long* spectrum;        // [spec_bins + 2]

@@ -32,6 +32,7 @@ struct BlockTallies {
     float2 voigt[VOIGT_NODES];
     unsigned long long counters[N_COUNTERS];
     unsigned int nscat_hist[64];
+    unsigned int max_nscat;
     unsigned int spectrum[MAX_SPEC_BINS + 2];
 };
 
@@ -45,6 +46,7 @@ __device__ __forceinline__ void tally_finish(const WalkParams& p, BlockTallies& 
     atomicAdd(&sh.counters[CT_REJ_ITERS], (unsigned long long)rej_iters);
     const int hb = nscat == 0 ? 0 : 32 - __clz(nscat);       // bin b: 2^(b-1) <= nscat < 2^b
     atomicAdd(&sh.nscat_hist[hb], 1u);
+    atomicMax(&sh.max_nscat, nscat);
     if ((status == CT_ESCAPED || status == CT_TERMINATED) && p.spec_bins > 0) {
         const float val = p.spec_mode == 0 ? V * p.spec_inv_vth_ref : -V;
         const float b = floorf((val - p.spec_lo) * p.spec_inv_width);
@@ -61,6 +63,7 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
     voigt_table_load(sh.voigt);
     for (int i = threadIdx.x; i < N_COUNTERS; i += blockDim.x) sh.counters[i] = 0ull;
     for (int i = threadIdx.x; i < 64; i += blockDim.x) sh.nscat_hist[i] = 0u;
+    if (threadIdx.x == 0) sh.max_nscat = 0u;
     for (int i = threadIdx.x; i < p.spec_bins + 2; i += blockDim.x) sh.spectrum[i] = 0u;
     __syncthreads();
 
@@ -280,6 +283,7 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
         if (sh.counters[i]) atomicAdd(p.counters + i, sh.counters[i]);
     for (int i = threadIdx.x; i < 64; i += blockDim.x)
         if (sh.nscat_hist[i]) atomicAdd(p.nscat_hist + i, (unsigned long long)sh.nscat_hist[i]);
+    if (threadIdx.x == 0 && sh.max_nscat) atomicMax(p.max_nscat, (unsigned long long)sh.max_nscat);
     for (int i = threadIdx.x; i < p.spec_bins + 2; i += blockDim.x)
         if (sh.spectrum[i]) atomicAdd(p.spectrum + i, (unsigned long long)sh.spectrum[i]);
 }

@@ -19,7 +19,7 @@ COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "
 RAW_DTYPE = np.dtype([("V", "<f4"), ("nscat", "<u4"), ("status", "<i4"), ("kx", "<f4"), ("ky", "<f4"), ("kz", "<f4")])
 
 EXPORTS = ["thor_grid_create", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run",
-           "thor_last_run_ms", "thor_last_run_feed_ms", "thor_raytrace", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_dda_trace",
+           "thor_last_run_ms", "thor_last_run_feed_ms", "thor_last_run_max_nscat", "thor_raytrace", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_dda_trace",
            "thor_unit_voigt", "thor_unit_scatter"]
 
 
@@ -68,6 +68,7 @@ def lib():
         L.thor_run.argtypes = [P, C.c_ulonglong, C.c_ulonglong, C.POINTER(Opts)]
         L.thor_last_run_ms.argtypes = [P, C.POINTER(f)]
         L.thor_last_run_feed_ms.argtypes = [P, C.POINTER(f)]
+        L.thor_last_run_max_nscat.argtypes = [P, C.POINTER(C.c_ulonglong)]
         L.thor_raytrace.argtypes = [P, i64, P, P, d, i32, d, d, P, P, P]
         L.thor_tally_get.argtypes = [P, i32, P, C.c_size_t, C.POINTER(C.c_size_t)]
         L.thor_last_error.argtypes = [P]
@@ -204,6 +205,11 @@ class Context:
         if tau is not None:
             out["tau"] = tau.cpu().numpy()
         return out
+
+    def last_run_max_nscat(self):
+        n = C.c_ulonglong()
+        _check(lib().thor_last_run_max_nscat(self._ctx, C.byref(n)), self._ctx)
+        return n.value
 
     def last_run_feed_ms(self):
         ms = C.c_float()

@@ -344,6 +344,7 @@ def test_edge_cases(thor):
         c = ctx.counters()
         assert c["escaped"] + c["capped"] == 33 and c["capped"] > 0
         assert ctx.raw()["nscat"].max() <= 3
+        assert ctx.last_run_max_nscat() == int(ctx.raw()["nscat"].max())     # the longest dependent chain of the run
         with pytest.raises(thor.ThorError):
             ctx.run(10, 1, dict(w["opts"], spec_bins=5000))
         with pytest.raises(thor.ThorError):
