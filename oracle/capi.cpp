@@ -221,4 +221,53 @@ void orc_raytrace(int nx, int ny, int nz, double cell_cm, const float* nHI, cons
     }
 }
 
+// Volume rendering (PAPER.md 3.5.3, Eq. 12): C = Int_0^L c(s) mu(s) exp(-Int_0^s mu dt) ds along each ray, observer at
+// the ray origin.  Transfer function as in PAPER.md:510 (Gaussian peaks in log10 T, brightness weighted by density):
+// g_p = exp(-(log10 T - c_p)^2 / (2 s_p^2)); mu = w Sum_p A_p g_p per cell length, c mu = w Sum_p A_p g_p (R,G,B)_p,
+// w = n_HI / n_ref (n_ref > 0) or 1 (n_ref = 0).  Cells are piecewise constant, so each face-to-face
+// segment of length l integrates exactly: C += Tr c (1 - e^{-mu l}), Tr *= e^{-mu l} (reading A25).  Output per ray:
+// (C_R, C_G, C_B, 1 - Tr).  peaks: double[n_peaks][6] = {c_p, s_p, R, G, B, A}.
+void orc_volume_render(int nx, int ny, int nz, const float* nHI, const float* T, int64_t n_rays, const float* org,
+                       const float* dir, int n_peaks, const double* peaks, double n_ref, double* out_rgba) {
+    Grid g{{{nx, ny, nz}, {false, false, false}}, 1.0, nHI, T, nullptr, nullptr, nullptr, nullptr};
+    for (int64_t i = 0; i < n_rays; ++i) {
+        Ray<double> r;
+        const double pos[3] = {org[3 * i], org[3 * i + 1], org[3 * i + 2]};
+        dda_locate(r, g.dims, pos);
+        const double k[3] = {dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
+        r.set_direction(k);
+        double C[3] = {0, 0, 0}, Tr = 1.0;
+        for (;;) {
+            double len;
+            const int ex = dda_next_face(r, g.dims, len);
+            if (std::isinf(len)) break;
+            const int64_t idx = ((int64_t)r.c[2] * ny + r.c[1]) * nx + r.c[0];
+            const double n = nHI[idx], Tc = T[idx];
+            const double w = n_ref > 0 ? n / n_ref : 1.0;
+            if (w > 0 && Tc > 0) {
+                const double lt = std::log10(Tc);
+                double mu = 0, e[3] = {0, 0, 0};
+                for (int p = 0; p < n_peaks; ++p) {
+                    const double* q = peaks + 6 * p;
+                    const double z = (lt - q[0]) / q[1];
+                    const double ag = w * q[5] * std::exp(-0.5 * z * z);
+                    mu += ag;
+                    for (int c = 0; c < 3; ++c) e[c] += ag * q[2 + c];
+                }
+                if (mu > 0) {
+                    const double att = std::exp(-mu * len);
+                    for (int c = 0; c < 3; ++c) C[c] += Tr * (e[c] / mu) * (1.0 - att);
+                    Tr *= att;
+                }
+            }
+            const int s = r.k[ex] > 0 ? 1 : -1;
+            const int cn = r.c[ex] + s;
+            if (cn < 0 || cn >= g.dims.n[ex]) break;
+            dda_cross(r, g.dims, ex, len);
+        }
+        for (int c = 0; c < 3; ++c) out_rgba[4 * i + c] = C[c];
+        out_rgba[4 * i + 3] = 1.0 - Tr;
+    }
+}
+
 }  // extern "C"

@@ -87,6 +87,8 @@ def lib():
         L.orc_dda_trace.argtypes = [i32] * 6 + [i64, P, P, i64, i32, P, P, P, P, P]
         L.orc_raytrace.restype = None
         L.orc_raytrace.argtypes = [i32, i32, i32, d] + [P] * 6 + [i64, P, P, d, i32, d, d, P, P, P]
+        L.orc_volume_render.restype = None
+        L.orc_volume_render.argtypes = [i32, i32, i32, P, P, i64, P, P, i32, P, d, P]
         L.orc_run.restype = d
         L.orc_run.argtypes = [i32] * 6 + [d] + [P] * 6 + [i64, P, P, P, P, u64, u64] + [P] * 5
         _lib = L
@@ -231,4 +233,18 @@ def raytrace(grid, origins, dirs, n_v=0, v_lo=0.0, v_hi=1.0, hubble_kms_per_cell
     out = dict(column=col, tmean=tm)
     if tau is not None:
         out["tau"] = tau
+    return out
+
+
+def volume_render(grid, origins, dirs, peaks, n_ref=0.0):
+    """Volume rendering (PAPER.md 3.5.3, Eq. 12) with Gaussian-peak transfer function in log10 T.
+    peaks: rows (log10 T centre, width in dex, R, G, B, A).  Returns float64[n][4] = (C_R, C_G, C_B, opacity)."""
+    nHI = np.ascontiguousarray(grid["nHI"], np.float32)
+    T = np.ascontiguousarray(grid["T"], np.float32)
+    org = np.ascontiguousarray(origins, np.float32).reshape(-1, 3)
+    dr = np.ascontiguousarray(dirs, np.float32).reshape(-1, 3)
+    pk = np.ascontiguousarray(peaks, np.float64).reshape(-1, 6)
+    out = np.zeros((org.shape[0], 4), np.float64)
+    lib().orc_volume_render(int(grid["nx"]), int(grid["ny"]), int(grid["nz"]), _ptr(nHI), _ptr(T), org.shape[0],
+                            _ptr(org), _ptr(dr), pk.shape[0], _ptr(pk), float(n_ref), _ptr(out))
     return out

@@ -88,3 +88,94 @@ def test_absorption_spectrum_hubble_flow(oracle):
     assert np.allclose(r["tau"][0], expect, rtol=5e-3)
     # absorption is strongest where the line sweeps through the sight line: V between 0 and Hc * N
     assert 0.0 <= V[int(np.argmax(r["tau"][0]))] <= Hc * N
+
+
+# ---- volume rendering (PAPER.md 3.5.3, Eq. 12) ----
+PEAKS = np.array([[4.3, 0.15, 0.1, 0.3, 1.0, 0.8],      # cold: blue      (log10 T centre, width [dex], R, G, B, A)
+                  [5.0, 0.20, 1.0, 0.6, 0.1, 0.5],      # warm: orange
+                  [5.5, 0.10, 1.0, 0.1, 0.1, 1.2]])     # hot: red
+
+
+def _tf(T, n, n_ref):
+    """Transfer function written out independently: returns (mu, c_rgb)."""
+    lt = math.log10(T)
+    gp = PEAKS[:, 5] * np.exp(-0.5 * ((lt - PEAKS[:, 0]) / PEAKS[:, 1]) ** 2) * (n / n_ref if n_ref > 0 else 1.0)
+    mu = gp.sum()
+    return mu, (gp[:, None] * PEAKS[:, 2:5]).sum(0) / mu
+
+
+def test_volume_render_uniform_medium_closed_form(oracle):
+    """Constant c and mu: Eq. 12 integrates to C = c (1 - e^{-mu L}) with L the analytic chord."""
+    rng = np.random.default_rng(3)
+    org = (rng.random((100, 3)) * N).astype(np.float32)
+    d = rng.standard_normal((100, 3))
+    d = (d / np.linalg.norm(d, axis=1)[:, None]).astype(np.float32)
+    T, n, n_ref = 10 ** 4.4, 0.02, 0.1
+    g = _uniform_grid(n, T)
+    out = oracle.volume_render(g, org, d, PEAKS, n_ref=n_ref)
+    mu, c = _tf(float(np.float32(T)), float(np.float32(n)), n_ref)
+    for o, k, rgba in zip(org, d, out):
+        L = _chord(o.astype(float), k.astype(float))
+        assert rgba[:3] == pytest.approx(c * (1 - math.exp(-mu * L)), rel=1e-6)
+        assert rgba[3] == pytest.approx(1 - math.exp(-mu * L), rel=1e-6)
+    # no density weighting: mu does not depend on n
+    out1 = oracle.volume_render(g, org[:1], d[:1], PEAKS, n_ref=0.0)
+    mu1, _ = _tf(float(np.float32(T)), 1.0, 0.0)
+    assert out1[0, 3] == pytest.approx(1 - math.exp(-mu1 * _chord(org[0].astype(float), d[0].astype(float))), rel=1e-6)
+
+
+def test_volume_render_front_slab_attenuates_back_slab(oracle):
+    """Observer at s = 0: the near slab is seen unattenuated, the far slab through e^{-mu1 L1}; reversing the ray
+    swaps the roles (catches a back-to-front / front-to-back mix-up)."""
+    g = _uniform_grid(1.0, 10 ** 4.3)
+    g["T"][8:, :, :] = 10 ** 5.5                       # z >= 8 hot (red), z < 8 cold (blue)
+    mu1, c1 = _tf(float(g["T"][0, 0, 0]), 1.0, 0.0)
+    mu2, c2 = _tf(float(g["T"][8, 0, 0]), 1.0, 0.0)
+    fwd = oracle.volume_render(g, [[5.5, 6.5, 0.0]], [[0, 0, 1]], PEAKS)[0]
+    bwd = oracle.volume_render(g, [[5.5, 6.5, 16.0]], [[0, 0, -1]], PEAKS)[0]
+    a1, a2 = math.exp(-mu1 * 8), math.exp(-mu2 * 8)
+    assert fwd[:3] == pytest.approx(c1 * (1 - a1) + a1 * c2 * (1 - a2), rel=1e-12)
+    assert bwd[:3] == pytest.approx(c2 * (1 - a2) + a2 * c1 * (1 - a1), rel=1e-12)
+    assert fwd[3] == pytest.approx(1 - a1 * a2, rel=1e-12) and bwd[3] == pytest.approx(fwd[3], rel=1e-12)
+    assert not np.allclose(fwd[:3], bwd[:3], rtol=1e-3)
+
+
+def test_volume_render_matches_quadrature_of_eq12(oracle):
+    """Eq. 12 by nested adaptive quadrature on a random 6^3 grid, the fields looked up by floor(position) (no DDA)."""
+    rng = np.random.default_rng(11)
+    n6 = 6
+    g = dict(nx=n6, ny=n6, nz=n6, periodic=(0, 0, 0), cell_cm=CELL,
+             nHI=np.exp(rng.normal(0, 1, (n6, n6, n6))).astype(np.float32),
+             T=(10 ** rng.uniform(4.0, 5.8, (n6, n6, n6))).astype(np.float32))
+    n_ref = 2.0
+    scale = 0.5                                        # keep the total optical depth O(1)
+    pk = PEAKS.copy()
+    pk[:, 5] *= scale
+    for o, k in [((0.3, 2.2, 4.1), (0.61, 0.35, -0.71)), ((5.9, 5.2, 0.4), (-0.7, -0.5, 0.51))]:
+        o = np.array(o, np.float32).astype(float)
+        k = np.array(k) / np.linalg.norm(k)
+        k = k.astype(np.float32).astype(float)
+        t_end = min(((n6 - o[i]) / k[i] if k[i] > 0 else (0 - o[i]) / k[i]) for i in range(3))
+
+        def mu_c(s):
+            c = np.clip(np.floor(o + s * k).astype(int), 0, n6 - 1)
+            T, n = float(g["T"][c[2], c[1], c[0]]), float(g["nHI"][c[2], c[1], c[0]])
+            lt = math.log10(T)
+            gp = pk[:, 5] * np.exp(-0.5 * ((lt - pk[:, 0]) / pk[:, 1]) ** 2) * n / n_ref
+            return gp.sum(), (gp[:, None] * pk[:, 2:5]).sum(0)
+
+        # breakpoints (face crossings) so that the adaptive rule sees the discontinuities
+        br = sorted({(f - o[i]) / k[i] for i in range(3) for f in range(n6 + 1) if 0 < (f - o[i]) / k[i] < t_end})
+        edges = [0.0] + br + [t_end]
+        tau_at = [0.0]
+        for a, b in zip(edges[:-1], edges[1:]):
+            tau_at.append(tau_at[-1] + integrate.quad(lambda s: mu_c(s)[0], a, b)[0])
+        C = np.zeros(3)
+        for j, (a, b) in enumerate(zip(edges[:-1], edges[1:])):
+            for ch in range(3):
+                f = lambda s: mu_c(s)[1][ch] * math.exp(-(tau_at[j] + mu_c(0.5 * (a + b))[0] * (s - a)))
+                C[ch] += integrate.quad(f, a, b)[0]
+        out = oracle.volume_render(g, [o], [k], pk, n_ref=n_ref)[0]
+        assert out[:3] == pytest.approx(C, rel=1e-7)
+        assert out[3] == pytest.approx(1 - math.exp(-tau_at[-1]), rel=1e-7)
+        assert 0.05 < out[3] < 0.999
