@@ -153,6 +153,18 @@ thor_status thor_raytrace(thor_ctx *ctx, long long n_rays, const float *org_xyz,
                           double hubble_kms_per_cell, int n_v, double v_lo, double v_hi, float *out_column,
                           float *out_tmean, float *out_tau);
 
+/* Volume rendering (PAPER.md 3.5.3, Eq. 12): C = Int_0^L c(s) mu(s) exp(-Int_0^s mu dt) ds along each ray, the observer
+ * at the ray origin, rays as in thor_raytrace.  Transfer function as in PAPER.md:510 (Gaussian peaks in log10 T,
+ * brightness weighted by density): peaks = HOST float[n_peaks][6] rows {log10 T centre, width [dex] > 0, R, G, B, A >= 0},
+ * 1 <= n_peaks <= THOR_MAX_TF_PEAKS (copied); g_p = exp(-(log10 T - c_p)^2 / (2 s_p^2)); absorption coefficient per
+ * cell length mu = w Sum_p A_p g_p, emission c mu = w Sum_p A_p g_p (R,G,B)_p, w = n_HI / n_ref, or 1 if n_ref == 0.
+ * Cells are piecewise constant, each face-to-face segment is integrated exactly (reading A25).
+ * out_rgba: DEVICE float[n_rays][4] = (C_R, C_G, C_B, 1 - exp(-Int mu)).  One kernel launch; synchronous.
+ * THOR_ERR_ARG for NULL / empty inputs, n_peaks out of range, a non-positive width, negative A or n_ref. */
+#define THOR_MAX_TF_PEAKS 8
+thor_status thor_volume_render(thor_ctx *ctx, long long n_rays, const float *org_xyz, const float *dir_xyz,
+                               int n_peaks, const float *peaks, double n_ref, float *out_rgba);
+
 /* Static-lifetime or context-owned text of the last error (ctx may be NULL for create-time errors). */
 const char *thor_last_error(const thor_ctx *ctx);
 

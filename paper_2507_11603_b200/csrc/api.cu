@@ -13,6 +13,8 @@
 
 namespace thor {
 cudaError_t launch_walk(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out);
+cudaError_t launch_volume_render(const WalkParams& p, const TransferFn& tf, long long n_rays, const float* org,
+                                 const float* dir, float* out_rgba, cudaStream_t stream);
 cudaError_t launch_raytrace(const WalkParams& p, long long n_rays, const float* org, const float* dir, float hubble,
                             int n_v, float v_lo, float dv, float* out_column, float* out_tmean, float* out_tau,
                             cudaStream_t stream);
@@ -364,6 +366,39 @@ extern "C" thor_status thor_raytrace(thor_ctx* ctx, long long n_rays, const floa
     CU(cudaSetDevice(ctx->device));
     CU(thor::launch_raytrace(p, n_rays, org_xyz, dir_xyz, (float)hubble_kms_per_cell, out_tau ? n_v : 0, (float)v_lo,
                              out_tau ? (float)((v_hi - v_lo) / n_v) : 0.f, out_column, out_tmean, out_tau, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return THOR_OK;
+}
+
+extern "C" thor_status thor_volume_render(thor_ctx* ctx, long long n_rays, const float* org_xyz, const float* dir_xyz,
+                                          int n_peaks, const float* peaks, double n_ref, float* out_rgba) {
+    if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_volume_render: ctx is NULL");
+    if (n_rays <= 0 || !org_xyz || !dir_xyz || !out_rgba) return fail(ctx, THOR_ERR_ARG, "thor_volume_render: no rays or no output");
+    if (!peaks || n_peaks < 1 || n_peaks > THOR_MAX_TF_PEAKS) return fail(ctx, THOR_ERR_ARG, "thor_volume_render: n_peaks out of range");
+    if (!(n_ref >= 0.0) || !std::isfinite(n_ref)) return fail(ctx, THOR_ERR_ARG, "thor_volume_render: bad n_ref");
+    static_assert(THOR_MAX_TF_PEAKS == thor::MAX_TF_PEAKS, "peak limit");
+    thor::TransferFn tf{};
+    tf.n_peaks = n_peaks;
+    tf.weight_by_density = n_ref > 0.0 ? 1 : 0;
+    const double l2_10 = 3.321928094887362;            // log2(10): log10 T = log2 T / log2 10
+    for (int q = 0; q < n_peaks; ++q) {
+        const float* k = peaks + 6 * q;
+        for (int j = 0; j < 6; ++j)
+            if (!std::isfinite(k[j])) return fail(ctx, THOR_ERR_ARG, "thor_volume_render: non-finite peak");
+        if (!(k[1] > 0.f) || k[5] < 0.f) return fail(ctx, THOR_ERR_ARG, "thor_volume_render: width must be > 0 and A >= 0");
+        const double s2 = (double)k[1] * l2_10;        // width in log2 T
+        tf.centre[q] = (float)((double)k[0] * l2_10);
+        tf.neg_inv_2s2[q] = (float)(-1.4426950408889634 / (2.0 * s2 * s2));
+        tf.amp[q] = (float)(n_ref > 0.0 ? (double)k[5] / n_ref : (double)k[5]);
+        tf.r[q] = k[2]; tf.g[q] = k[3]; tf.b[q] = k[4];
+    }
+    thor::WalkParams p{};
+    p.g = ctx->g;
+    p.nHI = ctx->f[0]; p.T = ctx->f[1]; p.vx = ctx->f[2]; p.vy = ctx->f[3]; p.vz = ctx->f[4]; p.kdust = ctx->f[5];
+    p.packed = ctx->d_packed; p.has_dust = ctx->has_dust ? 1 : 0;
+    p.cell_cm = (float)ctx->cell_cm;
+    CU(cudaSetDevice(ctx->device));
+    CU(thor::launch_volume_render(p, tf, n_rays, org_xyz, dir_xyz, out_rgba, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return THOR_OK;
 }

@@ -31,6 +31,18 @@ struct RawRecord { float V; uint32_t nscat; int32_t status; float kx, ky, kz; };
 
 constexpr double CUBE_FIXED_SCALE = 4294967296.0;   // peel weights are summed as round(w 2^32) in uint64
 
+constexpr int MAX_TF_PEAKS = 8;                    // THOR_MAX_TF_PEAKS
+
+// Transfer function of the volume renderer, prepared on the host in log2 units.
+struct TransferFn {
+    int n_peaks;
+    int weight_by_density;           // w = n_HI (1 / n_ref folded into amp) or w = 1
+    float centre[MAX_TF_PEAKS];      // log2 T of the peak
+    float neg_inv_2s2[MAX_TF_PEAKS]; // -log2(e) / (2 s^2), s in log2 T
+    float amp[MAX_TF_PEAKS];         // A_p (/ n_ref)
+    float r[MAX_TF_PEAKS], g[MAX_TF_PEAKS], b[MAX_TF_PEAKS];
+};
+
 struct WalkParams {
     GridDims g;
     const float* __restrict__ nHI;

@@ -345,6 +345,63 @@ cudaError_t launch_raytrace(const WalkParams& p, long long n_rays, const float* 
     return cudaGetLastError();
 }
 
+// Volume rendering (PAPER.md 3.5.3, Eq. 12) on the same march: front-to-back compositing with the exact integral of
+// each piecewise-constant segment, C += Tr c (1 - e^{-mu l}), Tr *= e^{-mu l}.  The transfer function (Gaussian peaks
+// in log10 T) arrives by value: per peak {centre in log2 T, -log2(e) / (2 s^2) in log2 units, R, G, B, A / n_ref}.
+__global__ void volume_render_kernel(const __grid_constant__ WalkParams p, const __grid_constant__ TransferFn tf,
+                                     long long n_rays, const float* __restrict__ org, const float* __restrict__ dir,
+                                     float4* __restrict__ out_rgba) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_rays) return;
+    Ray r;
+    dda_locate(r, p.g, org[3 * i], org[3 * i + 1], org[3 * i + 2]);
+    ray_set_direction(r, dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]);
+    float cr = 0.f, cg = 0.f, cb = 0.f, tr = 1.f;
+    for (;;) {
+        float len;
+        const int ex = dda_next_face(r, p.g, len);
+        if (!(len < CUDART_INF_F)) break;
+        const Cell c = load_cell_raw(p, dda_linear(r, p.g));
+        const float w = tf.weight_by_density ? c.nsig : 1.f, T = c.a;
+        if (w > 0.f && T > 0.f) {
+            const float lt = __log2f(T);
+            float mu = 0.f, er = 0.f, eg = 0.f, eb = 0.f;
+#pragma unroll
+            for (int q = 0; q < MAX_TF_PEAKS; ++q)
+                if (q < tf.n_peaks) {
+                    const float z = lt - tf.centre[q];
+                    const float ag = tf.amp[q] * exp2f(tf.neg_inv_2s2[q] * z * z);
+                    mu += ag;
+                    er = fmaf(ag, tf.r[q], er);
+                    eg = fmaf(ag, tf.g[q], eg);
+                    eb = fmaf(ag, tf.b[q], eb);
+                }
+            mu *= w;
+            if (mu > 0.f) {
+                const float att = exp2f(-1.4426950408889634f * mu * len);
+                const float f = tr * (1.f - att) * w / mu;      // Tr (1 - e^{-mu l}) / mu, times w for the emission
+                cr = fmaf(f, er, cr);
+                cg = fmaf(f, eg, cg);
+                cb = fmaf(f, eb, cb);
+                tr *= att;
+            }
+        }
+        const float ke = ex == 0 ? r.kx : ex == 1 ? r.ky : r.kz;
+        const int cn = (ex == 0 ? r.cx : ex == 1 ? r.cy : r.cz) + (ke > 0.f ? 1 : -1);
+        const int nn = ex == 0 ? p.g.nx : ex == 1 ? p.g.ny : p.g.nz;
+        if (cn < 0 || cn >= nn) break;
+        dda_cross(r, p.g, ex, len);
+    }
+    out_rgba[i] = make_float4(cr, cg, cb, 1.f - tr);
+}
+
+cudaError_t launch_volume_render(const WalkParams& p, const TransferFn& tf, long long n_rays, const float* org,
+                                 const float* dir, float* out_rgba, cudaStream_t stream) {
+    volume_render_kernel<<<(unsigned)((n_rays + 127) / 128), 128, 0, stream>>>(p, tf, n_rays, org, dir,
+                                                                              reinterpret_cast<float4*>(out_rgba));
+    return cudaGetLastError();
+}
+
 // Launch configuration: one persistent grid, blocks = SMs x resident blocks per SM.  The kernel is specialised at
 // compile time on (Hubble drift, peel-off) so that the common static, no-peel walk carries neither, and on the
 // register budget: 3 CTAs of 256 threads per SM (<= 80 registers) when the grid fits the 126 MB L2 and the walk is

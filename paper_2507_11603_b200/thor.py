@@ -19,7 +19,7 @@ COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "
 RAW_DTYPE = np.dtype([("V", "<f4"), ("nscat", "<u4"), ("status", "<i4"), ("kx", "<f4"), ("ky", "<f4"), ("kz", "<f4")])
 
 EXPORTS = ["thor_grid_create", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run",
-           "thor_last_run_ms", "thor_last_run_feed_ms", "thor_last_run_max_nscat", "thor_raytrace", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_dda_trace",
+           "thor_last_run_ms", "thor_last_run_feed_ms", "thor_last_run_max_nscat", "thor_raytrace", "thor_volume_render", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_dda_trace",
            "thor_unit_voigt", "thor_unit_scatter"]
 
 
@@ -70,6 +70,7 @@ def lib():
         L.thor_last_run_feed_ms.argtypes = [P, C.POINTER(f)]
         L.thor_last_run_max_nscat.argtypes = [P, C.POINTER(C.c_ulonglong)]
         L.thor_raytrace.argtypes = [P, i64, P, P, d, i32, d, d, P, P, P]
+        L.thor_volume_render.argtypes = [P, i64, P, P, i32, P, d, P]
         L.thor_tally_get.argtypes = [P, i32, P, C.c_size_t, C.POINTER(C.c_size_t)]
         L.thor_last_error.argtypes = [P]
         L.thor_last_error.restype = C.c_char_p
@@ -205,6 +206,19 @@ class Context:
         if tau is not None:
             out["tau"] = tau.cpu().numpy()
         return out
+
+    def volume_render(self, origins, dirs, peaks, n_ref=0.0):
+        """Volume rendering along rays (thor_volume_render, Eq. 12).  Returns float32[n][4] = (C_R, C_G, C_B, opacity)."""
+        import torch
+        org = torch.from_numpy(np.ascontiguousarray(origins, np.float32)).cuda()
+        dr = torch.from_numpy(np.ascontiguousarray(dirs, np.float32)).cuda()
+        pk = np.ascontiguousarray(peaks, np.float32).reshape(-1, 6)
+        n = org.shape[0]
+        out = torch.empty((n, 4), dtype=torch.float32, device="cuda")
+        _check(lib().thor_volume_render(self._ctx, n, C.c_void_p(org.data_ptr()), C.c_void_p(dr.data_ptr()),
+                                        pk.shape[0], pk.ctypes.data_as(C.c_void_p), float(n_ref),
+                                        C.c_void_p(out.data_ptr())), self._ctx)
+        return out.cpu().numpy()
 
     def last_run_max_nscat(self):
         n = C.c_ulonglong()

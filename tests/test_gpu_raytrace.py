@@ -48,3 +48,54 @@ def test_projection_and_absorption_parity(thor, oracle, pack):
     k = gx.size
     assert np.allclose(g["column"][-k:], o["column"][-k:], rtol=5e-6)
     assert np.allclose(g["tau"][-k:], o["tau"][-k:], rtol=2e-4, atol=1e-7)
+
+
+TF_PEAKS = np.array([[4.3, 0.15, 0.1, 0.3, 1.0, 0.8],     # (log10 T centre, width [dex], R, G, B, A): PAPER.md:510
+                     [5.0, 0.20, 1.0, 0.6, 0.1, 0.5],
+                     [5.5, 0.10, 1.0, 0.1, 0.1, 1.2]])
+
+
+@pytest.mark.parametrize("pack", [False, True])
+@pytest.mark.parametrize("n_ref", [0.0, 3e-9])
+def test_volume_render_parity(thor, oracle, pack, n_ref):
+    """Eq. 12 (PAPER.md 3.5.3) through the 48^3 cosmic web: random rays plus an image raster along +z."""
+    w = W.cosmic_web(n=48, n_src=16, n_photons=1, mean_n=1e-9, map_pix=8)
+    n = 48
+    org, dirs = W.random_rays(4000, (n, n, n), seed=6)
+    xs = (np.arange(12) + 0.5) * 4.0
+    gx, gy = np.meshgrid(xs, xs)
+    org = np.vstack([org, np.stack([gx.ravel(), gy.ravel(), np.zeros(gx.size)], 1)]).astype(np.float32)
+    dirs = np.vstack([dirs, np.tile([0.0, 0.0, 1.0], (gx.size, 1))]).astype(np.float32)
+    pk = TF_PEAKS.copy()
+    pk[:, 0] -= 1.2                                   # the web's temperatures sit around 10^3-10^4.5 K
+    pk[:, 5] *= 0.3 if n_ref == 0.0 else 0.15
+    ctx = thor.Context.from_workload(w["grid"], pack=pack)
+    try:
+        g = ctx.volume_render(org, dirs, pk, n_ref=n_ref)
+    finally:
+        ctx.close()
+    o = oracle.volume_render(w["grid"], org, dirs, pk.astype(np.float32), n_ref=n_ref)
+    assert 0.05 < np.median(o[:, 3]) and o[:, 3].min() < 0.9       # neither transparent nor saturated everywhere
+    # fp32 DDA against its fp64 twin: a ray grazing a corner may see one different cell (as in the projection test)
+    err = np.abs(g - o) / np.maximum(np.abs(o).max(axis=1, keepdims=True), 1e-3)
+    assert np.quantile(err, 0.999) < 1e-4 and err.max() < 1e-2
+    k = gx.size
+    assert np.allclose(g[-k:], o[-k:], rtol=1e-4, atol=1e-6)        # pencil beams: identical cell lists
+
+
+def test_volume_render_argument_errors(thor):
+    w = W.cosmic_web(n=16, n_src=4, n_photons=1, mean_n=1e-9, map_pix=8)
+    org, dirs = W.random_rays(8, (16, 16, 16), seed=1)
+    ctx = thor.Context.from_workload(w["grid"])
+    try:
+        bad = TF_PEAKS.copy()
+        bad[1, 1] = 0.0                                # zero width
+        with pytest.raises(thor.ThorError):
+            ctx.volume_render(org, dirs, bad)
+        with pytest.raises(thor.ThorError):
+            ctx.volume_render(org, dirs, np.tile(TF_PEAKS, (3, 1)))     # 9 peaks > THOR_MAX_TF_PEAKS
+        with pytest.raises(thor.ThorError):
+            ctx.volume_render(org, dirs, TF_PEAKS, n_ref=-1.0)
+        assert ctx.volume_render(org, dirs, TF_PEAKS).shape == (8, 4)   # context still usable
+    finally:
+        ctx.close()
