@@ -1,6 +1,6 @@
 """bench.py — throughput of the Lyα random walk (the whole hot path, DESIGN.md §Path rows a1-a14) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload shell|sphere|slab|turb|web] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload shell|sphere|slab|turb|web|gather|project|render] [--impl reference]
 
 A "step" is one thor_run over one batch of packets of the workload: BASELINE.json configs[1] (expanding dusty shell,
 128^3 grid, 1e6 packets) by default.  value = scatterings/s over the timed steps (whole job, all ranks), with
@@ -150,6 +150,124 @@ def run_reference(args, w):
     }))
 
 
+def run_operators(args):
+    """--workload project|render: one step = one 2048^2 image through the 512^3 cosmic-web fields (config 5's recipe at
+    512^3) with thor_raytrace (column density, PAPER.md 3.5.1) or thor_volume_render (Eq. 12), oblique parallel rays
+    from the z = 0 face.  The NEXT-row operators at the same measurement bar as the walk."""
+    import ctypes as C
+    import torch
+    import torch.distributed as dist
+    from paper_2507_11603_b200.csrc import build as cuda_build
+    rank, local, world = (int(os.environ.get(k, "0")) for k in ("RANK", "LOCAL_RANK", "WORLD_SIZE"))
+    world = max(world, 1)
+    if rank == 0:
+        cuda_build.build()
+    from paper_2507_11603_b200 import thor
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist.barrier()
+    L = thor.lib()
+    n, pix = 512, 2048
+    w = W.cosmic_web(n=n, n_src=16, n_photons=1, mean_n=1e-9, map_pix=8)
+    pack = bool(args.pack) if args.pack >= 0 else True
+    ctx = thor.Context.from_workload(w["grid"], pack=pack)
+    xs = (np.arange(pix) + 0.5) * (n / pix)
+    gx, gy = np.meshgrid(xs, xs)
+    org = np.stack([gx.ravel(), gy.ravel(), np.zeros(gx.size)], 1).astype(np.float32)
+    k = np.array([0.35, 0.25, 0.9]) / np.linalg.norm([0.35, 0.25, 0.9])
+    dirs = np.tile(k.astype(np.float32), (gx.size, 1))
+    # cells per ray from the slab exit point: 1 + face crossings on each axis (host arithmetic, not the kernel's)
+    o64, k64 = org.astype(np.float64), dirs[0].astype(np.float64)
+    t_exit = np.min(np.where(k64 > 0, (n - o64) / k64, np.inf), axis=1)
+    crossings = int((1 + np.abs(np.floor(np.minimum(o64 + t_exit[:, None] * k64, n - 1e-9)) - np.floor(o64)).sum(1)).sum())
+    peaks = np.array([[3.1, 0.15, 0.1, 0.3, 1.0, 0.016], [3.8, 0.2, 1.0, 0.6, 0.1, 0.01], [4.3, 0.1, 1.0, 0.1, 0.1, 0.024]],
+                     np.float32)                      # three Gaussian peaks in log10 T (PAPER.md:510)
+    render = args.workload == "render"
+    n_rays = org.shape[0]
+    h_org, h_dir = torch.from_numpy(org).pin_memory(), torch.from_numpy(dirs).pin_memory()
+    d_org, d_dir = h_org.cuda(), h_dir.cuda()
+    out = torch.empty((n_rays, 4 if render else 1), dtype=torch.float32, device="cuda")
+    h_out = torch.empty(out.shape, dtype=torch.float32).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def launch(o, d):
+        if render:
+            st = L.thor_volume_render(ctx._ctx, n_rays, C.c_void_p(o.data_ptr()), C.c_void_p(d.data_ptr()), len(peaks),
+                                      peaks.ctypes.data_as(C.c_void_p), 0.0, C.c_void_p(out.data_ptr()))
+        else:
+            st = L.thor_raytrace(ctx._ctx, n_rays, C.c_void_p(o.data_ptr()), C.c_void_p(d.data_ptr()), 0.0, 0, 0.0, 1.0,
+                                 C.c_void_p(out.data_ptr()), None, None)
+        assert st == 0, thor.lib().thor_last_error(ctx._ctx)
+
+    def timed(fn, steps):
+        ms = []
+        for _ in range(steps):
+            flush.zero_()
+            torch.cuda.synchronize()
+            if world > 1:
+                dist.barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        return ms
+
+    def e2e_step():
+        launch(h_org.cuda(non_blocking=True), h_dir.cuda(non_blocking=True))
+        h_out.copy_(out, non_blocking=True)
+
+    timed(lambda: launch(d_org, d_dir), max(args.warmup, 3))
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms = timed(lambda: launch(d_org, d_dir), args.steps)
+    clocks = sampler.stop()
+    ms_e2e = timed(e2e_step, args.steps)
+    tot = torch.tensor([sum(ms), sum(ms_e2e)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tot, op=dist.ReduceOp.MAX)
+    t, t_e2e = (float(x) * 1e-3 for x in tot)
+    if rank != 0:
+        return
+    I_C = 80.0                                         # thread-instructions per cell crossing: DDA 45, gather 10, accumulate ~25
+    peak = 148 * 4 * 32 * (clocks["sm_max_mhz"] or 1965) * 1e-3
+    val = crossings * args.steps * world / t
+    line = {"metric": "ray_cell_crossings_per_sec", "value": val, "unit": "cell crossings/s", "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": t * 1e3 / args.steps,
+            "images_per_sec": args.steps * world / t, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{args.workload}_web512_2048sq", "grid": [n, n, n], "rays": n_rays,
+                       "crossings_per_image": crossings, "direction": [float(x) for x in k],
+                       "layout": "packed 32 B/cell" if pack else "SoA fp32", "parallelism": f"one image per rank x{world}",
+                       "l2": "flushed between timed iterations (256 MB memset)"},
+            "clocks": clocks, "gpu_launches": args.steps,
+            "e2e": {"value": crossings * args.steps * world / t_e2e, "unit": "cell crossings/s",
+                    "h2d_bytes_per_step": int(h_org.numel() * 4 + h_dir.numel() * 4), "d2h_bytes_per_step": int(h_out.numel() * 4)},
+            "roofline": {"bound": "alu", "achieved": I_C * val * 1e-9, "peak": peak, "unit": "G thread-inst/s",
+                         "frac": I_C * val * 1e-9 / peak, "traffic": None,
+                         "kernel": "volume_render_kernel" if render else "raytrace_kernel",
+                         "kernel_ms_per_launch": t * 1e3 / args.steps,
+                         "peak_source": "148 SMs x 4 schedulers x 32 lanes x clocks.max.sm, derived in DESIGN.md 5",
+                         "hbm_GBs_algorithmic": (8 if render else 4) * n ** 3 / (t / args.steps) * 1e-9},
+            "cpu_baseline": None}
+    if not args.no_cpu_baseline:
+        from oracle import thor_oracle as orc          # the timed CPU baseline: the oracle on a bounded sample of the rays
+        orc.build()
+        sel = np.random.default_rng(0).choice(n_rays, 2000, replace=False)
+        t0 = time.perf_counter()
+        if render:
+            orc.volume_render(w["grid"], org[sel], dirs[sel], peaks)
+        else:
+            orc.raytrace(w["grid"], org[sel], dirs[sel])
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": crossings * (len(sel) / n_rays) / dt, "unit": "cell crossings/s", "cores": 1,
+                                "kind": "oracle", "sample": f"2000 of the {n_rays} rays, single thread, fp64, {dt:.1f} s"}
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -165,6 +283,10 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--pack", type=int, default=-1, help="THOR_GRID_PACK (1/0); default: on for the gather workload")
     args = ap.parse_args()
+    if args.workload in ("project", "render"):
+        if args.impl == "reference":
+            raise SystemExit("--impl reference times the walk workloads only")
+        return run_operators(args)
     w = make_workload(args.workload, args.n_photons)
     if args.impl == "reference":
         return run_reference(args, w)
