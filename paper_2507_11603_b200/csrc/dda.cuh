@@ -120,4 +120,69 @@ __device__ __forceinline__ int64_t dda_linear(const Ray& r, const GridDims& g) {
     return ((int64_t)r.cz * g.ny + r.cy) * (int64_t)g.nx + r.cx;
 }
 
+// The same specification for a ray whose direction never changes (ray-tracing operators): everything that depends on k
+// alone is folded into per-axis constants once, so a step is 6 flops for the face distances, one compare chain, and per
+// axis one multiply, one saturating add and one select.  Same cells, same segment lengths as dda_next_face / dda_cross:
+//   dead axis (k == 0 or frozen): face = +inf, inv = 1 -> t = (inf - f) * 1 = +inf;  frozen: k_move = 0 -> f unchanged
+//   clamp(x, 0, 1) is __saturatef(x) (NaN -> 0 as fminf(fmaxf(NaN, 0), 1) does)
+// The march ends at the first box face, periodic or not (thor_raytrace's contract), so there is no wrap.
+struct RayMarch {
+    float fx, fy, fz;          // in-cell offsets
+    float ax, ay, az;          // face coordinate 1 / 0, or +inf on a dead axis
+    float ix, iy, iz;          // 1/k, or 1 on a dead axis
+    float kx, ky, kz;          // k, or 0 on a frozen axis (offset never changes)
+    int cx, cy, cz;            // cell
+    int64_t idx;               // linear index of the cell
+};
+
+__device__ __forceinline__ void march_init(RayMarch& m, const GridDims& g, float px, float py, float pz, float kx,
+                                           float ky, float kz) {
+    dda_locate_axis(px, g.nx, m.cx, m.fx);
+    dda_locate_axis(py, g.ny, m.cy, m.fy);
+    dda_locate_axis(pz, g.nz, m.cz, m.fz);
+    const bool dx = kx == 0.0f || (g.frozen & 1u), dy = ky == 0.0f || (g.frozen & 2u), dz = kz == 0.0f || (g.frozen & 4u);
+    m.ax = dx ? CUDART_INF_F : (kx > 0.0f ? 1.0f : 0.0f);
+    m.ay = dy ? CUDART_INF_F : (ky > 0.0f ? 1.0f : 0.0f);
+    m.az = dz ? CUDART_INF_F : (kz > 0.0f ? 1.0f : 0.0f);
+    m.ix = dx ? 1.0f : __fdiv_rn(1.0f, kx);
+    m.iy = dy ? 1.0f : __fdiv_rn(1.0f, ky);
+    m.iz = dz ? 1.0f : __fdiv_rn(1.0f, kz);
+    m.kx = (g.frozen & 1u) ? 0.0f : kx;
+    m.ky = (g.frozen & 2u) ? 0.0f : ky;
+    m.kz = (g.frozen & 4u) ? 0.0f : kz;
+    m.idx = ((int64_t)m.cz * g.ny + m.cy) * (int64_t)g.nx + m.cx;
+}
+
+// Segment length through the current cell and the exit axis as two predicates (x, y; else z).
+__device__ __forceinline__ float march_next_face(const RayMarch& m, bool& ex_x, bool& ex_y) {
+    const float tx = __fmul_rn(__fsub_rn(m.ax, m.fx), m.ix);
+    const float ty = __fmul_rn(__fsub_rn(m.ay, m.fy), m.iy);
+    const float tz = __fmul_rn(__fsub_rn(m.az, m.fz), m.iz);
+    ex_x = tx <= ty && tx <= tz;
+    ex_y = !ex_x && ty <= tz;
+    return ex_x ? tx : ex_y ? ty : tz;
+}
+
+// Cross the exit face; false if the ray left the box.
+__device__ __forceinline__ bool march_cross(RayMarch& m, const GridDims& g, bool ex_x, bool ex_y, float len) {
+    const bool ex_z = !ex_x && !ex_y;
+    const float nx = __saturatef(__fadd_rn(m.fx, __fmul_rn(len, m.kx)));
+    const float ny = __saturatef(__fadd_rn(m.fy, __fmul_rn(len, m.ky)));
+    const float nz = __saturatef(__fadd_rn(m.fz, __fmul_rn(len, m.kz)));
+    const float ke = ex_x ? m.kx : ex_y ? m.ky : m.kz;         // the exit axis is never dead: its k is the ray's
+    const int s = ke > 0.0f ? 1 : -1;
+    const float fe = ke > 0.0f ? 0.0f : 1.0f;
+    m.fx = ex_x ? fe : nx;
+    m.fy = ex_y ? fe : ny;
+    m.fz = ex_z ? fe : nz;
+    m.cx += ex_x ? s : 0;
+    m.cy += ex_y ? s : 0;
+    m.cz += ex_z ? s : 0;
+    const int cn = ex_x ? m.cx : ex_y ? m.cy : m.cz;
+    const int nn = ex_x ? g.nx : ex_y ? g.ny : g.nz;
+    const int64_t stride = ex_x ? (int64_t)1 : ex_y ? (int64_t)g.nx : (int64_t)g.nx * g.ny;
+    m.idx += s > 0 ? stride : -stride;
+    return (unsigned)cn < (unsigned)nn;
+}
+
 }  // namespace thor

@@ -288,6 +288,12 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
         if (sh.spectrum[i]) atomicAdd(p.spectrum + i, (unsigned long long)sh.spectrum[i]);
 }
 
+// (n_HI, T) alone: 8 B of the cell's packed sector, or two SoA loads.
+__device__ __forceinline__ void load_nT(const WalkParams& p, int64_t i, float& n, float& T) {
+    if (p.packed) { const float2 q = __ldg(reinterpret_cast<const float2*>(p.packed + 2 * i)); n = q.x; T = q.y; }
+    else { n = __ldg(p.nHI + i); T = __ldg(p.T + i); }
+}
+
 // ---- ray-tracing operators on the same DDA + gather + Voigt (PAPER.md 3.5) ----
 // One thread per ray, marched from its origin to the first box face.  Projection (PAPER.md 3.5.1): Q = Int q w ds with
 // q = n_HI, w = 1 (column density, cm^-2) and q = T, w = n_HI (density-weighted temperature Q / Q^).  Absorption
@@ -302,23 +308,25 @@ __global__ void raytrace_kernel(const __grid_constant__ WalkParams p, long long 
     __syncthreads();
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_rays) return;
-    Ray r;
-    dda_locate(r, p.g, org[3 * i], org[3 * i + 1], org[3 * i + 2]);
-    ray_set_direction(r, dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]);
+    RayMarch r;
+    const float kx = dir[3 * i], ky = dir[3 * i + 1], kz = dir[3 * i + 2];
+    march_init(r, p.g, org[3 * i], org[3 * i + 1], org[3 * i + 2], kx, ky, kz);
     float col = 0.f, tn = 0.f, s_path = 0.f;
     float* tau = out_tau ? out_tau + i * n_v : nullptr;
     if (tau) for (int j = 0; j < n_v; ++j) tau[j] = 0.f;
     for (;;) {
-        float len;
-        const int ex = dda_next_face(r, p.g, len);
+        bool ex_x, ex_y;
+        const float len = march_next_face(r, ex_x, ex_y);
         if (!(len < CUDART_INF_F)) break;
-        Cell c = load_cell_raw(p, dda_linear(r, p.g));
+        Cell c;
+        if (tau) c = load_cell_raw(p, r.idx);
+        else load_nT(p, r.idx, c.nsig, c.a);                  // projections need 8 B of the cell only
         const float n = c.nsig, T = c.a;
         col += n * len;
         tn += n * T * len;
         if (tau) {
             derive_cell(p, c);
-            const float vgas = c.vx * r.kx + c.vy * r.ky + c.vz * r.kz + hubble * (s_path + 0.5f * len);
+            const float vgas = c.vx * kx + c.vy * ky + c.vz * kz + hubble * (s_path + 0.5f * len);
             if (c.nsig > 0.f || c.kd > 0.f)
                 for (int j = 0; j < n_v; ++j) {
                     const float V = v_lo + ((float)j + 0.5f) * dv;
@@ -327,11 +335,7 @@ __global__ void raytrace_kernel(const __grid_constant__ WalkParams p, long long 
                 }
         }
         s_path += len;
-        const float ke = ex == 0 ? r.kx : ex == 1 ? r.ky : r.kz;
-        const int cn = (ex == 0 ? r.cx : ex == 1 ? r.cy : r.cz) + (ke > 0.f ? 1 : -1);
-        const int nn = ex == 0 ? p.g.nx : ex == 1 ? p.g.ny : p.g.nz;
-        if (cn < 0 || cn >= nn) break;                        // rays end at the first box face, periodic or not
-        dda_cross(r, p.g, ex, len);
+        if (!march_cross(r, p.g, ex_x, ex_y, len)) break;     // rays end at the first box face, periodic or not
     }
     if (out_column) out_column[i] = col * p.cell_cm;
     if (out_tmean) out_tmean[i] = col > 0.f ? tn / col : 0.f;
@@ -348,37 +352,43 @@ cudaError_t launch_raytrace(const WalkParams& p, long long n_rays, const float* 
 // Volume rendering (PAPER.md 3.5.3, Eq. 12) on the same march: front-to-back compositing with the exact integral of
 // each piecewise-constant segment, C += Tr c (1 - e^{-mu l}), Tr *= e^{-mu l}.  The transfer function (Gaussian peaks
 // in log10 T) arrives by value: per peak {centre in log2 T, -log2(e) / (2 s^2) in log2 units, R, G, B, A / n_ref}.
-__global__ void volume_render_kernel(const __grid_constant__ WalkParams p, const __grid_constant__ TransferFn tf,
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__global__ void __launch_bounds__(128) volume_render_kernel(const __grid_constant__ WalkParams p, const __grid_constant__ TransferFn tf,
                                      long long n_rays, const float* __restrict__ org, const float* __restrict__ dir,
                                      float4* __restrict__ out_rgba) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_rays) return;
-    Ray r;
-    dda_locate(r, p.g, org[3 * i], org[3 * i + 1], org[3 * i + 2]);
-    ray_set_direction(r, dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]);
+    RayMarch r;
+    march_init(r, p.g, org[3 * i], org[3 * i + 1], org[3 * i + 2], dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]);
     float cr = 0.f, cg = 0.f, cb = 0.f, tr = 1.f;
     for (;;) {
-        float len;
-        const int ex = dda_next_face(r, p.g, len);
+        bool ex_x, ex_y;
+        const float len = march_next_face(r, ex_x, ex_y);
         if (!(len < CUDART_INF_F)) break;
-        const Cell c = load_cell_raw(p, dda_linear(r, p.g));
-        const float w = tf.weight_by_density ? c.nsig : 1.f, T = c.a;
+        float n, T;
+        load_nT(p, r.idx, n, T);
+        const float w = tf.weight_by_density ? n : 1.f;
         if (w > 0.f && T > 0.f) {
             const float lt = __log2f(T);
             float mu = 0.f, er = 0.f, eg = 0.f, eb = 0.f;
 #pragma unroll
-            for (int q = 0; q < MAX_TF_PEAKS; ++q)
-                if (q < tf.n_peaks) {
-                    const float z = lt - tf.centre[q];
-                    const float ag = tf.amp[q] * exp2f(tf.neg_inv_2s2[q] * z * z);
-                    mu += ag;
-                    er = fmaf(ag, tf.r[q], er);
-                    eg = fmaf(ag, tf.g[q], eg);
-                    eb = fmaf(ag, tf.b[q], eb);
-                }
+            for (int q = 0; q < MAX_TF_PEAKS; ++q) {
+                if (q >= tf.n_peaks) break;                     // uniform: n_peaks is a kernel parameter
+                const float z = lt - tf.centre[q];
+                const float ag = tf.amp[q] * ex2_approx(tf.neg_inv_2s2[q] * z * z);
+                mu += ag;
+                er = fmaf(ag, tf.r[q], er);
+                eg = fmaf(ag, tf.g[q], eg);
+                eb = fmaf(ag, tf.b[q], eb);
+            }
             mu *= w;
             if (mu > 0.f) {
-                const float att = exp2f(-1.4426950408889634f * mu * len);
+                const float att = ex2_approx(-1.4426950408889634f * mu * len);
                 const float f = tr * (1.f - att) * w / mu;      // Tr (1 - e^{-mu l}) / mu, times w for the emission
                 cr = fmaf(f, er, cr);
                 cg = fmaf(f, eg, cg);
@@ -386,11 +396,7 @@ __global__ void volume_render_kernel(const __grid_constant__ WalkParams p, const
                 tr *= att;
             }
         }
-        const float ke = ex == 0 ? r.kx : ex == 1 ? r.ky : r.kz;
-        const int cn = (ex == 0 ? r.cx : ex == 1 ? r.cy : r.cz) + (ke > 0.f ? 1 : -1);
-        const int nn = ex == 0 ? p.g.nx : ex == 1 ? p.g.ny : p.g.nz;
-        if (cn < 0 || cn >= nn) break;
-        dda_cross(r, p.g, ex, len);
+        if (!march_cross(r, p.g, ex_x, ex_y, len)) break;
     }
     out_rgba[i] = make_float4(cr, cg, cb, 1.f - tr);
 }
