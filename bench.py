@@ -247,7 +247,9 @@ def run_operators(args):
             "e2e": {"value": crossings * args.steps * world / t_e2e, "unit": "cell crossings/s",
                     "h2d_bytes_per_step": int(h_org.numel() * 4 + h_dir.numel() * 4), "d2h_bytes_per_step": int(h_out.numel() * 4)},
             "roofline": {"bound": "alu", "achieved": I_C * val * 1e-9, "peak": peak, "unit": "G thread-inst/s",
-                         "frac": I_C * val * 1e-9 / peak, "traffic": None,
+                         "frac": I_C * val * 1e-9 / peak,
+                         "traffic": {"render": 3.53e9, "project": 3.16e9}[args.workload] if pack else None,
+                         "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01_ray_operators_ncu.md",
                          "kernel": "volume_render_kernel" if render else "raytrace_kernel",
                          "kernel_ms_per_launch": t * 1e3 / args.steps,
                          "peak_source": "148 SMs x 4 schedulers x 32 lanes x clocks.max.sm, derived in DESIGN.md 5",

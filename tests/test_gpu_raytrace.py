@@ -99,3 +99,37 @@ def test_volume_render_argument_errors(thor):
         assert ctx.volume_render(org, dirs, TF_PEAKS).shape == (8, 4)   # context still usable
     finally:
         ctx.close()
+
+
+def test_marcher_degenerate_rays(thor, oracle):
+    """The constant-direction marcher on the cases its folded constants special-case: axis-aligned rays of either
+    sign (two dead axes, +0 and -0 components), rays in a coordinate plane, origins on faces, edges and corners with
+    inward and outward directions (zero-length first segments, reading A20)."""
+    w = W.cosmic_web(n=24, n_src=4, n_photons=1, mean_n=1e-9, map_pix=8)
+    n = 24.0
+    s2, s3 = 1 / np.sqrt(2), 1 / np.sqrt(3)
+    org, dirs = [], []
+    for o in ([3.5, 7.25, 11.0], [0.0, 0.0, 0.0], [n, n, n], [12.0, 0.0, 5.0], [n, 6.0, 6.0], [8.0, 8.0, 8.0]):
+        for k in ([1, 0, 0], [-1, 0, 0], [0, 1, 0], [0, -1, 0], [0, 0, 1], [0, 0, -1], [-1, -0.0, 0.0], [0.0, -0.0, 1],
+                  [s2, s2, 0], [-s2, 0, s2], [0, -s2, -s2], [s3, s3, s3], [-s3, -s3, -s3], [s3, -s3, s3]):
+            org.append(o)
+            dirs.append(k)
+    org, dirs = np.array(org, np.float32), np.array(dirs, np.float32)
+    pk = TF_PEAKS.copy()
+    pk[:, 0] -= 1.2
+    pk[:, 5] *= 0.3
+    for pack in (False, True):
+        ctx = thor.Context.from_workload(w["grid"], pack=pack)
+        try:
+            g = ctx.raytrace(org, dirs, n_v=8, v_lo=-100.0, v_hi=100.0)
+            gv = ctx.volume_render(org, dirs, pk)
+        finally:
+            ctx.close()
+        o = oracle.raytrace(w["grid"], org, dirs, n_v=8, v_lo=-100.0, v_hi=100.0)
+        ov = oracle.volume_render(w["grid"], org, dirs, pk.astype(np.float32))
+        # these rays run along cell edges or through exact lattice points only where both sides take the same ties
+        assert np.allclose(g["column"], o["column"], rtol=2e-5, atol=0)
+        assert np.allclose(g["tmean"], o["tmean"], rtol=2e-5)
+        assert np.allclose(g["tau"], o["tau"], rtol=5e-4, atol=1e-7 * o["tau"].max())
+        assert np.allclose(gv, ov, rtol=2e-4, atol=1e-6)
+        assert (o["column"] == 0).any() and (o["column"] > 0).any()      # outward rays from a corner see nothing
