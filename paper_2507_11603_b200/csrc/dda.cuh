@@ -131,7 +131,10 @@ struct RayMarch {
     float ax, ay, az;          // face coordinate 1 / 0, or +inf on a dead axis
     float ix, iy, iz;          // 1/k, or 1 on a dead axis
     float kx, ky, kz;          // k, or 0 on a frozen axis (offset never changes)
+    float ex, ey, ez;          // offset on entering the next cell along the axis: 0 (k > 0) or 1
     int cx, cy, cz;            // cell
+    int sx, sy, sz;            // sign(k) as the cell step
+    int64_t dy, dz;            // signed strides of y and z in the linear index (x: sx)
     int64_t idx;               // linear index of the cell
 };
 
@@ -150,6 +153,10 @@ __device__ __forceinline__ void march_init(RayMarch& m, const GridDims& g, float
     m.kx = (g.frozen & 1u) ? 0.0f : kx;
     m.ky = (g.frozen & 2u) ? 0.0f : ky;
     m.kz = (g.frozen & 4u) ? 0.0f : kz;
+    m.ex = kx > 0.0f ? 0.0f : 1.0f; m.ey = ky > 0.0f ? 0.0f : 1.0f; m.ez = kz > 0.0f ? 0.0f : 1.0f;
+    m.sx = kx > 0.0f ? 1 : -1; m.sy = ky > 0.0f ? 1 : -1; m.sz = kz > 0.0f ? 1 : -1;
+    m.dy = (int64_t)m.sy * g.nx;
+    m.dz = (int64_t)m.sz * g.nx * g.ny;
     m.idx = ((int64_t)m.cz * g.ny + m.cy) * (int64_t)g.nx + m.cx;
 }
 
@@ -169,20 +176,13 @@ __device__ __forceinline__ bool march_cross(RayMarch& m, const GridDims& g, bool
     const float nx = __saturatef(__fadd_rn(m.fx, __fmul_rn(len, m.kx)));
     const float ny = __saturatef(__fadd_rn(m.fy, __fmul_rn(len, m.ky)));
     const float nz = __saturatef(__fadd_rn(m.fz, __fmul_rn(len, m.kz)));
-    const float ke = ex_x ? m.kx : ex_y ? m.ky : m.kz;         // the exit axis is never dead: its k is the ray's
-    const int s = ke > 0.0f ? 1 : -1;
-    const float fe = ke > 0.0f ? 0.0f : 1.0f;
-    m.fx = ex_x ? fe : nx;
-    m.fy = ex_y ? fe : ny;
-    m.fz = ex_z ? fe : nz;
-    m.cx += ex_x ? s : 0;
-    m.cy += ex_y ? s : 0;
-    m.cz += ex_z ? s : 0;
-    const int cn = ex_x ? m.cx : ex_y ? m.cy : m.cz;
-    const int nn = ex_x ? g.nx : ex_y ? g.ny : g.nz;
-    const int64_t stride = ex_x ? (int64_t)1 : ex_y ? (int64_t)g.nx : (int64_t)g.nx * g.ny;
-    m.idx += s > 0 ? stride : -stride;
-    return (unsigned)cn < (unsigned)nn;
+    m.fx = ex_x ? m.ex : nx;                                   // the exit axis is never dead: entry offset 0 / 1 by sign(k)
+    m.fy = ex_y ? m.ey : ny;
+    m.fz = ex_z ? m.ez : nz;
+    if (ex_x) { m.cx += m.sx; m.idx += m.sx; }
+    if (ex_y) { m.cy += m.sy; m.idx += m.dy; }
+    if (ex_z) { m.cz += m.sz; m.idx += m.dz; }
+    return (unsigned)m.cx < (unsigned)g.nx && (unsigned)m.cy < (unsigned)g.ny && (unsigned)m.cz < (unsigned)g.nz;
 }
 
 }  // namespace thor
