@@ -221,6 +221,12 @@ void orc_raytrace(int nx, int ny, int nz, double cell_cm, const float* nHI, cons
     }
 }
 
+// Pins of orc_raytrace and orc_volume_render (tests/test_oracle_raytrace.py), none through this file's DDA or Voigt:
+// density x analytic chord, two-slab weighted mean, N sigma_0 H by scipy's Faddeeva function with a bulk-velocity shift,
+// Hubble-swept line against adaptive quadrature; volume rendering: c (1 - e^{-mu L}) in a uniform medium, two slabs seen
+// from either end (order of attenuation), nested adaptive quadrature of Eq. 12 on a random 6^3 grid with fields looked
+// up by floor(position).  The transfer function itself is the caller's and is restated in the test.
+//
 // Volume rendering (PAPER.md 3.5.3, Eq. 12): C = Int_0^L c(s) mu(s) exp(-Int_0^s mu dt) ds along each ray, observer at
 // the ray origin.  Transfer function as in PAPER.md:510 (Gaussian peaks in log10 T, brightness weighted by density):
 // g_p = exp(-(log10 T - c_p)^2 / (2 s_p^2)); mu = w Sum_p A_p g_p per cell length, c mu = w Sum_p A_p g_p (R,G,B)_p,
