@@ -92,6 +92,9 @@ typedef struct thor_opts {
     uint64_t max_scatter;             /* safety cap per packet (0 = none); capped packets are counted, not tallied */
     int32_t raw_output;               /* keep one thor_raw_record per packet (THOR_TALLY_RAW) */
     int32_t accumulate;               /* do not zero the tallies before this run */
+    uint64_t max_crossings;           /* cap on cell crossings per packet (capped packets are counted, not tallied);
+                                         0 = the built-in limit 2^32 - 1 (reading A26).  Required (> 0) on a
+                                         grid that is periodic on all three axes: no packet can ever leave it */
 } thor_opts;
 
 void thor_opts_default(thor_opts *o);
@@ -101,7 +104,9 @@ void thor_opts_default(thor_opts *o);
  * (u_par by rejection from Eq. 6, u_perp Gaussian, phase function, Eq. 7), until escape / dust absorption, tallying
  * into the context's spectrum / cube / counters.  One persistent kernel launch; synchronous: returns after the
  * stream has drained.  opts == NULL -> defaults.  Errors: THOR_ERR_STATE without sources; THOR_ERR_ARG for
- * inconsistent opts; THOR_ERR_OOM if tallies cannot be allocated; THOR_ERR_CUDA. */
+ * inconsistent opts, and for a grid periodic on all three axes (with at least one of extent > 1) when max_crossings
+ * is 0 — nothing could end a packet in empty gas there, and thor_run never hangs; THOR_ERR_OOM if tallies cannot be
+ * allocated; THOR_ERR_CUDA. */
 thor_status thor_run(thor_ctx *ctx, unsigned long long n_photons, unsigned long long seed, const thor_opts *opts);
 
 /* Duration of the walk kernel of the last thor_run in milliseconds, from CUDA events on the context's stream. */

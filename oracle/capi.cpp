@@ -138,7 +138,7 @@ struct orc_opts_c {
     double k_obs[3];
     int32_t peel_nx, peel_ny, peel_nv;
     double peel_v_lo, peel_v_hi, peel_width_cells, tau_peel_max;
-    uint64_t photon_id_offset, max_scatter;
+    uint64_t photon_id_offset, max_scatter, max_crossings;
 };
 
 // Outputs (any may be NULL): spectrum u64[spec_bins+2], nscat_hist u64[64], counters u64[9],
@@ -162,7 +162,7 @@ double orc_run(int nx, int ny, int nz, int px, int py, int pz, double cell_cm,
     o.peel_nx = oc->peel_nx; o.peel_ny = oc->peel_ny; o.peel_nv = oc->peel_nv;
     o.peel_v_lo = oc->peel_v_lo; o.peel_v_hi = oc->peel_v_hi; o.peel_width_cells = oc->peel_width_cells;
     o.tau_peel_max = oc->tau_peel_max;
-    o.photon_id_offset = oc->photon_id_offset; o.max_scatter = oc->max_scatter;
+    o.photon_id_offset = oc->photon_id_offset; o.max_scatter = oc->max_scatter; o.max_crossings = oc->max_crossings;
     Walker w(g, s, o);
     Result res;
     const auto t0 = std::chrono::steady_clock::now();

@@ -38,7 +38,7 @@ class _Opts(C.Structure):
         ("peel_nx", C.c_int32), ("peel_ny", C.c_int32), ("peel_nv", C.c_int32),
         ("peel_v_lo", C.c_double), ("peel_v_hi", C.c_double), ("peel_width_cells", C.c_double),
         ("tau_peel_max", C.c_double),
-        ("photon_id_offset", C.c_uint64), ("max_scatter", C.c_uint64),
+        ("photon_id_offset", C.c_uint64), ("max_scatter", C.c_uint64), ("max_crossings", C.c_uint64),
     ]
 
 
@@ -47,7 +47,7 @@ OPT_DEFAULTS = dict(
     spec_mode=0, spec_T_ref=1e4, spec_bins=0, spec_lo=0.0, spec_hi=1.0,
     hubble_kms_per_cell=0.0, hubble_eps=0.25, v_max_kms=0.0,
     peel_on=0, k_obs=(0.0, 0.0, 1.0), peel_nx=0, peel_ny=0, peel_nv=0, peel_v_lo=0.0, peel_v_hi=1.0,
-    peel_width_cells=0.0, tau_peel_max=30.0, photon_id_offset=0, max_scatter=0,
+    peel_width_cells=0.0, tau_peel_max=30.0, photon_id_offset=0, max_scatter=0, max_crossings=0,
 )
 
 RAW_DTYPE = np.dtype([("V", "<f4"), ("nscat", "<u4"), ("status", "<i4"), ("kx", "<f4"), ("ky", "<f4"), ("kz", "<f4")])

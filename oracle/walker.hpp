@@ -4,16 +4,17 @@
 // fp64, one packet at a time.  Numbered steps follow DESIGN.md §"Algorithm"; each cites the
 // passage it restates.  Readings of silent/ambiguous points are the A-numbers of DESIGN.md.
 //
-// Pins (tests/test_oracle_walk.py): Neufeld slab and Dijkstra sphere escape CDFs, E_2 unscattered fraction, thin
-// limit, dust-only escape fraction, interaction-kind probability, core-skip and Galilean invariance, Gunn-Peterson
-// depth under Hubble drift, peel-off (thin limit + pixel mapping, next-event-estimator identity, dipole weight
-// ratio), infinite segments, photon-number conservation.
+// Pins (tests/test_oracle_walk.py, tests/test_oracle_walk_pins2.py): Neufeld slab and Dijkstra sphere escape CDFs, E_2
+// unscattered fraction, thin limit, dust-only escape fraction, interaction-kind probability, core-skip and Galilean
+// invariance, Gunn-Peterson depth under Hubble drift, peel-off (thin limit + pixel mapping, next-event-estimator
+// identity, dipole weight ratio), infinite segments, photon-number conservation; local core-skipping (mode 2 == mode 1
+// with the cell's hand-computed x_crit, record for record, and spectrum invariance), source selection (every packet's V
+// and direction recomputed from its Philox draws through the luminosity CDF), peel rays under Hubble drift (exp(-tau) by
+// quadrature of scipy's Faddeeva function along the swept line), the crossing cap (reading A26).
 // PARITY UNPINNED: the scattering COUNT of a walk has no closed form in the paper or the literature quoted by it
 // (only "N_scat ∝ tau_0" at high tau_0), so the absolute number of scatterings per packet is checked
 // only for order of magnitude; and the paper's outflow-sphere, MgII and cosmological results (PAPER.md:326 right,
-// 358, Figs. 7-10) are figures without printed values.  Local core-skipping (mode 2, reading A7) is pinned only
-// through the global mode's invariance test; the sub-cell stepping criterion (A12) only through the Gunn-Peterson
-// depth.
+// 358, Figs. 7-10) are figures without printed values.
 #pragma once
 #include <cstdint>
 #include <cmath>
@@ -78,6 +79,7 @@ struct Opts {
     double tau_peel_max = 30.0;     // reading A13
     uint64_t photon_id_offset = 0;
     uint64_t max_scatter = 0;       // 0 = no cap
+    uint64_t max_crossings = 0;     // cap on cell crossings per packet; 0 = the built-in limit 2^32 - 1 (reading A26)
 };
 
 struct RawRecord { float V; uint32_t nscat; int32_t status; float kx, ky, kz; };
@@ -266,7 +268,10 @@ private:
         const double dV = (double)s_.sigma[j] * gauss;
         double V = dot3(cp.v, k) + dV;
         if (o_.peel_on) peel(ray, dot3(cp.v, kobs_) + dV, 1.0, res);
-        uint64_t nscat = 0;
+        uint64_t nscat = 0, ncross = 0;
+        // Reading A26: a packet that can neither escape nor be destroyed (periodic box, empty gas) would never end;
+        // it is finished as capped after max_crossings cell crossings (built-in limit 2^32 - 1).
+        const uint64_t cross_cap = (o_.max_crossings && o_.max_crossings < 0xffffffffull) ? o_.max_crossings : 0xffffffffull;
         int status = ST_ESCAPED;
         const double Hc = o_.hubble_kms_per_cell;
         for (;;) {
@@ -294,6 +299,7 @@ private:
                 res.counters[CT_CROSSINGS]++;
                 if (!dda_cross(ray, g_.dims, ex, len)) { status = ST_ESCAPED; done = true; break; }
                 if (o_.v_max_kms > 0 && std::fabs(V) > o_.v_max_kms) { status = ST_TERMINATED; done = true; break; }
+                if (++ncross >= cross_cap) { status = ST_CAPPED; done = true; break; }
             }
             if (done) break;
             // ---- Step 4: which interaction: dust with probability kappa_dust / kappa_total.

@@ -253,6 +253,10 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     if (o.spec_mode != 0 && o.spec_mode != 1) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_mode must be 0 or 1");
     if (o.spec_mode == 0 && !(o.spec_T_ref > 0)) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_T_ref must be > 0");
     if (!(o.hubble_eps > 0) || !(o.v_max_kms >= 0) || !std::isfinite(o.hubble_kms_per_cell)) return fail(ctx, THOR_ERR_ARG, "thor_run: bad Hubble / v_max options");
+    // reading A26: on a grid periodic on all three axes nothing ends a packet in empty gas; without a crossing cap the
+    // persistent kernel would never return (a fully frozen 1x1x1 grid has only infinite segments: reading A24 caps those)
+    if (ctx->g.periodic == 7u && ctx->g.frozen != 7u && o.max_crossings == 0)
+        return fail(ctx, THOR_ERR_ARG, "thor_run: the grid is periodic on all three axes (no packet can leave it): set opts.max_crossings");
     const thor::LyaConstants K = thor::lya_constants();
     thor::WalkParams p{};
     p.g = ctx->g;
@@ -261,6 +265,7 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     p.sig_cell = (float)(K.c_sig * ctx->cell_cm);
     p.c_a = (float)K.c_a; p.c_vth = (float)K.c_vth; p.inv_c_vth = (float)(1.0 / K.c_vth);
     p.cell_cm = (float)ctx->cell_cm;
+    p.max_crossings = (o.max_crossings && o.max_crossings < 0xffffffffull) ? (unsigned)o.max_crossings : 0xffffffffu;
     p.n_src = ctx->n_src; p.src_pos = ctx->d_src_pos; p.src_sigma = ctx->d_src_sigma; p.src_cdf = ctx->d_src_cdf;
     p.phase_core = o.phase_core; p.phase_wing = o.phase_wing; p.phase_frame = o.phase_frame;
     p.phase_split_x = (float)o.phase_split_x;

@@ -184,6 +184,9 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
                 } else if (p.v_max > 0.f && fabsf(V) > p.v_max) {
                     tally_finish(p, sh, CT_TERMINATED, V, nscat, crossings, rej_iters, rng.id(), ray.kx, ray.ky, ray.kz);
                     state = LS_IDLE;
+                } else if (crossings >= p.max_crossings) {        // reading A26: a packet nothing else would ever end
+                    tally_finish(p, sh, CT_CAPPED, V, nscat, crossings, rej_iters, rng.id(), ray.kx, ray.ky, ray.kz);
+                    state = LS_IDLE;
                 } else {
                     // a5: beyond L2 the gather is issued now and used next iteration, hiding the loop control and the
                     // other stage sections in its shadow; a cache-resident grid gathers at first use (fewer live values)

@@ -44,6 +44,7 @@ class Opts(C.Structure):
         ("tau_peel_max", C.c_double),
         ("photon_id_offset", C.c_uint64), ("max_scatter", C.c_uint64),
         ("raw_output", C.c_int32), ("accumulate", C.c_int32),
+        ("max_crossings", C.c_uint64),
     ]
 
 

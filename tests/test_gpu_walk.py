@@ -460,3 +460,49 @@ def test_full_size_configs_properties(thor, which):
         assert stats.kstest(ax[::50], lambda x: 4 / math.pi * np.arctan(np.tanh(kk * x ** 3 / 2))).statistic < 0.05   # P4
     else:
         assert full["counters"]["absorbed"] > 0.85 * n
+
+
+def test_crossing_cap_and_periodic_guard(thor, oracle):
+    """Reading A26 on the GPU: a grid periodic on all three axes is refused without a crossing cap (thor_run must never
+    hang), and with max_crossings = K every packet of an empty box ends as capped after exactly K crossings — the
+    oracle's numbers, integer for integer."""
+    N, n, K = 4, 300, 100
+    z = np.zeros((N, N, N), np.float32)
+    grid = dict(nx=N, ny=N, nz=N, periodic=(1, 1, 1), cell_cm=W.PC_CM, nHI=z, T=np.full((N, N, N), 1e4, np.float32), vx=z,
+                vy=z, vz=z, kdust=None)
+    src = dict(pos=np.array([[2.2, 1.7, 0.4]], np.float32), lum=np.ones(1, np.float32), sigma=np.zeros(1, np.float32))
+    opts = dict(spec_bins=4, spec_lo=-1.0, spec_hi=1.0)
+    with pytest.raises(thor.ThorError) as e:
+        thor.run_workload(dict(grid=grid, sources=src, opts=opts, n_photons=n, seed=8))
+    assert e.value.status == 1 and "max_crossings" in str(e.value)
+    w = dict(grid=grid, sources=src, opts=dict(opts, max_crossings=K), n_photons=n, seed=8)
+    g = thor.run_workload(w)
+    o = oracle.run(grid, src, w["opts"], n, 8)
+    assert g["counters"] == o["counters"]
+    assert g["counters"]["capped"] == n and g["counters"]["cell_crossings"] == n * K
+    assert int(g["spectrum"].sum()) == 0
+
+
+def test_peel_ray_under_hubble_drift(thor, oracle):
+    """The oracle pin of the same name (tests/test_oracle_walk_pins2.py) on the GPU: source in an empty moving cell,
+    static gas, walks capped at their first crossing, so the cube is n exp(-tau_obs) in ONE voxel with the line swept
+    through resonance along the peel ray.  fp32 midpoint sums against the oracle's fp64: 1e-4 relative."""
+    n, T, Hc, V0 = 500, 1e4, 2.0, 40.0
+    nx, nz, zs = 3, 40, 4
+    shape = (nz, nx, nx)
+    dens = np.full(shape, 0.13 / (oracle.sigma0_cm2(T) * W.PC_CM), np.float32)
+    vz = np.zeros(shape, np.float32)
+    dens[zs, 1, 1] = 0.0
+    vz[zs, 1, 1] = V0
+    zero = np.zeros(shape, np.float32)
+    grid = dict(nx=nx, ny=nx, nz=nz, periodic=(0, 0, 0), cell_cm=W.PC_CM, nHI=dens, T=np.full(shape, T, np.float32),
+                vx=zero, vy=zero, vz=vz, kdust=None)
+    src = dict(pos=np.array([[1.5, 1.5, zs + 0.5]], np.float32), lum=np.ones(1, np.float32), sigma=np.zeros(1, np.float32))
+    opts = dict(spec_mode=1, spec_bins=4, spec_lo=-100.0, spec_hi=100.0, hubble_kms_per_cell=Hc, max_crossings=1,
+                peel_on=1, k_obs=(0.0, 0.0, 1.0), peel_nx=4, peel_ny=4, peel_nv=50, peel_v_lo=-100.0, peel_v_hi=100.0,
+                peel_width_cells=3.0)
+    g = thor.run_workload(dict(grid=grid, sources=src, opts=opts, n_photons=n, seed=3))
+    o = oracle.run(grid, src, opts, n, 3)
+    assert g["counters"] == o["counters"] and g["counters"]["capped"] == n
+    assert np.count_nonzero(g["cube"]) == 1 and np.argmax(g["cube"]) == np.argmax(o["cube"])
+    assert abs(g["cube"].max() / o["cube"].max() - 1.0) < 1e-4
