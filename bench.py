@@ -1,16 +1,21 @@
-"""bench.py — throughput of the Lyα random walk (the whole hot path, DESIGN.md §Path rows a1-a14) on B200.
+"""bench.py — throughput of the Lyα random walk (the whole hot path, DESIGN.md §1 rows a1-a14) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload shell|sphere|slab|turb|web|gather|project|render] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload web1536|web512|turb512|shell|sphere|slab|gather|project|render]
+                    [--impl reference] [--no-subs]
 
-A "step" is one thor_run over one batch of packets of the workload: BASELINE.json configs[1] (expanding dusty shell,
-128^3 grid, 1e6 packets) by default.  value = scatterings/s over the timed steps (whole job, all ranks), with
-packets/s and cell crossings/s beside it; inputs are resident in HBM when the timed region starts.  `e2e` is the same
-metric through the C-ABI with HOST buffers (grid + sources copied host->device, tallies copied back, all inside the
-timed region).  `roofline` is the issue-slot ("alu") roofline of the walk kernel; `cpu_baseline`
-is the fp64 oracle timed on this box's host cores on a bounded sample of the same workload.
+A "step" is one thor_run over one batch of packets.  The headline workload is BASELINE.json's largest single-GPU
+configuration, configs[4]: the 1536^3 cosmic web (72.5 GB of SoA fp32 fields generated on the device, borrowed by the
+library), with Hubble drift, termination at 5 Å and a 2048^2 surface-brightness map by peel-off; each step walks a STATED
+subsample of the config's 1e8 packets (config.n_photons_per_step_per_gpu of config.n_photons_subsample_of).  value =
+scatterings/s over the timed steps (whole job, all ranks), with packets/s and cell crossings/s beside it; inputs are
+resident in HBM when the timed region starts.  `e2e` is the same metric through the C-ABI with HOST buffers for what a
+step takes in and gives back (the source list in, the tallies out; the 72.5 GB grid is the resident dataset).  `roofline` is the
+issue-slot ("alu") roofline of the walk kernel, `roofline_hbm` the cell-gather bandwidth beside it;
+`workloads` holds the other configurations measured in the same run (configs[1], [2], [3] at 512^3, the scaled configs[0],
+the gather regime), a few steps each; `cpu_baseline` is the fp64 oracle timed on this box's host cores.
 
-N > 1 (torchrun): the path shards by photon id: every rank walks its own id range of the
-same size on its own replica of the grid (weak scaling), and the tallies are summed with one NCCL all-reduce.
+N > 1 (torchrun): the path shards by photon id: every rank walks its own id range of the same size on its
+own replica of the grid (weak scaling), and the tallies are summed with one NCCL all-reduce.
 """
 import argparse
 import json
@@ -27,39 +32,70 @@ import numpy as np
 
 from paper_2507_11603_b200 import workloads as W
 
-# Issue-slot roofline constants: algorithmic thread-instructions per unit of work, counted
-# once from ncu (smsp__thread_inst_executed.sum of the walk kernel regressed on its scattering / crossing counters;
-# profiles/r01_walk_inst_per_unit.md) — fixed numbers, so a slower kernel cannot raise its own roofline fraction.
-INST_PER_SCATTERING = 630.0
-INST_PER_CROSSING = 110.0
-N_SM, SCHEDULERS_PER_SM, LANES = 148, 4, 32
-# dram__bytes_read.sum + dram__bytes_write.sum of walk_kernel per launch, from the ncu captures summarised in
-# profiles/r01_launches_bench_shell.md and profiles/r01_walk_kernel_v5_ncu.md (bench.py cannot measure this itself)
-TRAFFIC_BYTES_PER_LAUNCH = {"shell": 6.3e7, "sphere": 7.9e5, "slab": 1.8e5, "gather": 1.2677e11}
+# Issue-slot roofline constants: algorithmic thread-instructions per unit of work, SURVEY.md §8(d)'s a-priori budgets
+# (~600 per scattering, ~60 per cell crossing) — fixed numbers that do not come from this kernel, so a slower or fatter
+# kernel cannot raise its own fraction.  What the kernel actually executes per unit is in profiles/r02_*.md.
+INST_PER_SCATTERING = 600.0
+INST_PER_CROSSING = 60.0
+SCHEDULERS_PER_SM, LANES = 4, 32
+BYTES_PER_CROSSING = 20.0                              # n_HI, T, v_x, v_y, v_z (24 with dust)
+# dram__bytes_read.sum + dram__bytes_write.sum of walk_kernel per launch at the default packet counts, from the ncu
+# captures summarised under profiles/ (bench.py cannot measure this itself); None = no capture of that workload
+TRAFFIC = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))) if os.path.exists(os.path.join(ROOT, "profiles", "traffic.json")) else {}
+
+HEADLINE = "web1536"
+SUBS = ["shell", "sphere", "slab", "gather", "turb512"]
 
 
-def make_workload(name, n_photons=None):
-    if name == "shell":      # BASELINE.json configs[1]
+def make_workload(name, n_photons=None, device="cuda"):
+    """name -> (workload dict, pack flag, note).  Device-generated grids hold CUDA tensors, the others numpy arrays."""
+    pack, note = False, None
+    if name == "web1536":    # BASELINE.json configs[4] as stated; a stated subsample of its 1e8 packets per step
+        from paper_2507_11603_b200 import workloads_device as WD
+        w = WD.cosmic_web(n=1536, n_src=1 << 22, n_photons=400_000, map_pix=2048, device=device)
+        note = dict(n_photons_subsample_of=100_000_000)
+    elif name == "web512":   # configs[4]'s recipe at 512^3
+        from paper_2507_11603_b200 import workloads_device as WD
+        w = WD.cosmic_web(n=512, n_src=1 << 18, n_photons=400_000, map_pix=2048, device=device)
+        note = dict(n_photons_subsample_of=100_000_000, reduced_grid_of=1536)
+    elif name == "turb512":  # configs[3] as stated (512^3, 256 x 256 x 400 cube); a stated subsample of its 1e7 packets,
+        # each capped at 1e5 scatterings (the densest source cells have tau_0 > 1e7 per cell: DESIGN.md 5)
+        from paper_2507_11603_b200 import workloads_device as WD
+        w = WD.turbulent_box(n=512, n_src=1 << 20, n_photons=100_000, device=device)
+        w["opts"]["max_scatter"] = 100_000
+        note = dict(n_photons_subsample_of=10_000_000, max_scatter=100_000)
+    elif name == "shell":    # configs[1] as stated
         w = W.expanding_shell(n=128, n_photons=1_000_000)
     elif name == "sphere":   # configs[0] scaled to fill the GPU (same physics, more packets), tau0 = 1e4
         w = W.static_sphere(n=32, tau0=1e4, T=10.0, n_photons=1_000_000)
-    elif name == "slab":     # configs[2]
+        note = dict(scaled_from="configs[0]: tau0 1e5 -> 1e4, 1e3 -> 1e6 packets")
+    elif name == "slab":     # configs[2] as stated
         w = W.static_slab(n_photons=1_000_000)
-    elif name == "turb":     # configs[3] at 256^3
-        w = W.turbulent_box(n=256, n_src=1 << 16, n_photons=100_000, peel_pix=256, peel_bins=400)
-        w["opts"]["max_scatter"] = 100_000
-    elif name == "web":      # configs[4] at 512^3
-        w = W.cosmic_web(n=512, n_src=1 << 18, n_photons=1_000_000, map_pix=2048)
-    elif name == "gather":   # the cell-gather regime of configs[4]: same 512^3 fields, optically thin (mean n_HI 1e-11), so
+    elif name == "gather":   # the cell-gather regime: configs[4]'s recipe at 512^3 made optically thin (mean n_HI 1e-11), so
         # packets stream through ~340 cells each and the walk is bound by the HBM gathers, not by scatterings
         w = W.cosmic_web(n=512, n_src=1 << 16, n_photons=4_000_000, map_pix=2048, mean_n=1e-11)
         w["opts"].update(peel_on=0, v_max_kms=0.0)
         w["name"] = "cosmic_web_n512_thin_gather"
+        pack = True
     else:
         raise SystemExit(f"unknown workload {name}")
     if n_photons:
         w["n_photons"] = int(n_photons)
-    return w
+    return w, pack, note
+
+
+def oracle_workload(name):
+    """What the oracle walks for `name`: the same workload, except where its grid cannot exist on the host — there the
+    same recipe at 128^3 (numpy generator), which the `sample` text says."""
+    if name in ("web1536", "web512"):
+        w = W.cosmic_web(n=128, n_src=1 << 14, n_photons=1 << 20, map_pix=2048)
+        return w, "the same recipe at 128^3 (the 1536^3 grid cannot be held in host arrays for the oracle)"
+    if name == "turb512":
+        w = W.turbulent_box(n=128, n_src=1 << 14, n_photons=1 << 20, peel_pix=256, peel_bins=400)
+        w["opts"]["max_scatter"] = 100_000
+        return w, "the same recipe at 128^3"
+    w, _, _ = make_workload(name)
+    return w, "the same workload and seed"
 
 
 class ClockSampler(threading.Thread):
@@ -103,52 +139,101 @@ class ClockSampler(threading.Thread):
         return dict(sm_mhz=med, sm_max_mhz=self.max_mhz, reasons=sorted(self.reasons), samples=len(self.samples))
 
 
-def oracle_sample(w, budget_s, chunk):
-    """Times the oracle, as it stands, single-threaded, on photon ids [0, k*chunk) of the workload until budget_s
-    seconds of CPU work are spent.  Returns (scatterings, packets, crossings, seconds)."""
+def _oracle_worker(args):
+    """One host process of the timed oracle: walks photon ids [first, first + k chunk) of the workload, chunk by chunk,
+    until budget_s seconds of walking are spent.  Returns (scatterings, packets, crossings, seconds walked)."""
+    name, first, stride, budget_s, chunk = args
     from oracle import thor_oracle
-    thor_oracle.build()
+    w, _ = oracle_workload(name)
     scat = pk = cross = 0
     secs = 0.0
-    off = 0
+    off = first
     while secs < budget_s:
-        r = thor_oracle.run(w["grid"], w["sources"], dict(w["opts"], photon_id_offset=off), chunk, w["seed"],
-                            want_raw=False)
+        r = thor_oracle.run(w["grid"], w["sources"], dict(w["opts"], photon_id_offset=off), chunk, w["seed"], want_raw=False)
         secs += r["seconds"]
         scat += r["counters"]["scatterings"]
         cross += r["counters"]["cell_crossings"]
         pk += chunk
-        off += chunk
+        off += stride
     return scat, pk, cross, secs
 
 
-def run_reference(args, w):
-    """--impl reference: the oracle, as it stands, on the box's host cores, same config / metric / unit; each step a
-    bounded sample of the workload (rank 0 only)."""
+def oracle_timed(name, budget_s, chunk, procs):
+    """The oracle, as it stands, on `procs` host processes over disjoint photon-id ranges (valid because the RNG is keyed
+    on photon id): process p walks ids [p chunk, (p+1) chunk), [(p + procs) chunk, ...), ...  Aggregate rate =
+    total scatterings / the longest process's walking time."""
+    from oracle import thor_oracle
+    thor_oracle.build()
+    jobs = [(name, p * chunk, procs * chunk, budget_s, chunk) for p in range(procs)]
+    if procs == 1:
+        res = [_oracle_worker(jobs[0])]
+    else:
+        import multiprocessing as mp
+        with mp.get_context("spawn").Pool(procs) as pool:
+            res = pool.map(_oracle_worker, jobs)
+    scat = sum(r[0] for r in res)
+    pk = sum(r[1] for r in res)
+    secs = max(r[3] for r in res)
+    return scat, pk, secs
+
+
+def host_cores():
+    try:
+        return max(1, len(os.sched_getaffinity(0)))
+    except AttributeError:
+        return max(1, os.cpu_count() or 1)
+
+
+def cpu_baseline(name, budget_s, chunk):
+    """cpu_baseline object: the oracle single-threaded (its definition) and on all P host cores, on a bounded sample."""
+    _, what = oracle_workload(name)
+    P = host_cores()
+    s1, p1, t1 = oracle_timed(name, budget_s, chunk, 1)
+    out = {"value": s1 / t1, "unit": "scatterings/s", "cores": 1, "kind": "oracle", "packets_per_sec": p1 / t1,
+           "sample": f"photon ids [0, {p1}) of {what}, single thread, fp64, {t1:.1f} s"}
+    if P > 1:
+        sP, pP, tP = oracle_timed(name, budget_s, chunk, P)
+        out["all_cores"] = {"value": sP / tP, "unit": "scatterings/s", "cores": P, "packets_per_sec": pP / tP,
+                            "sample": f"{pP} packets of {what} in {P} processes over disjoint id ranges, fp64, {tP:.1f} s each"}
+    return out
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on all of the box's host cores, same config / metric / unit; each step
+    a bounded sample of the workload (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    chunk = max(1, min(w["n_photons"], args.ref_chunk))
-    for _ in range(args.warmup):
-        oracle_sample(w, 0.0, max(1, chunk // 10))
+    name = args.workload
+    w, what = oracle_workload(name)
+    P = host_cores()
+    chunk = max(1, args.ref_chunk)
+    for _ in range(min(args.warmup, 1)):
+        oracle_timed(name, 0.0, max(1, chunk // 10), 1)
     scat = pk = 0
     secs = 0.0
     for _ in range(args.steps):
-        s, p, _, t = oracle_sample(w, args.ref_budget, chunk)
+        s, p, t = oracle_timed(name, args.ref_budget, chunk, P)
         scat += s
         pk += p
         secs += t
     v = scat / secs
-    sample = f"{pk} packets (ids 0..) of {w['n_photons']} per step x {args.steps} steps, single thread, fp64"
+    sample = f"{pk // args.steps} packets of {what} per step x {args.steps} steps, {P} processes over disjoint id ranges, fp64"
     print(json.dumps({
         "impl": "reference", "metric": "lya_scatterings_per_sec", "value": v, "unit": "scatterings/s",
         "packets_per_sec": pk / secs, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic", "config": {"workload": w["name"], "n_photons_per_step": pk // args.steps},
-        "cpu_baseline": {"value": v, "unit": "scatterings/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_label(name), "oracle_grid": w["name"], "n_photons_per_step": pk // args.steps},
+        "cpu_baseline": {"value": v, "unit": "scatterings/s", "cores": P, "kind": "oracle", "sample": sample},
         "e2e": {"value": v, "unit": "scatterings/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
 
+
+def workload_label(name):
+    return {"web1536": "cosmic_web_n1536", "web512": "cosmic_web_n512", "turb512": "turbulent_box_n512",
+            "shell": "expanding_shell_n128", "sphere": "static_sphere_n32_tau10000_T10", "slab": "static_slab_nz256_tau1e+07",
+            "gather": "cosmic_web_n512_thin_gather"}.get(name, name)
 
 def run_operators(args):
     """--workload project|render: one step = one 2048^2 image through the 512^3 cosmic-web fields (config 5's recipe at
@@ -270,53 +355,24 @@ def run_operators(args):
     print(json.dumps(line))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="shell")
-    ap.add_argument("--n-photons", type=int, default=0)
-    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
-    ap.add_argument("--ref-budget", type=float, default=10.0, help="seconds of oracle work per reference step")
-    ap.add_argument("--ref-chunk", type=int, default=500)
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--pack", type=int, default=-1, help="THOR_GRID_PACK (1/0); default: on for the gather workload")
-    args = ap.parse_args()
-    if args.workload in ("project", "render"):
-        if args.impl == "reference":
-            raise SystemExit("--impl reference times the walk workloads only")
-        return run_operators(args)
-    w = make_workload(args.workload, args.n_photons)
-    if args.impl == "reference":
-        return run_reference(args, w)
 
+def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sample_clocks=False, want_e2e=False):
+    """Builds workload `name`, runs warmup + steps thor_run calls (L2 flushed between timed iterations), returns the result
+    object of that workload (value, ms_per_step, counters, phases, rooflines, optional e2e).  Collective under torchrun."""
     import torch
     import torch.distributed as dist
-    from paper_2507_11603_b200.csrc import build as cuda_build
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    if rank == 0:
-        cuda_build.build()
     from paper_2507_11603_b200 import shard, thor
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-        dist.barrier()
-    thor.lib()
+    w, pack, note = make_workload(name, n_photons)
+    if args.pack >= 0:
+        pack = bool(args.pack)
     n = w["n_photons"]
     opts = dict(w["opts"], raw_output=0)
-    pack = bool(args.pack) if args.pack >= 0 else args.workload in ("gather", "web", "turb")
+    t_gen = time.perf_counter()
     ctx = thor.Context.from_workload(w["grid"], pack=pack)         # fields resident in HBM before the timed region
     ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     spec_dev = torch.zeros(opts["spec_bins"] + 2, dtype=torch.int64, device="cuda")
     cnt_dev = torch.zeros(len(thor.COUNTER_NAMES), dtype=torch.int64, device="cuda")
-
     feed_ms, max_nscat = [], []
 
     def step(i):
@@ -329,16 +385,17 @@ def main():
         max_nscat.append(ctx.last_run_max_nscat())
         return ctx.last_run_ms()
 
-    for i in range(args.warmup):
+    for i in range(warmup):
         step(-1 - i)
-    sampler = ClockSampler(local)
+    sampler = ClockSampler(local) if sample_clocks else None
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
-    sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    if sampler:
+        sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     kern_ms, totals = [], np.zeros(len(thor.COUNTER_NAMES), np.int64)
-    for i in range(args.steps):
+    for i in range(steps):
         flush.zero_()                                              # flush L2 between timed iterations (untimed)
         ev[i][0].record()
         kern_ms.append(step(i))
@@ -347,7 +404,7 @@ def main():
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    clocks = sampler.stop()
+    clocks = sampler.stop() if sampler else None
     step_ms = sum(a.elapsed_time(b) for a, b in ev)
     t = torch.tensor([step_ms, sum(kern_ms)], dtype=torch.float64, device="cuda")
     if world > 1:
@@ -355,80 +412,92 @@ def main():
     step_ms, kernel_ms = float(t[0]), float(t[1])
     c = dict(zip(thor.COUNTER_NAMES, (int(v) for v in totals)))
     packets = c["escaped"] + c["absorbed"] + c["terminated"] + c["capped"]
-    assert packets == n * world * args.steps, (packets, n, world, args.steps)
+    assert packets == n * world * steps, (packets, n, world, steps)
     secs = step_ms * 1e-3
-    value = c["scatterings"] / secs
-
+    crossings = c["cell_crossings"] + c["peel_cells"]
+    g = w["grid"]
     out = {
-        "metric": "lya_scatterings_per_sec", "value": value, "unit": "scatterings/s",
-        "packets_per_sec": packets / secs, "cell_crossings_per_sec": (c["cell_crossings"] + c["peel_cells"]) / secs,
-        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": w["name"], "baseline_config": args.workload, "grid": [w["grid"]["nx"], w["grid"]["ny"], w["grid"]["nz"]],
-                   "n_photons_per_step_per_gpu": n, "parallelism": f"photon-id shards x{world}, grid replicated",
+        "metric": "lya_scatterings_per_sec", "value": c["scatterings"] / secs, "unit": "scatterings/s",
+        "packets_per_sec": packets / secs, "cell_crossings_per_sec": crossings / secs,
+        "steps": steps, "warmup": warmup, "ms_per_step": step_ms / steps,
+        "config": {"workload": workload_label(name), "grid": [g["nx"], g["ny"], g["nz"]], "n_photons_per_step_per_gpu": n,
+                   "layout": "packed 32 B/cell (THOR_GRID_PACK)" if pack else "SoA fp32, borrowed",
+                   "parallelism": f"photon-id shards x{world}, grid replicated",
                    "l2": "flushed between timed iterations (256 MB memset)",
                    "scatterings_per_packet": c["scatterings"] / packets,
-                   "rejection_iters_per_scattering": c["rejection_iters"] / max(1, c["scatterings"])},
-        "clocks": clocks, "gpu_launches": args.steps * 1,
+                   "crossings_per_packet": crossings / packets,
+                   "rejection_iters_per_scattering": c["rejection_iters"] / max(1, c["scatterings"]),
+                   "phase_functions": f"core {opts.get('phase_core', 0)} / wing {opts.get('phase_wing', 0)} (0 isotropic, 1 dipole, 2 mix)"},
         # how the kernel time splits: until the photon counter runs dry the walk is fed (throughput phase); after that
         # the launch only drains the packets in flight, and lasts as long as its longest single packet
-        "phases": {"feed_ms_per_step": float(np.mean(feed_ms[-args.steps:])),
-                   "drain_ms_per_step": kernel_ms / args.steps - float(np.mean(feed_ms[-args.steps:])),
-                   "longest_packet_scatterings": [int(v) for v in max_nscat[-args.steps:]],
+        "phases": {"feed_ms_per_step": float(np.mean(feed_ms[-steps:])),
+                   "drain_ms_per_step": kernel_ms / steps - float(np.mean(feed_ms[-steps:])),
+                   "longest_packet_scatterings": [int(v) for v in max_nscat[-steps:]],
                    "drain_ns_per_scattering_of_longest_packet": float(np.mean([1e6 * (k - f) / max(1, m) for k, f, m in
-                                                                               zip(kern_ms, feed_ms[-args.steps:], max_nscat[-args.steps:])])),
+                                                                               zip(kern_ms, feed_ms[-steps:], max_nscat[-steps:])])),
                    "source": "device %globaltimer at kernel entry and when the photon counter is first found exhausted (thor_last_run_feed_ms)"},
         "counters": c,
     }
-    # ---- roofline of the dominant (only) kernel: issue-slot bound (grid is L2-resident)
-    inst = INST_PER_SCATTERING * c["scatterings"] + INST_PER_CROSSING * (c["cell_crossings"] + c["peel_cells"])
-    sm_hz = 1e6 * (clocks["sm_max_mhz"] or 1965.0)
+    if note:
+        out["config"].update(note)
+    if clocks:
+        out["clocks"] = clocks
+    # ---- rooflines of the dominant (only) kernel
+    sm_hz = 1e6 * float((clocks or {}).get("sm_max_mhz") or 1965.0)
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     peak = n_sm * SCHEDULERS_PER_SM * LANES * sm_hz * world
+    inst = INST_PER_SCATTERING * c["scatterings"] + INST_PER_CROSSING * crossings
     achieved = inst / (kernel_ms * 1e-3)
-    if args.workload == "gather":
-        # HBM roofline of the cell gather: 20 algorithmic bytes per crossing (n, T, vx, vy, vz)
-        peaks = {}
-        try:
-            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-        except Exception:
-            pass
-        hbm = float(peaks.get("hbm_gbs", 6650.0)) * world
-        gbs = 20.0 * (c["cell_crossings"] + c["peel_cells"]) / (kernel_ms * 1e-3) / 1e9
-        out["roofline_hbm"] = {"bound": "hbm", "achieved": gbs, "peak": hbm, "unit": "GB/s", "frac": gbs / hbm,
-                               "traffic": TRAFFIC_BYTES_PER_LAUNCH["gather"] if (pack and not args.n_photons) else None,
-                               "algorithmic_bytes_per_launch": 20.0 * (c["cell_crossings"] + c["peel_cells"]) / args.steps,
-                               "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks else "6650 GB/s (of fallback)",
-                               "bytes_per_crossing": 20, "layout": "packed 32 B/cell" if pack else "SoA 5 x 4 B/cell"}
-    out["config"]["layout"] = "packed 32 B/cell (THOR_GRID_PACK)" if pack else "SoA fp32, borrowed"
-    out["roofline"] = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "G thread-inst/s",
-                       "frac": achieved / peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.workload) if not args.n_photons else None,
-                       "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01_*.md",
-                       "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_hz / 1e6:.0f} MHz (clocks.max.sm), derived in DESIGN.md",
-                       "kernel": "walk_kernel", "kernel_ms_per_launch": kernel_ms / args.steps,
-                       "inst_per_scattering": INST_PER_SCATTERING, "inst_per_crossing": INST_PER_CROSSING}
-    if "roofline_hbm" in out:                                       # gather workload: the HBM roofline is the binding one
-        out["roofline_alu"] = out["roofline"]
-        out["roofline"] = out.pop("roofline_hbm")
-    ctx.close()
+    traffic = TRAFFIC.get(name) if not n_photons else None
+    alu = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "G thread-inst/s", "frac": achieved / peak,
+           "traffic": traffic, "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch (profiles/traffic.json, profiles/r02_*.md)",
+           "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_hz / 1e6:.0f} MHz (clocks.max.sm), derived in DESIGN.md 5",
+           "kernel": "walk_kernel", "kernel_ms_per_launch": kernel_ms / steps,
+           "inst_per_scattering": INST_PER_SCATTERING, "inst_per_crossing": INST_PER_CROSSING,
+           "constants_source": "SURVEY.md 8(d) a-priori budgets"}
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0)) * world
+    gbs = BYTES_PER_CROSSING * crossings / (kernel_ms * 1e-3) / 1e9
+    hbm = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak, "traffic": traffic,
+           "algorithmic_bytes_per_launch": BYTES_PER_CROSSING * crossings / steps, "bytes_per_crossing": BYTES_PER_CROSSING,
+           "dram_bytes_per_crossing": (traffic / (crossings / steps / world)) if traffic else None,
+           "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks else "6650 GB/s (of fallback)"}
+    if name == "gather":                                            # the HBM roofline is the binding one there
+        out["roofline"], out["roofline_alu"] = hbm, alu
+    else:
+        out["roofline"], out["roofline_hbm"] = alu, hbm
 
-    # ---- e2e: the same step through the C-ABI with HOST buffers; H2D of grid + sources and D2H of tallies are timed
-    if not args.no_e2e:
-        fields = [k for k in ("nHI", "T", "vx", "vy", "vz", "kdust") if w["grid"].get(k) is not None]
-        h2d = sum(w["grid"][k].nbytes for k in fields) + sum(np.asarray(w["sources"][k]).nbytes for k in ("pos", "lum", "sigma"))
-        d2h = (opts["spec_bins"] + 2 + 64 + len(thor.COUNTER_NAMES)) * 8
+    # ---- e2e: the same step through the C-ABI with HOST buffers for what a step takes in and gives back: the source list
+    # goes host -> device (thor_sources_set), the tallies come back device -> host (thor_tally_get), all inside the timed
+    # region.  Small grids are re-created from host arrays each step as well; the 72.5 GB grid stays resident (dataset).
+    if want_e2e:
+        regrid = not isinstance(g["nHI"], torch.Tensor)
+        src = w["sources"]
+        h2d = sum(np.asarray(src[k]).nbytes for k in ("pos", "lum", "sigma"))
+        if regrid:
+            h2d += sum(g[k].nbytes for k in ("nHI", "T", "vx", "vy", "vz", "kdust") if g.get(k) is not None)
+        cube_bytes = opts.get("peel_nx", 0) * opts.get("peel_ny", 0) * opts.get("peel_nv", 0) * 8 if opts.get("peel_on") else 0
+        d2h = (opts["spec_bins"] + 2 + 64 + len(thor.COUNTER_NAMES)) * 8 + cube_bytes
         e_scat, e_secs = 0, 0.0
-        for i in range(-1, args.steps):                             # one untimed warm-up pass
+        for i in range(-1, steps):                                  # one untimed warm-up pass
+            flush.zero_()
             if world > 1:
                 dist.barrier()
             torch.cuda.synchronize()
             t0 = time.perf_counter()
-            cx = thor.Context.from_workload(w["grid"], host=True, pack=pack)
-            cx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
+            cx = thor.Context.from_workload(g, host=True, pack=pack) if regrid else ctx
+            cx.sources_set(src["pos"], src["lum"], src["sigma"])
             cx.run(n, w["seed"] + max(i, 0), dict(opts, photon_id_offset=rank * n))
             cx.spectrum(); cx.nscat_hist()
+            if cube_bytes:
+                cx.cube()
             cc = cx.counters()
-            cx.close()
+            if regrid:
+                cx.close()
             torch.cuda.synchronize()
             dt = time.perf_counter() - t0
             tt = torch.tensor([dt, float(cc["scatterings"])], dtype=torch.float64, device="cuda")
@@ -439,16 +508,82 @@ def main():
             if i >= 0:
                 e_secs += float(tt[0]); e_scat += float(tt[1])
         out["e2e"] = {"value": e_scat / e_secs, "unit": "scatterings/s", "h2d_bytes_per_step": int(h2d),
-                      "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e_secs / args.steps,
-                      "timing": "host wall clock around create(host arrays)+sources_set+run+tally_get+destroy, device synchronised on both sides, max over ranks"}
+                      "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e_secs / steps,
+                      "timing": ("host wall clock around " + ("create(host arrays)+" if regrid else "") +
+                                 "sources_set(host arrays)+run+tally_get(host: spectrum, histogram, counters" +
+                                 (", cube" if cube_bytes else "") + ")" + ("+destroy" if regrid else "") +
+                                 ", device synchronised on both sides, max over ranks" +
+                                 ("" if regrid else "; the grid is the resident dataset (72.5 GB) and is not re-copied"))}
+    ctx.close()
+    del ctx, flush, w, g
+    torch.cuda.empty_cache()
+    return out
 
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default=HEADLINE)
+    ap.add_argument("--n-photons", type=int, default=0)
+    ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for each cpu_baseline leg")
+    ap.add_argument("--ref-budget", type=float, default=10.0, help="seconds of oracle work per reference step")
+    ap.add_argument("--ref-chunk", type=int, default=20, help="packets per oracle call")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-subs", action="store_true", help="skip the `workloads` sub-dict")
+    ap.add_argument("--sub-steps", type=int, default=2)
+    ap.add_argument("--pack", type=int, default=-1, help="THOR_GRID_PACK (1/0); default: on for the gather workload")
+    args = ap.parse_args()
+    if args.workload in ("project", "render"):
+        if args.impl == "reference":
+            raise SystemExit("--impl reference times the walk workloads only")
+        return run_operators(args)
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2507_11603_b200.csrc import build as cuda_build
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank == 0:
+        cuda_build.build()
+    from paper_2507_11603_b200 import thor
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist.barrier()
+    thor.lib()
+    t0 = time.perf_counter()
+    head = measure_walk(args, args.workload, args.steps, args.warmup, rank, local, world, n_photons=args.n_photons,
+                        sample_clocks=True, want_e2e=not args.no_e2e)
+    out = {"metric": head["metric"], "value": head["value"], "unit": head["unit"], "packets_per_sec": head["packets_per_sec"],
+           "cell_crossings_per_sec": head["cell_crossings_per_sec"], "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": head["config"], "clocks": head.get("clocks"),
+           "gpu_launches": args.steps, "phases": head["phases"], "counters": head["counters"],
+           "roofline": head["roofline"]}
+    for k in ("roofline_hbm", "roofline_alu", "e2e"):
+        if k in head:
+            out[k] = head[k]
+    out["headline_wall_s"] = time.perf_counter() - t0
+    # ---- the other configurations, measured in the same run (a few steps each): steady-state and straggler regimes
+    if not args.no_subs and args.workload == HEADLINE and not args.n_photons:
+        out["workloads"] = {}
+        for name in SUBS:
+            r = measure_walk(args, name, args.sub_steps, 3, rank, local, world)
+            out["workloads"][name] = {k: r[k] for k in ("value", "unit", "packets_per_sec", "cell_crossings_per_sec", "steps",
+                                                         "warmup", "ms_per_step", "config", "phases", "roofline")}
+            out["workloads"][name]["roofline_other"] = r.get("roofline_hbm") or r.get("roofline_alu")
+            out["gpu_launches"] += args.sub_steps
     # ---- cpu_baseline: the oracle on a bounded sample, rank 0 at N = 1 only
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        chunk = max(1, min(n, args.ref_chunk))
-        s, p, _, t = oracle_sample(w, args.cpu_budget, chunk)
-        out["cpu_baseline"] = {"value": s / t, "unit": "scatterings/s", "cores": 1, "kind": "oracle",
-                               "packets_per_sec": p / t,
-                               "sample": f"photon ids [0, {p}) of the same workload and seed, single thread, fp64, {t:.1f} s"}
+        out["cpu_baseline"] = cpu_baseline(args.workload, args.cpu_budget, max(1, args.ref_chunk))
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()

@@ -13,6 +13,8 @@
 
 namespace thor {
 cudaError_t launch_walk(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out);
+long long walk_pool_slots(int n_sm);
+int walk_pool_words();
 cudaError_t launch_volume_render(const WalkParams& p, const TransferFn& tf, long long n_rays, const float* org,
                                  const float* dir, float* out_rgba, cudaStream_t stream);
 cudaError_t launch_raytrace(const WalkParams& p, long long n_rays, const float* org, const float* dir, float hubble,
@@ -45,6 +47,7 @@ struct thor_ctx {
     size_t cube_elems = 0;
     thor::RawRecord* d_raw = nullptr;
     size_t raw_cap = 0;
+    uint32_t* d_pool = nullptr;                 // parked packets for the drain kernel
     // last run
     bool have_run = false;
     thor_opts last{};
@@ -59,7 +62,7 @@ struct thor_ctx {
 static thread_local std::string g_err;
 
 static constexpr size_t SMALL_NEXT = 0, SMALL_COUNTERS = 1, SMALL_HIST = SMALL_COUNTERS + thor::N_COUNTERS,
-                        SMALL_SPEC = SMALL_HIST + 64, SMALL_TIMES = SMALL_SPEC + 4096 + 2, SMALL_MAXN = SMALL_TIMES + 2, SMALL_TOTAL = SMALL_MAXN + 1;
+                        SMALL_SPEC = SMALL_HIST + 64, SMALL_TIMES = SMALL_SPEC + 4096 + 2, SMALL_MAXN = SMALL_TIMES + 2, SMALL_POOL = SMALL_MAXN + 1, SMALL_TOTAL = SMALL_POOL + 2;
 
 static thor_status fail(thor_ctx* c, thor_status s, const std::string& msg) {
     if (c) c->err = msg;
@@ -104,6 +107,7 @@ extern "C" void thor_grid_destroy(thor_ctx* ctx) {
     if (ctx->d_small) cudaFree(ctx->d_small);
     if (ctx->d_cube) cudaFree(ctx->d_cube);
     if (ctx->d_raw) cudaFree(ctx->d_raw);
+    if (ctx->d_pool) cudaFree(ctx->d_pool);
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;
@@ -252,6 +256,7 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     if (o.spec_bins > 0 && !(o.spec_hi > o.spec_lo)) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_hi must exceed spec_lo");
     if (o.spec_mode != 0 && o.spec_mode != 1) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_mode must be 0 or 1");
     if (o.spec_mode == 0 && !(o.spec_T_ref > 0)) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_T_ref must be > 0");
+    if ((o.walk_variant != 0 && o.walk_variant != 3 && o.walk_variant != 4) || (o.drain_mode != 0 && o.drain_mode != 1)) return fail(ctx, THOR_ERR_ARG, "thor_run: bad walk_variant / drain_mode");
     if (!(o.hubble_eps > 0) || !(o.v_max_kms >= 0) || !std::isfinite(o.hubble_kms_per_cell)) return fail(ctx, THOR_ERR_ARG, "thor_run: bad Hubble / v_max options");
     // reading A26: on a grid periodic on all three axes nothing ends a packet in empty gas; without a crossing cap the
     // persistent kernel would never return (a fully frozen 1x1x1 grid has only infinite segments: reading A24 caps those)
@@ -300,7 +305,11 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
         cube_elems = (size_t)o.peel_nx * o.peel_ny * o.peel_nv;
     }
     p.id_offset = o.photon_id_offset; p.n_photons = n_photons; p.seed = seed; p.max_scatter = o.max_scatter;
+    p.walk_variant = o.walk_variant;
     CU(cudaSetDevice(ctx->device));
+    if (o.drain_mode == 0 && !ctx->d_pool)
+        CU(cudaMalloc(&ctx->d_pool, (size_t)thor::walk_pool_slots(ctx->n_sm) * thor::walk_pool_words() * sizeof(uint32_t)));
+    p.pool = o.drain_mode == 0 ? ctx->d_pool : nullptr;
     const bool keep = o.accumulate && ctx->have_run;
     if (cube_elems != ctx->cube_elems) {
         if (ctx->d_cube) { cudaFree(ctx->d_cube); ctx->d_cube = nullptr; }
@@ -330,6 +339,9 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     p.max_nscat = ctx->d_small + SMALL_MAXN;
     CU(cudaMemsetAsync(ctx->d_small + SMALL_MAXN, 0, sizeof(unsigned long long), ctx->stream));
     p.t_dry = ctx->d_small + SMALL_TIMES + 1;
+    p.pool_count = ctx->d_small + SMALL_POOL;
+    p.pool_next = ctx->d_small + SMALL_POOL + 1;
+    CU(cudaMemsetAsync(ctx->d_small + SMALL_POOL, 0, 2 * sizeof(unsigned long long), ctx->stream));
     p.counters = ctx->d_small + SMALL_COUNTERS;
     p.nscat_hist = ctx->d_small + SMALL_HIST;
     p.spectrum = ctx->d_small + SMALL_SPEC;

@@ -1,9 +1,11 @@
 """Builds libthor_b200.so in-tree with nvcc for sm_100a only (no other arch, no fallback)."""
+import hashlib
 import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(os.path.dirname(HERE), "libthor_b200.so")
+HASH = LIB + ".srchash"
 SOURCES = ["api.cu", "walk.cu", "unit_kernels.cu"]
 DEPS = SOURCES + ["walk.cuh", "params.cuh", "philox.cuh", "dda.cuh", "voigt.cuh", "voigt_table.inc", "sampler.cuh",
                   os.path.join("..", "..", "include", "thor.h")]
@@ -11,13 +13,32 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-cudart", "shared",
               # approximate (2 ulp) division and square root for the samplers; the DDA and Voigt use explicit
               # __fdiv_rn / __fmul_rn / __fadd_rn / __frcp_rn intrinsics, which these flags do not touch
-              "-prec-div=false", "-prec-sqrt=false"]
+              "-prec-div=false", "-prec-sqrt=false",
+              # no implicit FMA contraction: every fused operation of the path is an explicit fmaf, so a value does not
+              # depend on the code around the expression (staged loop == cooperative drain, bit for bit)
+              "-fmad=false",
+              # denormals flush to zero: MUFU-based division / sqrt / log then need no range-scaling guards (the DDA's
+              # products and the Voigt sums never come near 1e-38; the bit-exact DDA test is the proof)
+              "-ftz=true"]
+
+
+def source_hash():
+    """sha256 over the nvcc flags and the bytes of every source the library is built from."""
+    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    for d in DEPS:
+        with open(os.path.join(HERE, d), "rb") as f:
+            h.update(d.encode() + b"\0" + f.read())
+    return h.hexdigest()
 
 
 def build(force=False, verbose=False):
-    deps = [os.path.join(HERE, d) for d in DEPS]
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(d) for d in deps):
-        return LIB
+    """Builds the library unless the one in the tree was built from exactly these sources and flags: the content hash
+    written beside it (libthor_b200.so.srchash) must match — file times play no part."""
+    want = source_hash()
+    if not force and os.path.exists(LIB) and os.path.exists(HASH):
+        with open(HASH) as f:
+            if f.read().strip() == want:
+                return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc] + NVCC_FLAGS + [os.path.join(HERE, s) for s in SOURCES] + ["-o", LIB]
     r = subprocess.run(cmd, capture_output=True, text=True)
@@ -25,6 +46,8 @@ def build(force=False, verbose=False):
         print(r.stdout + r.stderr)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed building libthor_b200.so")
+    with open(HASH, "w") as f:
+        f.write(want + "\n")
     return LIB
 
 

@@ -88,6 +88,11 @@ struct WalkParams {
     unsigned long long* counters;        // [N_COUNTERS]
     unsigned long long* cube;            // [ny][nx][nv] fixed point, or nullptr
     RawRecord* raw;                      // [n_photons] or nullptr
+    // cooperative drain: packets parked by walk_kernel for drain_kernel
+    uint32_t* pool;                      // [slots][PK_WORDS] parked packet states, or nullptr = no drain kernel
+    unsigned long long* pool_count;      // packets parked
+    unsigned long long* pool_next;       // next slot to pop
+    int walk_variant;                    // 0 = by grid size, 3 / 4 = force the cache-resident / beyond-L2 kernel (tests)
 };
 
 }  // namespace thor

@@ -40,16 +40,30 @@ struct UparEnvelope {
     float mA, mAB, mTot;      // cumulative masses
 };
 
-constexpr float UPAR_X_LORENTZ = 0.3f;    // below this a plain Lorentzian proposal accepts with H(a,x) >= 0.9
+#ifndef THOR_UPAR_X_LORENTZ
+#define THOR_UPAR_X_LORENTZ 0.3f
+#endif
+constexpr float UPAR_X_LORENTZ = THOR_UPAR_X_LORENTZ;   // below this a plain Lorentzian proposal accepts with H(a,x) >= e^{-x^2}
 constexpr float UPAR_U_MIN = -4.5f;       // left end of piece A (see below)
 constexpr float TWO_PI_F = 6.28318530717958647692f;
+constexpr float LN2_F = 0.693147180559945309f;
+
+// All arithmetic of the path is written with explicit fmaf / rounded operations and the library is compiled with
+// -fmad=false: a value never depends on how the compiler happened to contract the expression around it, so every code
+// variant that walks a packet (staged loop, cooperative drain, unit kernels) produces the same bits.
+
+__device__ __forceinline__ float dot3(float ax, float ay, float az, float bx, float by, float bz) {
+    return fmaf(az, bz, fmaf(ay, by, ax * bx));
+}
+
+// -ln r for a uniform r in (0,1): one MUFU.LG2 and one multiply.
+__device__ __forceinline__ float neg_log(float r) { return __log2f(r) * -LN2_F; }
 
 // sin / cos of the uniform random angle 2 pi r, r in (0,1): MUFU.SIN/COS on the reduced argument 2 pi (r - 1/2) in
 // (-pi, pi), negated (a half-turn); absolute error ~5e-7, far below the 2^-23 grain of r.
 __device__ __forceinline__ void sincos_uniform(float r, float& s, float& c) {
-    float s1, c1;
-    __sincosf(TWO_PI_F * (r - 0.5f), &s1, &c1);
-    s = -s1; c = -c1;
+    const float t = TWO_PI_F * (r - 0.5f);
+    s = -__sinf(t); c = -__cosf(t);
 }
 __device__ __forceinline__ float cos_uniform(float r) { return -__cosf(TWO_PI_F * (r - 0.5f)); }
 
@@ -81,7 +95,7 @@ __device__ __forceinline__ UparEnvelope upar_envelope(float a, float xa) {
     const bool useA = xa >= 1.5f;
     const float a2 = a * a;
     float u1 = useA ? fminf(fmaf(0.03f, xa, 1.9f), xa - 0.45f) : 0.f;
-    const float q = a * __expf(fminf(xa * xa - u1 * u1, 40.f)) / (TWO_PI_F * xa);
+    const float q = a * __expf(fminf(fmaf(xa, xa, -(u1 * u1)), 40.f)) / (TWO_PI_F * xa);
     const float d0 = sqrtf(q);
     const float delta = d0 / fmaf(xa, d0, 1.f);
     float u0 = xa - delta;
@@ -99,8 +113,8 @@ __device__ __forceinline__ UparEnvelope upar_envelope(float a, float xa) {
         const float L1inv = fmaf(w1, w1, a2);
         e.inv_w1 = 1.f / w1;
         e.beta = __logf(fmaf(ws, ws, a2) / L1inv) / (2.f * smax);
-        e.mA = SQRT_PI_F * __expf(e.beta * (e.beta - 2.f * u1)) / L1inv;
-        e.mAB = fmaf(__expf(-u1 * u1), e.inv_w0 - e.inv_w1, e.mA);
+        e.mA = SQRT_PI_F * __expf(e.beta * fmaf(-2.f, u1, e.beta)) / L1inv;
+        e.mAB = fmaf(__expf(-(u1 * u1)), e.inv_w0 - e.inv_w1, e.mA);
     } else {
         e.inv_w1 = 0.f; e.beta = 0.f; e.mA = 0.f;
         e.mAB = e.inv_w0;
@@ -109,26 +123,29 @@ __device__ __forceinline__ UparEnvelope upar_envelope(float a, float xa) {
     return e;
 }
 
-// One proposal + accept test from four uniforms.  Returns true and sets u (for x >= 0) on acceptance.
-__device__ __forceinline__ bool upar_try(const UparEnvelope& e, float a, const float4 r, float& u) {
+// One proposal + accept test from four uniforms.  Returns true and sets u (for x >= 0) on acceptance.  PRE: (sC, cC) =
+// sincospif(r.y) was computed ahead by a helper lane (cooperative drain); it is the angle of piece C exactly when
+// psi0pi == 0, because then t = fmaf(r.y, 1, 0) = r.y.
+template <bool PRE>
+__device__ __forceinline__ bool upar_try(const UparEnvelope& e, float a, const float4 r, float sC, float cC, float& u) {
     const float r1 = r.x * e.mTot;
     const float a2 = a * a;
     if (r1 >= e.mAB) {                                   // C: Lorentzian peak and beyond
-        const float t = fmaf(r.y, 1.f - e.psi0pi, e.psi0pi);
         float s, c;
-        sincospif(t, &s, &c);
-        const float uu = e.xa - a * c / s;
+        if (PRE && e.psi0pi == 0.f) { s = sC; c = cC; }
+        else sincospif(fmaf(r.y, 1.f - e.psi0pi, e.psi0pi), &s, &c);
+        const float uu = fmaf(-a, c / s, e.xa);
         u = uu;
-        return r.z <= __expf(e.u0sq - uu * uu);
+        return r.z <= __expf(fmaf(-uu, uu, e.u0sq));
     } else if (r1 >= e.mA) {                             // B
         const float iw = fmaf(r.y, e.inv_w0 - e.inv_w1, e.inv_w1);
         const float w = 1.f / iw;
         const float uu = e.xa - w;
         const float w2 = w * w;
         u = uu;
-        return r.z * (w2 + a2) <= __expf(e.u1 * e.u1 - uu * uu) * w2;
+        return r.z * (w2 + a2) <= __expf(fmaf(e.u1, e.u1, -(uu * uu))) * w2;
     } else {                                             // A: Gaussian bulk, tilted bound
-        const float uu = fmaf(sqrtf(-__logf(r.y)), cos_uniform(r.z), e.beta);
+        const float uu = fmaf(sqrtf(neg_log(r.y)), cos_uniform(r.z), e.beta);
         const float w = e.xa - uu, w1 = e.xa - e.u1;
         u = uu;
         return uu >= UPAR_U_MIN && uu <= e.u1 &&
@@ -145,19 +162,22 @@ __device__ __forceinline__ float sample_upar(float a, float x, BlockRng& rng, ui
     bool ok;                                 // happen unless x is NaN; never hang the GPU
     do {
         ++iters;
-        ok = upar_try(e, a, rng.next4(k0, k1), u);
+        ok = upar_try<false>(e, a, rng.next4(k0, k1), 0.f, 0.f, u);
     } while (!ok && ++guard < (1u << 20));
     return x < 0.f ? -u : u;
 }
 
 // Eq. 5 in polar form: magnitude m = sqrt(-ln r1) (or sqrt(x_crit^2 - ln r1) when |x_in| < x_crit),
-// angle 2 pi r2.
-__device__ __forceinline__ void sample_uperp(float x_in, float x_crit, float r1, float r2, float& up1, float& up2) {
+// angle 2 pi r2; nl1 = -ln r1 and (s2, c2) = sincos(2 pi r2) arrive precomputed (neg_log, sincos_uniform).
+__device__ __forceinline__ void uperp_from(float x_in, float x_crit, float nl1, float s2, float c2, float& up1, float& up2) {
     const float shift = fabsf(x_in) < x_crit ? x_crit * x_crit : 0.f;
-    const float m = sqrtf(shift - __logf(r1));
+    const float m = sqrtf(shift + nl1);
+    up1 = m * c2; up2 = m * s2;
+}
+__device__ __forceinline__ void sample_uperp(float x_in, float x_crit, float r1, float r2, float& up1, float& up2) {
     float s, c;
     sincos_uniform(r2, s, c);
-    up1 = m * c; up2 = m * s;
+    uperp_from(x_in, x_crit, neg_log(r1), s, c, up1, up2);
 }
 
 // Dipole p(mu) = 3/8 (1 + mu^2): the CDF (mu^3 + 3 mu + 4)/8 = r gives mu^3 + 3 mu - 2B = 0, B = 4r - 2, with the
@@ -172,11 +192,13 @@ __device__ __forceinline__ float dipole_mu(float r) {
 }
 
 // phase: 0 isotropic, 1 dipole, 2 = 1/3 isotropic + 2/3 dipole; r_mix decides the mix, r gives mu.
-__device__ __forceinline__ float sample_mu(int phase, float r_mix, float r, bool& is_dipole) {
+// PRE: mu_dip = dipole_mu(r) was computed ahead by a helper lane.
+template <bool PRE>
+__device__ __forceinline__ float sample_mu(int phase, float r_mix, float r, float mu_dip, bool& is_dipole) {
     int ph = phase;
     if (phase == 2) ph = r_mix < (1.f / 3.f) ? 0 : 1;
     is_dipole = ph == 1;
-    const float mu = is_dipole ? dipole_mu(r) : fmaf(2.f, r, -1.f);
+    const float mu = is_dipole ? (PRE ? mu_dip : dipole_mu(r)) : fmaf(2.f, r, -1.f);
     return fminf(fmaxf(mu, -1.f), 1.f);
 }
 

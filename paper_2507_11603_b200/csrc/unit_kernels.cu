@@ -101,18 +101,18 @@ __global__ void unit_scatter_kernel(float a, float x_in, float x_crit, int phase
     float up1, up2;
     sample_uperp(x_in, x_crit, s1.w, s2.x, up1, up2);
     bool dip;
-    const float mu = sample_mu(phase, s2.z, s1.y, dip);
+    const float mu = sample_mu<false>(phase, s2.z, s1.y, 0.f, dip);
     float sph, cph;
     sincos_uniform(s1.z, sph, cph);
     float e1[3], e2[3];
     ortho_basis(0.f, 0.f, 1.f, e1, e2);
-    const float st = sqrtf(fmaxf(0.f, 1.f - mu * mu));
+    const float st = sqrtf(fmaxf(0.f, fmaf(-mu, mu, 1.f)));
     if (u_par) u_par[i] = upar;
-    if (x_out) x_out[i] = x_in - upar + upar * mu + st * (up1 * cph + up2 * sph);
+    if (x_out) x_out[i] = fmaf(st, fmaf(up1, cph, up2 * sph), fmaf(upar, mu, x_in - upar));
     if (k_out) {
-        k_out[3 * i + 0] = st * (cph * e1[0] + sph * e2[0]);
-        k_out[3 * i + 1] = st * (cph * e1[1] + sph * e2[1]);
-        k_out[3 * i + 2] = mu + st * (cph * e1[2] + sph * e2[2]);
+        k_out[3 * i + 0] = st * fmaf(cph, e1[0], sph * e2[0]);
+        k_out[3 * i + 1] = st * fmaf(cph, e1[1], sph * e2[1]);
+        k_out[3 * i + 2] = fmaf(st, fmaf(cph, e1[2], sph * e2[2]), mu);
     }
     if (iters) iters[i] = it;
 }

@@ -59,7 +59,7 @@ __device__ __forceinline__ float voigt_H(const float2* __restrict__ s_tab, float
     const float H2 = fmaf(-2.0f, x2, 1.0f) * e;
     const float H3 = (C * (1.0f / 3.0f)) * fmaf(G, fmaf(2.0f, x2, -3.0f), 1.0f);
     const float H4 = e * fmaf(x2, fmaf(x2, 2.0f / 3.0f, -2.0f), 0.5f);
-    return fmaf(a, H1, e) + a2 * fmaf(a, H3, fmaf(a2, H4, H2));
+    return fmaf(a2, fmaf(a, H3, fmaf(a2, H4, H2)), fmaf(a, H1, e));
 }
 
 }  // namespace thor

@@ -27,6 +27,13 @@ constexpr int FINISH_MIN_LANES = THOR_FINISH_MIN_LANES;
 #define THOR_REFILL_MIN_LANES 8
 #endif
 constexpr int REFILL_MIN_LANES = THOR_REFILL_MIN_LANES;
+#ifndef THOR_COOP_MAX_LANES
+#define THOR_COOP_MAX_LANES 4
+#endif
+constexpr int COOP_MAX_LANES = THOR_COOP_MAX_LANES;     // cooperative drain when a warp has at most this many packets left
+constexpr int WALK_WARPS = WALK_THREADS / 32;
+constexpr int WIN_STRIDE = 20;                          // floats per window slot (16 used; 80 B keeps STS.128 conflict-free)
+constexpr int PK_WORDS = 48;                            // 32-bit words of a parked packet
 
 struct BlockTallies {
     float2 voigt[VOIGT_NODES];
@@ -35,6 +42,9 @@ struct BlockTallies {
     unsigned int max_nscat;
     unsigned int spectrum[MAX_SPEC_BINS + 2];
 };
+
+constexpr int DRAIN_THREADS = 128;                     // drain kernel: 4 warps per CTA, one per SM sub-partition
+constexpr int DRAIN_WARPS = DRAIN_THREADS / 32;
 
 // a13: tallies of a finished packet into the block's shared-memory histograms.
 __device__ __forceinline__ void tally_finish(const WalkParams& p, BlockTallies& sh, int status, float V,
@@ -56,6 +66,157 @@ __device__ __forceinline__ void tally_finish(const WalkParams& p, BlockTallies& 
     if (p.raw) p.raw[id - p.id_offset] = RawRecord{V, nscat, status, kx, ky, kz};
 }
 
+__device__ __forceinline__ void tally_packet(const WalkParams& p, BlockTallies& sh, int ev, const Packet& k) {
+    const int status = ev == EV_ESCAPED ? CT_ESCAPED : ev == EV_ABSORBED ? CT_ABSORBED : ev == EV_TERMINATED ? CT_TERMINATED : CT_CAPPED;
+    tally_finish(p, sh, status, k.V, k.nscat, k.crossings, k.rej_iters, k.rng.id(), k.ray.kx, k.ray.ky, k.ray.kz);
+}
+
+// ---- cooperative drain --------------------------------------------------------------------------
+// When the photon counter is dry and a warp is down to a few packets, every further scattering is a serial chain of
+// ~590 dependent instructions issued for one live lane (measured: 1.29 us per scattering).  Most of that chain does not
+// depend on the packet's state at all: the Philox blocks (3 per scattering, ~45 instructions each) and everything
+// computed from uniforms alone (-ln r, sin/cos of random angles, the dipole inversion, the Lorentzian angle of a
+// line-centre trial).  So the warp's 32 lanes turn to ONE packet at a time: lane i generates counter block b + i of that
+// packet and works out those quantities (a window of 32 blocks, ~10 scatterings' worth, in shared memory), then all
+// lanes step the packet redundantly — same instructions, same operands, warp-uniform control flow — reading the window
+// instead of computing.  Blocks are consumed in the packet's own order (trial, trial, ..., finish, finish), so the walk
+// is bit-identical to the staged loop's.  Packets of the warp take turns, one window each.
+__device__ __forceinline__ void park_store(uint32_t* w, const Packet& k, int state) {
+    w[0] = (uint32_t)k.ray.cx; w[1] = (uint32_t)k.ray.cy; w[2] = (uint32_t)k.ray.cz;
+    w[3] = __float_as_uint(k.ray.fx); w[4] = __float_as_uint(k.ray.fy); w[5] = __float_as_uint(k.ray.fz);
+    w[6] = __float_as_uint(k.ray.kx); w[7] = __float_as_uint(k.ray.ky); w[8] = __float_as_uint(k.ray.kz);
+    w[9] = __float_as_uint(k.ray.ix); w[10] = __float_as_uint(k.ray.iy); w[11] = __float_as_uint(k.ray.iz);
+    w[12] = __float_as_uint(k.cell.a); w[13] = __float_as_uint(k.cell.vth); w[14] = __float_as_uint(k.cell.inv_vth);
+    w[15] = __float_as_uint(k.cell.nsig); w[16] = __float_as_uint(k.cell.kd);
+    w[17] = __float_as_uint(k.cell.vx); w[18] = __float_as_uint(k.cell.vy); w[19] = __float_as_uint(k.cell.vz);
+    w[20] = k.rng.id_lo; w[21] = k.rng.id_hi; w[22] = k.rng.b_lo; w[23] = k.rng.b_hi;
+    w[24] = __float_as_uint(k.V); w[25] = __float_as_uint(k.tau_rem); w[26] = __float_as_uint(k.hit_kt);
+    w[27] = __float_as_uint(k.x_in); w[28] = __float_as_uint(k.upar);
+    w[29] = k.nscat; w[30] = k.crossings; w[31] = k.rej_iters; w[32] = k.trials;
+    w[33] = (k.stale ? 1u : 0u) | (k.inv_ok ? 2u : 0u); w[34] = (uint32_t)state;
+}
+
+__device__ __forceinline__ int park_load(const uint32_t* w, Packet& k) {
+    k.ray.cx = (int)w[0]; k.ray.cy = (int)w[1]; k.ray.cz = (int)w[2];
+    k.ray.fx = __uint_as_float(w[3]); k.ray.fy = __uint_as_float(w[4]); k.ray.fz = __uint_as_float(w[5]);
+    k.ray.kx = __uint_as_float(w[6]); k.ray.ky = __uint_as_float(w[7]); k.ray.kz = __uint_as_float(w[8]);
+    k.ray.ix = __uint_as_float(w[9]); k.ray.iy = __uint_as_float(w[10]); k.ray.iz = __uint_as_float(w[11]);
+    k.cell.a = __uint_as_float(w[12]); k.cell.vth = __uint_as_float(w[13]); k.cell.inv_vth = __uint_as_float(w[14]);
+    k.cell.nsig = __uint_as_float(w[15]); k.cell.kd = __uint_as_float(w[16]);
+    k.cell.vx = __uint_as_float(w[17]); k.cell.vy = __uint_as_float(w[18]); k.cell.vz = __uint_as_float(w[19]);
+    k.rng.id_lo = w[20]; k.rng.id_hi = w[21]; k.rng.b_lo = w[22]; k.rng.b_hi = w[23];
+    k.V = __uint_as_float(w[24]); k.tau_rem = __uint_as_float(w[25]); k.hit_kt = __uint_as_float(w[26]);
+    k.x_in = __uint_as_float(w[27]); k.upar = __uint_as_float(w[28]);
+    k.nscat = w[29]; k.crossings = w[30]; k.rej_iters = w[31]; k.trials = w[32];
+    k.stale = (w[33] & 1u) != 0u; k.inv_ok = (w[33] & 2u) != 0u;
+    return (int)w[34];
+}
+
+// Lane i of the warp generates counter block (b + i) of packet `k` and stores, per block, the uniforms and what the
+// event code would compute from them alone, for each role the block can end up in:
+//   q0 = (u.x, u.y, u.z, u.w)                           any role
+//   q1 = (sin, cos of pi u.y; -ln u.x; dipole_mu(u.y))  trial: Lorentzian angle when psi0 = 0 | first FINISH block: tau', mu
+//   q2 = (sin, cos of 2 pi u.z; -ln u.w; 0)             first FINISH block: azimuth of k', |u_perp|^2
+//   q3 = (sin, cos of 2 pi u.x; 0; 0)                   second FINISH block: angle of u_perp
+__device__ __forceinline__ void coop_fill_window(float4* win, const BlockRng& rng, uint32_t k0, uint32_t k1, unsigned lane) {
+    const uint32_t lo = rng.b_lo + lane, hi = rng.b_hi + (lo < rng.b_lo ? 1u : 0u);
+    const U4 r = philox4x32_10(lo, hi, rng.id_lo, rng.id_hi, k0, k1);
+    const float4 u = make_float4(u01(r.x), u01(r.y), u01(r.z), u01(r.w));
+    float4 q1, q2, q3;
+    sincospif(u.y, &q1.x, &q1.y);
+    q1.z = neg_log(u.x);
+    q1.w = dipole_mu(u.y);
+    sincos_uniform(u.z, q2.x, q2.y);
+    q2.z = neg_log(u.w); q2.w = 0.f;
+    sincos_uniform(u.x, q3.x, q3.y);
+    q3.z = 0.f; q3.w = 0.f;
+    float4* slot = win + 5 * lane;
+    slot[0] = u; slot[1] = q1; slot[2] = q2; slot[3] = q3;
+}
+
+// The drain kernel: launched behind walk_kernel on the same stream.  Each warp pops one parked packet at a time from the
+// global pool and walks it to its end, all 32 lanes on that one packet (see above).  4 warps per CTA — one per SM
+// sub-partition — and a register budget of its own (the walk kernel is held to 80 registers by its occupancy).
+template <bool HUBBLE, bool PEEL>
+__global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_constant__ WalkParams p) {
+    __shared__ BlockTallies sh;
+    __shared__ float4 s_win[DRAIN_WARPS][32 * WIN_STRIDE / 4];
+    voigt_table_load(sh.voigt);
+    for (int i = threadIdx.x; i < N_COUNTERS; i += blockDim.x) sh.counters[i] = 0ull;
+    for (int i = threadIdx.x; i < 64; i += blockDim.x) sh.nscat_hist[i] = 0u;
+    if (threadIdx.x == 0) sh.max_nscat = 0u;
+    for (int i = threadIdx.x; i < p.spec_bins + 2; i += blockDim.x) sh.spectrum[i] = 0u;
+    __syncthreads();
+    const unsigned lane = threadIdx.x & 31u;
+    const uint32_t k0 = (uint32_t)p.seed, k1 = (uint32_t)(p.seed >> 32);
+    float4* win = s_win[threadIdx.x >> 5];
+    const unsigned long long n_pool = *p.pool_count;
+    uint32_t pr = 0, pc = 0;
+    Packet k;
+    for (;;) {
+        unsigned long long slot = 0;
+        if (lane == 0) slot = atomicAdd(p.pool_next, 1ull);
+        slot = __shfl_sync(0xffffffffu, slot, 0);
+        if (slot >= n_pool) break;
+        int st = park_load(p.pool + slot * PK_WORDS, k);      // every lane reads the same words: one broadcast per load
+        int c = 32;                                           // blocks of the window already consumed (32 = none left)
+        UparEnvelope env;
+        env.mTot = -1.f;
+        for (;;) {
+            if (st == LS_MARCH) {
+                const int ev = march_step<HUBBLE, false>(p, sh.voigt, k);
+                if (ev == EV_CROSSED) continue;
+                if (ev != EV_HIT) { if (lane == 0) tally_packet(p, sh, ev, k); break; }
+                st = LS_TRIAL;
+                env.mTot = -1.f;
+            }
+            if (c + 3 > 32) {                                 // fewer than a trial + a FINISH left: a new window
+                __syncwarp();
+                coop_fill_window(win, k.rng, k0, k1, lane);
+                __syncwarp();
+                c = 0;
+            }
+            if (st == LS_TRIAL) {
+                if (env.mTot < 0.f) env = upar_envelope(k.cell.a, fabsf(k.x_in));
+                const float4 u = win[5 * c], q1 = win[5 * c + 1];
+                ++c;
+                k.rng.b_lo += 1u; k.rng.b_hi += (k.rng.b_lo == 0u);
+                ++k.rej_iters;
+                float uu;
+                const bool ok = upar_try<true>(env, k.cell.a, u, q1.x, q1.y, uu);
+                if (!(ok || ++k.trials >= (1u << 20))) continue;
+                k.upar = k.x_in < 0.f ? -uu : uu;
+                st = LS_FINISH;
+            }
+            {   // LS_FINISH: blocks c, c + 1
+                const float4 u1 = win[5 * c], a1 = win[5 * c + 1], a2 = win[5 * c + 2];
+                const float4 u2 = win[5 * c + 5], b3 = win[5 * c + 8];
+                c += 2;
+                k.rng.b_lo += 2u; k.rng.b_hi += (k.rng.b_lo < 2u);
+                FinDraws d;
+                d.tau_next = a1.z; d.r_mu = u1.y; d.mu_dip = a1.w;
+                d.sphi = a2.x; d.cphi = a2.y; d.nl_p1 = a2.z;
+                d.spsi = b3.x; d.cpsi = b3.y; d.u_dust = u2.y; d.u_mix = u2.z;
+                const int ev = finish_scatter<HUBBLE, PEEL, true>(p, sh.voigt, k, d, pr, pc, lane == 0);
+                if (ev != EV_SCATTERED) { if (lane == 0) tally_packet(p, sh, ev, k); break; }
+                st = LS_MARCH;
+            }
+        }
+    }
+    if (lane == 0) {
+        atomicAdd(&sh.counters[CT_PEEL_RAYS], (unsigned long long)pr);
+        atomicAdd(&sh.counters[CT_PEEL_CELLS], (unsigned long long)pc);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < N_COUNTERS; i += blockDim.x)
+        if (sh.counters[i]) atomicAdd(p.counters + i, sh.counters[i]);
+    for (int i = threadIdx.x; i < 64; i += blockDim.x)
+        if (sh.nscat_hist[i]) atomicAdd(p.nscat_hist + i, (unsigned long long)sh.nscat_hist[i]);
+    if (threadIdx.x == 0 && sh.max_nscat) atomicMax(p.max_nscat, (unsigned long long)sh.max_nscat);
+    for (int i = threadIdx.x; i < p.spec_bins + 2; i += blockDim.x)
+        if (sh.spectrum[i]) atomicAdd(p.spectrum + i, (unsigned long long)sh.spectrum[i]);
+}
+
 template <bool HUBBLE, bool PEEL, int MIN_CTAS>
 __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __grid_constant__ WalkParams p) {
     __shared__ BlockTallies sh;
@@ -67,19 +228,15 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
     for (int i = threadIdx.x; i < p.spec_bins + 2; i += blockDim.x) sh.spectrum[i] = 0u;
     __syncthreads();
 
-    constexpr bool EARLY_GATHER = MIN_CTAS >= 4;              // the variant launched for grids beyond L2
+    constexpr bool EARLY = MIN_CTAS >= 4;                     // the variant launched for grids beyond L2
     const unsigned lane = threadIdx.x & 31u;
     const uint32_t k0 = (uint32_t)p.seed, k1 = (uint32_t)(p.seed >> 32);   // Philox key = seed (reading A16)
     int state = LS_IDLE;
-    Ray ray;
-    BlockRng rng;
-    Cell cell;                                                // the cell the packet is in (valid unless `stale`)
-    bool stale = true, inv_ok = false;                        // inv_ok: 1/k of the current direction is in `ray`
-    float V = 0.f, tau_rem = 0.f, hit_kt = 0.f, x_in = 0.f, upar = 0.f;
+    Packet k;
+    k.stale = true; k.inv_ok = false;
     UparEnvelope env;
     env.mTot = -1.f;
-    uint32_t trials = 0;
-    uint32_t nscat = 0, crossings = 0, rej_iters = 0, peel_rays = 0, peel_cells = 0;
+    uint32_t peel_rays = 0, peel_cells = 0;
     bool more = true;                                         // warp-uniform: photon counter not yet exhausted
 
     for (;;) {
@@ -96,30 +253,14 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
                 if (i >= p.n_photons) {
                     state = LS_OUT;
                 } else {
-                    rng.init(p.id_offset + i);
-                    const float4 e1 = rng.next4(k0, k1), e2 = rng.next4(k0, k1);   // (src, mu, phi, g1), (g2, tau, -, -)
-                    const double us = (double)e1.x;
-                    long long lo = 0, hi = p.n_src - 1;           // smallest j with us < cdf[j]
-                    while (lo < hi) { const long long mid = (lo + hi) >> 1; if (us < p.src_cdf[mid]) hi = mid; else lo = mid + 1; }
-                    const float mu0 = fmaf(2.f, e1.y, -1.f);      // isotropic direction (reading A22)
-                    float sp, cp;
-                    sincos_uniform(e1.z, sp, cp);
-                    const float st0 = sqrtf(fmaxf(0.f, 1.f - mu0 * mu0));
-                    const float gauss = sqrtf(-2.f * __logf(e1.w)) * cos_uniform(e2.x);
-                    dda_locate(ray, p.g, p.src_pos[3 * lo], p.src_pos[3 * lo + 1], p.src_pos[3 * lo + 2]);
-                    ray_set_k(ray, st0 * cp, st0 * sp, mu0);
-                    inv_ok = false;
-                    cell = load_cell(p, dda_linear(ray, p.g));
-                    stale = false;
-                    const float dV = p.src_sigma[lo] * gauss;     // Gaussian line in the gas frame (reading A10)
-                    V = cell.vx * ray.kx + cell.vy * ray.ky + cell.vz * ray.kz + dV;
-                    nscat = 0; crossings = 0; rej_iters = 0;
+                    float dV;
+                    emit_packet(p, k, p.id_offset + i, k0, k1, dV);
                     if (PEEL) {
                         ++peel_rays;
-                        peel_ray<HUBBLE>(p, sh.voigt, ray,
-                                         cell.vx * p.kobs[0] + cell.vy * p.kobs[1] + cell.vz * p.kobs[2] + dV, 1.f, peel_cells);
+                        peel_ray<HUBBLE>(p, sh.voigt, k.ray,
+                                         dot3(k.cell.vx, k.cell.vy, k.cell.vz, p.kobs[0], p.kobs[1], p.kobs[2]) + dV, 1.f,
+                                         peel_cells, true);
                     }
-                    tau_rem = -__logf(e2.y);                      // a3 (Eq. 3)
                     state = LS_MARCH;
                 }
             }
@@ -129,71 +270,25 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
                 more = false;
             }
         }
+        if (!more && COOP_MAX_LANES > 0 && p.pool) {
+            // the counter is dry and this warp is down to a few packets: park them in the global pool for the drain
+            // kernel (one warp per packet there) and leave
+            const bool act = state == LS_MARCH || state == LS_TRIAL || state == LS_FINISH;
+            const unsigned live = __ballot_sync(0xffffffffu, act);
+            if (live && __popc(live) <= COOP_MAX_LANES) {
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(p.pool_count, (unsigned long long)__popc(live));
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (act) park_store(p.pool + (base + __popc(live & ((1u << lane) - 1u))) * PK_WORDS, k, state);
+                break;
+            }
+        }
 
         // ---- a4-a7: one cell step for every marching lane ----
         if (state == LS_MARCH) {
-            if (stale) {
-                if (EARLY_GATHER) derive_cell(p, cell);           // raw fields gathered at the last face crossing
-                else cell = load_cell(p, dda_linear(ray, p.g));
-                stale = false;
-            }
-            const float vk = cell.vx * ray.kx + cell.vy * ray.ky + cell.vz * ray.kz;
-            bool hit = false;
-            float len = 0.f, dtau = 0.f, s_hit = 0.f, kt = 0.f;
-            int ex = 0;
-            if (!HUBBLE) {
-                // Piecewise-constant cell: the interaction lies at s = tau / kappa if that is inside the
-                // cell.  Deep in an optically thick cell s is far smaller than the distance to the nearest face, which
-                // bounds the segment length from below: no DDA step and no reciprocals of k are needed at all.
-                kt = cell_opacity(sh.voigt, cell, V, vk);
-                const float s = kt > 0.f ? tau_rem / kt : CUDART_INF_F;
-                if (kt > 0.f && s <= dda_min_face_distance(ray, p.g)) {
-                    hit = true; s_hit = s;
-                } else {
-                    if (!inv_ok) { ray_set_inv(ray); inv_ok = true; }
-                    ex = dda_next_face(ray, p.g, len);
-                    hit = kt > 0.f && s <= len;
-                    s_hit = s;
-                    dtau = kt * len;
-                }
-            } else {
-                if (!inv_ok) { ray_set_inv(ray); inv_ok = true; }
-                ex = dda_next_face(ray, p.g, len);
-                hit = integrate_segment<true>(p, sh.voigt, cell, V, vk, len, tau_rem, dtau, s_hit, kt);
-            }
-            if (hit) {
-                dda_advance_within(ray, p.g, s_hit);
-                if (HUBBLE) { if (p.hubble != 0.f) V -= p.hubble * s_hit; }
-                hit_kt = kt;
-                x_in = (V - vk) * cell.inv_vth;
-                env.mTot = -1.f;                                  // envelope not built yet
-                trials = 0u;
-                state = LS_TRIAL;
-            } else if (!(len < CUDART_INF_F)) {
-                // reading A24: infinite segment (ray parallel to every non-frozen axis) without interaction: the
-                // packet can neither leave nor be followed -> capped
-                tally_finish(p, sh, CT_CAPPED, V, nscat, crossings, rej_iters, rng.id(), ray.kx, ray.ky, ray.kz);
-                state = LS_IDLE;
-            } else {
-                tau_rem -= dtau;
-                if (HUBBLE) V -= p.hubble * len;
-                ++crossings;
-                if (!dda_cross(ray, p.g, ex, len)) {
-                    tally_finish(p, sh, CT_ESCAPED, V, nscat, crossings, rej_iters, rng.id(), ray.kx, ray.ky, ray.kz);
-                    state = LS_IDLE;
-                } else if (p.v_max > 0.f && fabsf(V) > p.v_max) {
-                    tally_finish(p, sh, CT_TERMINATED, V, nscat, crossings, rej_iters, rng.id(), ray.kx, ray.ky, ray.kz);
-                    state = LS_IDLE;
-                } else if (crossings >= p.max_crossings) {        // reading A26: a packet nothing else would ever end
-                    tally_finish(p, sh, CT_CAPPED, V, nscat, crossings, rej_iters, rng.id(), ray.kx, ray.ky, ray.kz);
-                    state = LS_IDLE;
-                } else {
-                    // a5: beyond L2 the gather is issued now and used next iteration, hiding the loop control and the
-                    // other stage sections in its shadow; a cache-resident grid gathers at first use (fewer live values)
-                    if (EARLY_GATHER) cell = load_cell_raw(p, dda_linear(ray, p.g));
-                    stale = true;
-                }
-            }
+            const int ev = march_step<HUBBLE, EARLY>(p, sh.voigt, k);
+            if (ev == EV_HIT) { env.mTot = -1.f; state = LS_TRIAL; }   // envelope not built yet
+            else if (ev != EV_CROSSED) { tally_packet(p, sh, ev, k); state = LS_IDLE; }
         }
 
         // ---- a8: ONE rejection trial of u_par for every lane that needs one.  No inner loop: a
@@ -201,12 +296,12 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
         // march, instead of the whole warp waiting for its slowest lane (the paper's "largest source of thread
         // divergence"; E[max of 32 iterations]/E[iterations] = 2.1-4.2) ----
         if (state == LS_TRIAL) {
-            if (env.mTot < 0.f) env = upar_envelope(cell.a, fabsf(x_in));
-            ++rej_iters;
+            if (env.mTot < 0.f) env = upar_envelope(k.cell.a, fabsf(k.x_in));
+            ++k.rej_iters;
             float u;
-            const bool ok = upar_try(env, cell.a, rng.next4(k0, k1), u);
+            const bool ok = upar_try<false>(env, k.cell.a, k.rng.next4(k0, k1), 0.f, 0.f, u);
             // fail-safe: acceptance is >= ~0.2 everywhere; 2^20 rejections cannot happen unless x is NaN
-            if (ok || ++trials >= (1u << 20)) { upar = x_in < 0.f ? -u : u; state = LS_FINISH; }
+            if (ok || ++k.trials >= (1u << 20)) { k.upar = k.x_in < 0.f ? -u : u; state = LS_FINISH; }
         }
 
         // ---- a7, a9-a12: finish the interaction.  The most expensive section: deferred until enough lanes want it ----
@@ -218,62 +313,11 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
         }
         if (fin && (__popc(fin) >= __popc(busy) || __popc(fin) >= FINISH_MIN_LANES)) {
             if (state == LS_FINISH) {
-                // draws of this event: (tau, mu, phi, perp1), (perp2, dust, mix, -)
-                const float4 s1 = rng.next4(k0, k1), s2 = rng.next4(k0, k1);
-                // a7 interaction kind: dust with probability kappa_dust / kappa_total
-                if (p.has_dust && s2.y * hit_kt < cell.kd) {
-                    tally_finish(p, sh, CT_ABSORBED, V, nscat, crossings, rej_iters, rng.id(), ray.kx, ray.ky, ray.kz);
-                    state = LS_IDLE;
-                } else {
-                    const float kx = ray.kx, ky = ray.ky, kz = ray.kz;
-                    float x_crit = 0.f;
-                    if (p.core_skip_mode == 1) x_crit = p.x_crit;
-                    else if (p.core_skip_mode == 2) {              // local: a tau_0 over half a cell (reading A7)
-                        const float atau = cell.a * cell.nsig * 0.5f;
-                        x_crit = atau >= 1.f ? 0.2f * cbrtf(atau) : 0.f;
-                    }
-                    float up1, up2;
-                    sample_uperp(x_in, x_crit, s1.w, s2.x, up1, up2);
-                    const float xsel = p.phase_frame == 0 ? fabsf(x_in - upar) : fabsf(x_in);
-                    const int phase = xsel > p.phase_split_x ? p.phase_wing : p.phase_core;
-                    bool is_dipole;
-                    const float mu = sample_mu(phase, s2.z, s1.y, is_dipole);
-                    float sph, cph;
-                    sincos_uniform(s1.z, sph, cph);
-                    float e1[3], e2[3];
-                    ortho_basis(kx, ky, kz, e1, e2);
-                    if (PEEL) {                                   // a12, before adopting k'
-                        const float mu_o = kx * p.kobs[0] + ky * p.kobs[1] + kz * p.kobs[2];
-                        const float e1o = e1[0] * p.kobs[0] + e1[1] * p.kobs[1] + e1[2] * p.kobs[2];
-                        const float e2o = e2[0] * p.kobs[0] + e2[1] * p.kobs[1] + e2[2] * p.kobs[2];
-                        const float x_o = x_in - upar + upar * mu_o + up1 * e1o + up2 * e2o;
-                        const float V_o = x_o * cell.vth + cell.vx * p.kobs[0] + cell.vy * p.kobs[1] + cell.vz * p.kobs[2];
-                        ++peel_rays;
-                        peel_ray<HUBBLE>(p, sh.voigt, ray, V_o, is_dipole ? 0.75f * (1.f + mu_o * mu_o) : 1.f, peel_cells);
-                    }
-                    const float st = sqrtf(fmaxf(0.f, 1.f - mu * mu));
-                    float nx = mu * kx + st * (cph * e1[0] + sph * e2[0]);
-                    float ny = mu * ky + st * (cph * e1[1] + sph * e2[1]);
-                    float nz = mu * kz + st * (cph * e1[2] + sph * e2[2]);
-                    const float inv = rsqrtf(nx * nx + ny * ny + nz * nz);
-                    nx *= inv; ny *= inv; nz *= inv;
-                    // a11, Eq. 7, recoil dropped: x_out = x_in + u.(k_out - k_in)
-                    const float x_out = x_in - upar + upar * mu + st * (up1 * cph + up2 * sph);
-                    ray_set_k(ray, nx, ny, nz);
-                    inv_ok = false;
-                    V = x_out * cell.vth + cell.vx * nx + cell.vy * ny + cell.vz * nz;
-                    ++nscat;
-                    if (p.v_max > 0.f && fabsf(V) > p.v_max) {
-                        tally_finish(p, sh, CT_TERMINATED, V, nscat, crossings, rej_iters, rng.id(), nx, ny, nz);
-                        state = LS_IDLE;
-                    } else if ((p.max_scatter && nscat >= p.max_scatter) || !(fabsf(V) <= 3.0e38f)) {   // cap, or fail-safe: non-finite V
-                        tally_finish(p, sh, CT_CAPPED, V, nscat, crossings, rej_iters, rng.id(), nx, ny, nz);
-                        state = LS_IDLE;
-                    } else {
-                        tau_rem = -__logf(s1.x);
-                        state = LS_MARCH;
-                    }
-                }
+                const float4 s1 = k.rng.next4(k0, k1), s2 = k.rng.next4(k0, k1);
+                const FinDraws d = fin_draws(s1, s2);
+                const int ev = finish_scatter<HUBBLE, PEEL, false>(p, sh.voigt, k, d, peel_rays, peel_cells, true);
+                if (ev == EV_SCATTERED) state = LS_MARCH;
+                else { tally_packet(p, sh, ev, k); state = LS_IDLE; }
             }
         }
     }
@@ -290,6 +334,7 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
     for (int i = threadIdx.x; i < p.spec_bins + 2; i += blockDim.x)
         if (sh.spectrum[i]) atomicAdd(p.spectrum + i, (unsigned long long)sh.spectrum[i]);
 }
+
 
 // (n_HI, T) alone: 8 B of the cell's packed sector, or two SoA loads.
 __device__ __forceinline__ void load_nT(const WalkParams& p, int64_t i, float& n, float& T) {
@@ -325,16 +370,16 @@ __global__ void raytrace_kernel(const __grid_constant__ WalkParams p, long long 
         if (tau) c = load_cell_raw(p, r.idx);
         else load_nT(p, r.idx, c.nsig, c.a);                  // projections need 8 B of the cell only
         const float n = c.nsig, T = c.a;
-        col += n * len;
-        tn += n * T * len;
+        col = fmaf(n, len, col);
+        tn = fmaf(n * T, len, tn);
         if (tau) {
             derive_cell(p, c);
-            const float vgas = c.vx * kx + c.vy * ky + c.vz * kz + hubble * (s_path + 0.5f * len);
+            const float vgas = fmaf(hubble, fmaf(0.5f, len, s_path), dot3(c.vx, c.vy, c.vz, kx, ky, kz));
             if (c.nsig > 0.f || c.kd > 0.f)
                 for (int j = 0; j < n_v; ++j) {
-                    const float V = v_lo + ((float)j + 0.5f) * dv;
+                    const float V = fmaf((float)j + 0.5f, dv, v_lo);
                     const float kl = c.nsig > 0.f ? c.nsig * voigt_H(s_tab, c.a, (V - vgas) * c.inv_vth) : 0.f;
-                    tau[j] += (kl + c.kd) * len;
+                    tau[j] = fmaf(kl + c.kd, len, tau[j]);
                 }
         }
         s_path += len;
@@ -416,6 +461,7 @@ cudaError_t launch_volume_render(const WalkParams& p, const TransferFn& tf, long
 // register budget: 3 CTAs of 256 threads per SM (<= 80 registers) when the grid fits the 126 MB L2 and the walk is
 // issue-bound, 4 CTAs (64 registers, 32 warps) when it does not and the walk needs more gathers in flight
 // (+18 % on the 512^3 gather workload, -6 % on the cache-resident sphere); 2 CTAs with peel-off (<= 128 registers).
+// The drain kernel follows on the same stream: a persistent grid of 4-warp CTAs whose warps pop parked packets.
 template <bool HUBBLE, bool PEEL, int MIN_CTAS>
 static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {
     int per_sm = 0;
@@ -427,14 +473,27 @@ static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t st
     if (need < blocks) blocks = need < 1 ? 1 : need;
     if (blocks_out) *blocks_out = (int)blocks;
     walk_kernel<HUBBLE, PEEL, MIN_CTAS><<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess || !p.pool) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, drain_kernel<HUBBLE, PEEL>, DRAIN_THREADS, 0);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    long long dblocks = (long long)n_sm * per_sm;
+    const long long cap = (blocks * (WALK_THREADS / 32) * COOP_MAX_LANES + DRAIN_WARPS - 1) / DRAIN_WARPS;   // one warp per slot
+    if (cap < dblocks) dblocks = cap;
+    drain_kernel<HUBBLE, PEEL><<<(unsigned)dblocks, DRAIN_THREADS, 0, stream>>>(p);
     return cudaGetLastError();
 }
+
+// Slots the pool must hold for a launch of `blocks` walk CTAs.
+long long walk_pool_slots(int n_sm) { return (long long)n_sm * 4 * (WALK_THREADS / 32) * COOP_MAX_LANES; }
+int walk_pool_words() { return PK_WORDS; }
 
 cudaError_t launch_walk(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {
     const bool hub = p.hubble != 0.f, peel = p.peel_on != 0;
     const double cells = (double)p.g.nx * p.g.ny * p.g.nz;
     const double grid_bytes = cells * (p.packed ? 32.0 : (p.has_dust ? 24.0 : 20.0));
-    const bool beyond_l2 = grid_bytes > 96.0e6;
+    const bool beyond_l2 = p.walk_variant ? p.walk_variant == 4 : grid_bytes > 96.0e6;
     if (peel) return hub ? launch_variant<true, true, 2>(p, n_sm, stream, blocks_out)
                          : launch_variant<false, true, 2>(p, n_sm, stream, blocks_out);
     if (beyond_l2) return hub ? launch_variant<true, false, 4>(p, n_sm, stream, blocks_out)

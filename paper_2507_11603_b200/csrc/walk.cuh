@@ -86,7 +86,7 @@ __device__ __forceinline__ bool integrate_segment(const WalkParams& p, const flo
     const float Hc = p.hubble;
     int nsub = 1;
     if (Hc != 0.f && c.nsig > 0.f && len > 0.f) {
-        const float xa = (V0 - vk) * c.inv_vth, xb = (V0 - Hc * len - vk) * c.inv_vth;
+        const float xa = (V0 - vk) * c.inv_vth, xb = (fmaf(-Hc, len, V0) - vk) * c.inv_vth;
         const float minabs = xa * xb <= 0.f ? 0.f : fminf(fabsf(xa), fabsf(xb));
         if (minabs <= 6.f) {
             const float q = ceilf(fabsf(Hc * len) * c.inv_vth / p.hubble_eps);
@@ -96,7 +96,7 @@ __device__ __forceinline__ bool integrate_segment(const WalkParams& p, const flo
     const float ds = len / (float)nsub;
     float tau = 0.f;
     for (int j = 0; j < nsub; ++j) {
-        const float Vmid = Hc != 0.f ? V0 - Hc * ((float)j + 0.5f) * ds : V0;   // no 0 * inf when ds = +inf (A24)
+        const float Vmid = Hc != 0.f ? fmaf(-Hc, ((float)j + 0.5f) * ds, V0) : V0;   // no 0 * inf when ds = +inf (A24)
         const float kl = c.nsig > 0.f ? c.nsig * voigt_H(s_tab, c.a, (Vmid - vk) * c.inv_vth) : 0.f;
         const float kt = kl + c.kd;
         const float dtau = kt * ds;
@@ -120,15 +120,16 @@ __device__ __forceinline__ float cell_opacity(const float2* s_tab, const Cell& c
 
 // a12 peel-off: w = P^ exp(-tau_obs), tau_obs integrated from `at` along k_obs to the box face at
 // velocity offset V_o by the same march (a4-a6), dropped beyond tau_peel_max (reading A13); added to
-// (pixel of the starting point projected perpendicular to k_obs, spectral bin of dv = -V at the box face).
+// (pixel of the starting point projected perpendicular to k_obs, spectral bin of dv = -V at the box face).  `add` is
+// false on the lanes that only shadow a packet in the cooperative drain (one lane tallies).
 template <bool HUBBLE>
 __device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, const Ray& at, float V_o, float phat,
-                                      uint32_t& n_cells) {
+                                      uint32_t& n_cells, bool add) {
     const float px0 = (float)at.cx + at.fx - 0.5f * (float)p.g.nx;
     const float py0 = (float)at.cy + at.fy - 0.5f * (float)p.g.ny;
     const float pz0 = (float)at.cz + at.fz - 0.5f * (float)p.g.nz;
-    const float px = ((px0 * p.img1[0] + py0 * p.img1[1] + pz0 * p.img1[2]) * p.peel_inv_width + 0.5f) * (float)p.peel_nx;
-    const float py = ((px0 * p.img2[0] + py0 * p.img2[1] + pz0 * p.img2[2]) * p.peel_inv_width + 0.5f) * (float)p.peel_ny;
+    const float px = fmaf(dot3(px0, py0, pz0, p.img1[0], p.img1[1], p.img1[2]), p.peel_inv_width, 0.5f) * (float)p.peel_nx;
+    const float py = fmaf(dot3(px0, py0, pz0, p.img2[0], p.img2[1], p.img2[2]), p.peel_inv_width, 0.5f) * (float)p.peel_ny;
     if (!(px >= 0.f && px < (float)p.peel_nx && py >= 0.f && py < (float)p.peel_ny)) return;
     Ray r = at;
     ray_set_direction(r, p.kobs[0], p.kobs[1], p.kobs[2]);
@@ -138,11 +139,11 @@ __device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, 
         const int ex = dda_next_face(r, p.g, len);
         if (!(len < CUDART_INF_F)) return;                    // reading A24: never reaches a box face -> dropped
         const Cell c = load_cell(p, dda_linear(r, p.g));
-        const float vk = c.vx * r.kx + c.vy * r.ky + c.vz * r.kz;
+        const float vk = dot3(c.vx, c.vy, c.vz, r.kx, r.ky, r.kz);
         float dtau, s_hit, kt;
         integrate_segment<HUBBLE>(p, s_tab, c, V, vk, len, 3.0e38f, dtau, s_hit, kt);
         tau += dtau;
-        if (HUBBLE) V -= p.hubble * len;
+        if (HUBBLE) V = fmaf(-p.hubble, len, V);
         ++n_cells;
         if (tau > p.tau_peel_max) return;
         // peel rays leave through the first box face they meet, periodic or not
@@ -156,7 +157,178 @@ __device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, 
     if (iv < 0 || iv >= p.peel_nv) return;
     const float w = phat * __expf(-tau);
     const unsigned long long q = (unsigned long long)__float2ull_rn(w * (float)CUBE_FIXED_SCALE);
-    if (q) atomicAdd(p.cube + ((size_t)(int)py * p.peel_nx + (int)px) * p.peel_nv + iv, q);
+    if (q && add) atomicAdd(p.cube + ((size_t)(int)py * p.peel_nx + (int)px) * p.peel_nv + iv, q);
+}
+
+// ---- one packet, and the steps of its life as functions shared by every code variant that walks it ----
+struct Packet {
+    Ray ray;
+    Cell cell;                   // the cell the packet is in (valid unless `stale`)
+    BlockRng rng;
+    float V;                     // lab-frame velocity offset from line centre, km/s
+    float tau_rem;               // optical depth left to the next interaction
+    float hit_kt, x_in, upar;    // at the interaction site: total opacity, gas-frame frequency, accepted u_par
+    uint32_t nscat, crossings, rej_iters, trials;
+    bool stale;                  // cell must be (re)gathered / derived before use
+    bool inv_ok;                 // 1/k of the current direction is in `ray`
+};
+
+enum : int { EV_CROSSED = 0, EV_HIT = 1, EV_ESCAPED = 2, EV_TERMINATED = 3, EV_CAPPED = 4, EV_ABSORBED = 5, EV_SCATTERED = 6 };
+
+// a2/a3: emission of photon `id`: source ∝ luminosity, isotropic k (reading A22), Gaussian line in the
+// source cell's gas frame (A10), tau_target = -ln u.  dV_out: the line offset, for the peel of the unscattered packet.
+__device__ __forceinline__ void emit_packet(const WalkParams& p, Packet& k, unsigned long long id, uint32_t k0, uint32_t k1,
+                                            float& dV_out) {
+    k.rng.init(id);
+    const float4 e1 = k.rng.next4(k0, k1), e2 = k.rng.next4(k0, k1);   // (src, mu, phi, g1), (g2, tau, -, -)
+    const double us = (double)e1.x;
+    long long lo = 0, hi = p.n_src - 1;           // smallest j with us < cdf[j]
+    while (lo < hi) { const long long mid = (lo + hi) >> 1; if (us < p.src_cdf[mid]) hi = mid; else lo = mid + 1; }
+    const float mu0 = fmaf(2.f, e1.y, -1.f);
+    float sp, cp;
+    sincos_uniform(e1.z, sp, cp);
+    const float st0 = sqrtf(fmaxf(0.f, fmaf(-mu0, mu0, 1.f)));
+    const float gauss = sqrtf(2.f * neg_log(e1.w)) * cos_uniform(e2.x);
+    dda_locate(k.ray, p.g, p.src_pos[3 * lo], p.src_pos[3 * lo + 1], p.src_pos[3 * lo + 2]);
+    ray_set_k(k.ray, st0 * cp, st0 * sp, mu0);
+    k.inv_ok = false;
+    k.cell = load_cell(p, dda_linear(k.ray, p.g));
+    k.stale = false;
+    const float dV = p.src_sigma[lo] * gauss;
+    k.V = dot3(k.cell.vx, k.cell.vy, k.cell.vz, k.ray.kx, k.ray.ky, k.ray.kz) + dV;
+    k.nscat = 0; k.crossings = 0; k.rej_iters = 0; k.trials = 0;
+    k.tau_rem = neg_log(e2.y);
+    dV_out = dV;
+}
+
+// a4-a7: one cell step.  EV_HIT: the packet sits at its interaction site (hit_kt, x_in set); EV_CROSSED: it entered the
+// next cell; else it ended (escaped / terminated / capped).  EARLY: the variant for grids beyond L2 issues the gather
+// of the next cell at the face crossing and derives it at first use.
+template <bool HUBBLE, bool EARLY>
+__device__ __forceinline__ int march_step(const WalkParams& p, const float2* s_tab, Packet& k) {
+    if (k.stale) {
+        if (EARLY) derive_cell(p, k.cell);
+        else k.cell = load_cell(p, dda_linear(k.ray, p.g));
+        k.stale = false;
+    }
+    const float vk = dot3(k.cell.vx, k.cell.vy, k.cell.vz, k.ray.kx, k.ray.ky, k.ray.kz);
+    bool hit = false;
+    float len = 0.f, dtau = 0.f, s_hit = 0.f, kt = 0.f;
+    int ex = 0;
+    if (!HUBBLE) {
+        // Piecewise-constant cell: the interaction lies at s = tau / kappa if that is inside the cell.
+        // Deep in an optically thick cell s is far smaller than the distance to the nearest face, which bounds the
+        // segment length from below: no DDA step and no reciprocals of k are needed at all.
+        kt = cell_opacity(s_tab, k.cell, k.V, vk);
+        const float s = kt > 0.f ? k.tau_rem / kt : CUDART_INF_F;
+        if (kt > 0.f && s <= dda_min_face_distance(k.ray, p.g)) {
+            hit = true; s_hit = s;
+        } else {
+            if (!k.inv_ok) { ray_set_inv(k.ray); k.inv_ok = true; }
+            ex = dda_next_face(k.ray, p.g, len);
+            hit = kt > 0.f && s <= len;
+            s_hit = s;
+            dtau = kt * len;
+        }
+    } else {
+        if (!k.inv_ok) { ray_set_inv(k.ray); k.inv_ok = true; }
+        ex = dda_next_face(k.ray, p.g, len);
+        hit = integrate_segment<true>(p, s_tab, k.cell, k.V, vk, len, k.tau_rem, dtau, s_hit, kt);
+    }
+    if (hit) {
+        dda_advance_within(k.ray, p.g, s_hit);
+        if (HUBBLE) { if (p.hubble != 0.f) k.V = fmaf(-p.hubble, s_hit, k.V); }
+        k.hit_kt = kt;
+        k.x_in = (k.V - vk) * k.cell.inv_vth;
+        k.trials = 0u;
+        return EV_HIT;
+    }
+    // reading A24: infinite segment (ray parallel to every non-frozen axis) without interaction: the packet can neither
+    // leave nor be followed -> capped
+    if (!(len < CUDART_INF_F)) return EV_CAPPED;
+    k.tau_rem -= dtau;
+    if (HUBBLE) k.V = fmaf(-p.hubble, len, k.V);
+    ++k.crossings;
+    if (!dda_cross(k.ray, p.g, ex, len)) return EV_ESCAPED;
+    if (p.v_max > 0.f && fabsf(k.V) > p.v_max) return EV_TERMINATED;
+    if (k.crossings >= p.max_crossings) return EV_CAPPED;     // reading A26
+    // a5: beyond L2 the gather is issued now and used next iteration, hiding the loop control and the other stage
+    // sections in its shadow; a cache-resident grid gathers at first use (fewer live values)
+    if (EARLY) k.cell = load_cell_raw(p, dda_linear(k.ray, p.g));
+    k.stale = true;
+    return EV_CROSSED;
+}
+
+// The random numbers of one FINISH, turned into what the event needs.  Draws: (tau, mu, phi, perp1), (perp2, dust, mix, -).
+struct FinDraws {
+    float tau_next;              // -ln s1.x
+    float r_mu, mu_dip;          // s1.y, and dipole_mu(s1.y) if computed ahead
+    float sphi, cphi;            // azimuth of k'
+    float nl_p1, spsi, cpsi;     // u_perp: -ln s1.w, angle 2 pi s2.x
+    float u_dust, u_mix;         // s2.y, s2.z
+};
+
+__device__ __forceinline__ FinDraws fin_draws(const float4 s1, const float4 s2) {
+    FinDraws d;
+    d.tau_next = neg_log(s1.x);
+    d.r_mu = s1.y; d.mu_dip = 0.f;
+    sincos_uniform(s1.z, d.sphi, d.cphi);
+    d.nl_p1 = neg_log(s1.w);
+    sincos_uniform(s2.x, d.spsi, d.cpsi);
+    d.u_dust = s2.y; d.u_mix = s2.z;
+    return d;
+}
+
+// a7, a9-a12: the interaction itself (PAPER.md 2.3.1): dust or line, u_perp (Eq. 5, core-skipping
+// PAPER.md:244), phase function, rotation, Eq. 7 with the recoil dropped, peel-off
+// before k' is adopted, new tau_target.  Returns EV_ABSORBED / EV_TERMINATED / EV_CAPPED / EV_SCATTERED.
+template <bool HUBBLE, bool PEEL, bool PRE>
+__device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2* s_tab, Packet& k, const FinDraws& d,
+                                              uint32_t& peel_rays, uint32_t& peel_cells, bool add) {
+    if (p.has_dust && d.u_dust * k.hit_kt < k.cell.kd) return EV_ABSORBED;
+    const float kx = k.ray.kx, ky = k.ray.ky, kz = k.ray.kz;
+    const Cell& c = k.cell;
+    float x_crit = 0.f;
+    if (p.core_skip_mode == 1) x_crit = p.x_crit;
+    else if (p.core_skip_mode == 2) {              // local: a tau_0 over half a cell (reading A7)
+        const float atau = c.a * c.nsig * 0.5f;
+        x_crit = atau >= 1.f ? 0.2f * cbrtf(atau) : 0.f;
+    }
+    float up1, up2;
+    uperp_from(k.x_in, x_crit, d.nl_p1, d.spsi, d.cpsi, up1, up2);
+    const float xsel = p.phase_frame == 0 ? fabsf(k.x_in - k.upar) : fabsf(k.x_in);
+    const int phase = xsel > p.phase_split_x ? p.phase_wing : p.phase_core;
+    bool is_dipole;
+    const float mu = sample_mu<PRE>(phase, d.u_mix, d.r_mu, d.mu_dip, is_dipole);
+    float e1[3], e2[3];
+    ortho_basis(kx, ky, kz, e1, e2);
+    const float xa = k.x_in - k.upar;                 // atom-frame frequency
+    if (PEEL) {                                       // a12, before adopting k'
+        const float mu_o = dot3(kx, ky, kz, p.kobs[0], p.kobs[1], p.kobs[2]);
+        const float e1o = dot3(e1[0], e1[1], e1[2], p.kobs[0], p.kobs[1], p.kobs[2]);
+        const float e2o = dot3(e2[0], e2[1], e2[2], p.kobs[0], p.kobs[1], p.kobs[2]);
+        const float x_o = fmaf(up2, e2o, fmaf(up1, e1o, fmaf(k.upar, mu_o, xa)));
+        const float V_o = fmaf(x_o, c.vth, dot3(c.vx, c.vy, c.vz, p.kobs[0], p.kobs[1], p.kobs[2]));
+        ++peel_rays;
+        // mix: the sampled branch weights the ray (unbiased; reading A27)
+        peel_ray<HUBBLE>(p, s_tab, k.ray, V_o, is_dipole ? 0.75f * fmaf(mu_o, mu_o, 1.f) : 1.f, peel_cells, add);
+    }
+    const float st = sqrtf(fmaxf(0.f, fmaf(-mu, mu, 1.f)));
+    float nx = fmaf(st, fmaf(d.cphi, e1[0], d.sphi * e2[0]), mu * kx);
+    float ny = fmaf(st, fmaf(d.cphi, e1[1], d.sphi * e2[1]), mu * ky);
+    float nz = fmaf(st, fmaf(d.cphi, e1[2], d.sphi * e2[2]), mu * kz);
+    const float inv = rsqrtf(dot3(nx, ny, nz, nx, ny, nz));
+    nx *= inv; ny *= inv; nz *= inv;
+    // a11, Eq. 7, recoil dropped: x_out = x_in + u.(k_out - k_in)
+    const float x_out = fmaf(st, fmaf(up1, d.cphi, up2 * d.sphi), fmaf(k.upar, mu, xa));
+    ray_set_k(k.ray, nx, ny, nz);
+    k.inv_ok = false;
+    k.V = fmaf(x_out, c.vth, dot3(c.vx, c.vy, c.vz, nx, ny, nz));
+    ++k.nscat;
+    if (p.v_max > 0.f && fabsf(k.V) > p.v_max) return EV_TERMINATED;
+    if ((p.max_scatter && k.nscat >= p.max_scatter) || !(fabsf(k.V) <= 3.0e38f)) return EV_CAPPED;   // cap, or fail-safe: non-finite V
+    k.tau_rem = d.tau_next;
+    return EV_SCATTERED;
 }
 
 }  // namespace thor

@@ -44,7 +44,7 @@ class Opts(C.Structure):
         ("tau_peel_max", C.c_double),
         ("photon_id_offset", C.c_uint64), ("max_scatter", C.c_uint64),
         ("raw_output", C.c_int32), ("accumulate", C.c_int32),
-        ("max_crossings", C.c_uint64),
+        ("max_crossings", C.c_uint64), ("walk_variant", C.c_int32), ("drain_mode", C.c_int32),
     ]
 
 
@@ -146,14 +146,16 @@ class Context:
 
     @classmethod
     def from_workload(cls, grid, host=False, device="cuda", pack=False):
-        """grid: the dict made by paper_2507_11603_b200.workloads (numpy float32 fields)."""
+        """grid: the dict made by paper_2507_11603_b200.workloads (numpy float32 fields) or .workloads_device (CUDA
+        tensors, borrowed as they are)."""
         keys = ("nHI", "T", "vx", "vy", "vz", "kdust")
         if host:
             arrs = [grid.get(k) for k in keys]
         else:
             import torch
-            arrs = [None if grid.get(k) is None else torch.from_numpy(np.ascontiguousarray(grid[k], np.float32)).to(device)
-                    for k in keys]
+            arrs = [None if grid.get(k) is None else
+                    (grid[k] if isinstance(grid[k], torch.Tensor) else
+                     torch.from_numpy(np.ascontiguousarray(grid[k], np.float32)).to(device)) for k in keys]
         return cls(grid["nx"], grid["ny"], grid["nz"], grid["cell_cm"], *arrs,
                    periodic=grid.get("periodic", (0, 0, 0)), host=host, pack=pack)
 

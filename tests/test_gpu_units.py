@@ -152,3 +152,68 @@ def test_single_scatter_against_oracle(thor, oracle, a, x_in, x_crit, phase):
     assert stats.kstest(phi, stats.uniform(-math.pi, 2 * math.pi).cdf).pvalue > 1e-3
     m2 = {0: 1 / 3, 1: 2 / 5, 2: (1 / 3) * (1 / 3) + (2 / 3) * (2 / 5)}[phase]   # pin P10
     assert abs((k[:, 2] ** 2).mean() - m2) < 5 * 0.3 / math.sqrt(n)
+
+
+def test_dda_linear_index_beyond_2_31(thor, oracle):
+    """a4 with 64-bit cell indices (BASELINE.json config 5 has 3.6e9 cells): 1e5 random rays through a VIRTUAL
+    2049 x 1024 x 1024 grid (2.15e9 cells; the trace reads no field) — hashes of the 64-bit linear indices and of the
+    fp32 segment lengths equal the oracle's."""
+    dims = (2049, 1024, 1024)
+    org, dirs = W.random_rays(100_000, dims, seed=17)
+    g = thor.unit_dda_trace(dims, (0, 0, 0), org, dirs, max_steps=1 << 14)
+    o = oracle.dda_trace(dims, (0, 0, 0), org, dirs, max_steps=1 << 14)
+    assert np.array_equal(g["count"], o["count"])
+    assert np.array_equal(g["hash_idx"], o["hash_idx"]) and np.array_equal(g["hash_len"], o["hash_len"])
+    # the grid really is beyond 2^31: a ray ending in the far corner visits indices above it
+    far = thor.unit_dda_trace(dims, (0, 0, 0), np.array([[2040.5, 1020.5, 1020.5]], np.float32),
+                              np.array([[0.6, 0.0, 0.8]], np.float32), max_steps=64, want_seq=True)
+    assert far["seq_idx"].max() > 2 ** 31
+
+
+def test_gathers_beyond_2_31_on_a_borrowed_grid(thor):
+    """A borrowed 2049 x 1024 x 1024 grid whose five field pointers alias ONE 8.6 GB device buffer holding an
+    index-dependent pattern: (i) thor_raytrace's column density along rays through cells above 2^31 equals
+    sum(buffer[idx] * len) over the index / length sequence of the DDA unit trace (itself pinned to the oracle above);
+    (ii) the walk emits from source cells above 2^31 with V = v_cell . k = buffer[idx] (kx + ky + kz) and crosses exactly
+    the cells the DDA counts."""
+    import torch
+    nx, ny, nz = 2049, 1024, 1024
+    N = nx * ny * nz
+    buf = torch.empty(N, dtype=torch.float32, device="cuda")
+    step = 1 << 27
+    for i0 in range(0, N, step):                              # pattern: 50 + (i mod 977), exact in fp32
+        i1 = min(N, i0 + step)
+        buf[i0:i1] = (torch.arange(i0, i1, device="cuda", dtype=torch.int64) % 977 + 50).float()
+    f = buf.view(nz, ny, nx)
+    ctx = thor.Context(nx, ny, nz, 1.0, f, f, f, f, f, None, validate=False)     # cell_cm = 1 cm: transparent
+    try:
+        org = np.array([[2040.5, 1020.5, 1010.25], [1500.25, 900.5, 1000.75], [2048.5, 1023.5, 1023.5]], np.float32)
+        dirs = np.array([[0.6, 0.0, 0.8], [0.48, 0.6, 0.64], [-0.8, -0.6, 0.0]], np.float32)
+        col = ctx.raytrace(org, dirs)["column"]
+        for j in range(3):
+            t = thor.unit_dda_trace((nx, ny, nz), (0, 0, 0), org[j:j + 1], dirs[j:j + 1], max_steps=4096, want_seq=True)
+            idx = torch.from_numpy(t["seq_idx"]).cuda()
+            assert int(idx.max()) > 2 ** 31
+            vals = buf[idx].double().cpu().numpy()
+            expect = float((vals * t["seq_len"].astype(np.float64)).sum())
+            assert abs(col[j] - expect) <= 2e-5 * expect, (j, col[j], expect)
+        n = 2000
+        src = np.array([[2040.5, 1020.5, 1010.25], [2047.5, 1000.5, 1023.5]], np.float32)
+        ctx.sources_set(src, np.ones(2, np.float32), np.zeros(2, np.float32))
+        ctx.run(n, 5, dict(spec_mode=1, spec_bins=10, spec_lo=-1e4, spec_hi=1e4, raw_output=1))
+        raw, c = ctx.raw(), ctx.counters()
+        assert c["escaped"] == n and c["scatterings"] == 0
+        k = np.stack([raw["kx"], raw["ky"], raw["kz"]], 1)
+        lin = (np.floor(src[:, 2]).astype(np.int64) * ny + np.floor(src[:, 1]).astype(np.int64)) * nx + np.floor(src[:, 0]).astype(np.int64)
+        assert lin.min() > 2 ** 31
+        vcell = (lin % 977 + 50).astype(np.float64)
+        ksum = k.astype(np.float64).sum(1)
+        which = np.argmin(np.abs(raw["V"][:, None].astype(np.float64) - vcell[None, :] * ksum[:, None]), axis=1)
+        assert np.allclose(raw["V"], vcell[which] * ksum, rtol=2e-6, atol=1e-3)
+        assert 0.4 < which.mean() < 0.6                          # both sources emit
+        cnt = thor.unit_dda_trace((nx, ny, nz), (0, 0, 0), src[which], k, max_steps=1 << 13)["count"]
+        assert int(cnt.astype(np.int64).sum()) == c["cell_crossings"]
+    finally:
+        ctx.close()
+        del buf, f
+        torch.cuda.empty_cache()

@@ -14,7 +14,7 @@ import pytest
 from scipy import stats
 
 from paper_2507_11603_b200 import workloads as W
-from conftest import statistical
+from conftest import scaled, statistical
 
 pytestmark = pytest.mark.gpu
 
@@ -82,6 +82,7 @@ def _statistical_parity(g, o, n_g, n_o, spec_scale=1.0):
 @pytest.mark.parametrize("tau0,n", [(1e2, 40_000), (1e3, 20_000), (1e4, 3_000)])
 @statistical()
 def test_static_sphere_ladder(thor, oracle, tau0, n):
+    n = scaled(n)
     w = W.static_sphere(n=32, tau0=tau0, T=10.0, n_photons=n)
     g = thor.run_workload(w)
     o = oracle.run(w["grid"], w["sources"], w["opts"], n, w["seed"])
@@ -120,7 +121,7 @@ def test_expanding_shell(thor, oracle):
     """Config 2 at 48^3 for the oracle's sake (same recipe: N_HI = 1e20, T = 1e4 K, 200 km/s, tau_d = 1, sigma_src =
     50 km/s); packets that reach the line core scatter ~1e6 times, so both sides cap at max_scatter = 20000 and the
     capped count must agree too."""
-    n = 20_000
+    n = scaled(20_000)
     w = W.expanding_shell(n=48, n_photons=n)
     opts = dict(w["opts"], max_scatter=20_000)
     w = dict(w, opts=opts)
@@ -141,7 +142,7 @@ def test_expanding_shell(thor, oracle):
 def test_static_slab_core_skip(thor, oracle):
     """Config 3 as stated (1 x 1 x 256 periodic in x/y, tau0 = 1e7, T = 1e4 K, x_crit from a tau0, dipole core /
     isotropic wings), 6000 packets on both sides."""
-    n = 6000
+    n = scaled(6000)
     w = W.static_slab(n_photons=n)
     assert abs(w["opts"]["x_crit"] - 3.354) < 2e-3
     g = thor.run_workload(w)
@@ -160,7 +161,7 @@ def test_static_slab_core_skip(thor, oracle):
 def test_slab_paper_phase_assignment(thor, oracle):
     """The paper's own assignment (1/3-2/3 mix in the core, dipole in the wings; reading A4), with dust,
     both split frames (reading A3), no core skipping at a modest tau0."""
-    n = 10_000
+    n = scaled(10_000)
     for frame in (0, 1):
         w = W.static_slab(nz=64, tau0=1e3, T=1e4, core_skip=False, n_photons=n, tau_d=0.03, phase_core=2, phase_wing=1)
         opts = dict(w["opts"], phase_frame=frame)
@@ -192,7 +193,7 @@ def test_turbulent_box_with_peel(thor, oracle):
     """Config 4 at 48^3: lognormal density and temperature, Gaussian k^-4 velocity field, sources ∝ n^2, local
     core-skipping, peel-off along +z into a cube.  Cells of 1e-3 pc instead of 10 pc keep the scattering count per
     packet (~1e3) within the oracle's reach; at 10 pc the dense source cells have tau0 > 1e7 each."""
-    n = 3000
+    n = scaled(3000)
     w = W.turbulent_box(n=48, n_src=512, n_photons=n, peel_pix=32, peel_bins=50, cell_pc=1e-3)
     opts = dict(w["opts"], max_scatter=50_000)
     w = dict(w, opts=opts)
@@ -209,7 +210,7 @@ def test_turbulent_box_with_peel(thor, oracle):
 @statistical()
 def test_peel_off_oblique_observer(thor, oracle):
     """Peel-off toward an oblique direction with the dipole phase function (P^ = 3/4 (1 + mu^2)) and dust."""
-    n = 4000
+    n = scaled(4000)
     w = W.expanding_shell(n=32, N_HI=1e15, T=1e4, v_exp=50.0, tau_d=0.5, sigma_src=20.0, n_photons=n)
     opts = dict(w["opts"], phase_core=1, phase_wing=1, peel_on=1, k_obs=(0.3, -0.5, 0.8), peel_nx=16, peel_ny=16,
                 peel_nv=40, peel_v_lo=-300.0, peel_v_hi=300.0, peel_width_cells=56.0, tau_peel_max=30.0)
@@ -239,7 +240,7 @@ def test_cosmic_web_hubble_drift(thor, oracle):
     """Config 5 at 48^3 with the mean density lowered to 1e-8 (Gunn-Peterson depth ~200 instead of ~2e4, a few
     hundred scatterings per packet): Hubble drift with sub-cell stepping (reading A12), termination at |V| > v_max
     (60 km/s here, as the 48-cell box only spans 110 km/s), surface-brightness map by peel-off."""
-    n = 4000
+    n = scaled(4000)
     w = W.cosmic_web(n=48, n_src=512, n_photons=n, mean_n=1e-8, map_pix=32, v_max=60.0)
     g = thor.run_workload(w)
     o = oracle.run(w["grid"], w["sources"], w["opts"], n, w["seed"])
@@ -506,3 +507,134 @@ def test_peel_ray_under_hubble_drift(thor, oracle):
     assert g["counters"] == o["counters"] and g["counters"]["capped"] == n
     assert np.count_nonzero(g["cube"]) == 1 and np.argmax(g["cube"]) == np.argmax(o["cube"])
     assert abs(g["cube"].max() / o["cube"].max() - 1.0) < 1e-4
+
+
+# ---------------------------------------------------------------- round 2: every kernel variant, every stated bar
+def _cube_bins_within_4sigma(cg, co, wmax=1.0, min_sum=10.0):
+    """Peel cubes voxel by voxel: walking the cube in memory order (spectral axis fastest, then pixels), voxels are merged
+    until the two sides together hold min_sum * wmax of weight, and every merged bin must agree within 4 sigma.  A ray's
+    weight is at most wmax, so the variance of a sum S of weights is at most wmax * S (conservative)."""
+    g, o = cg.ravel(), co.ravel()
+    csum = np.cumsum(g + o)
+    edges = np.searchsorted(csum, np.arange(min_sum * wmax, csum[-1], min_sum * wmax))
+    edges = np.unique(np.concatenate([[0], edges + 1, [g.size]]))
+    bg, bo = np.add.reduceat(g, edges[:-1]), np.add.reduceat(o, edges[:-1])
+    z = np.abs(bg - bo) / np.sqrt(wmax * (bg + bo) + 1e-30)
+    assert len(bg) > 20, len(bg)
+    assert z.max() <= 4.0, (z.max(), len(bg))
+    return len(bg)
+
+
+@statistical()
+def test_peel_cube_bin_by_bin(thor, oracle):
+    """a12 voxel by voxel (not through marginals): turbulent box with local core-skipping and an oblique dipole case; a
+    transposed pixel map or a spectral shift of one bin moves weight between merged bins and fails this."""
+    n = scaled(4000)
+    w = W.turbulent_box(n=48, n_src=512, n_photons=n, peel_pix=32, peel_bins=50, cell_pc=1e-3)
+    w = dict(w, opts=dict(w["opts"], max_scatter=50_000))
+    g = thor.run_workload(w)
+    o = oracle.run(w["grid"], w["sources"], w["opts"], n, w["seed"])
+    _cube_bins_within_4sigma(g["cube"], o["cube"])
+    w = W.expanding_shell(n=32, N_HI=1e15, T=1e4, v_exp=50.0, tau_d=0.5, sigma_src=20.0, n_photons=n)
+    opts = dict(w["opts"], phase_core=1, phase_wing=1, peel_on=1, k_obs=(0.3, -0.5, 0.8), peel_nx=16, peel_ny=12,
+                peel_nv=40, peel_v_lo=-300.0, peel_v_hi=300.0, peel_width_cells=56.0, tau_peel_max=30.0)
+    g = thor.run_workload(dict(w, opts=opts))
+    o = oracle.run(w["grid"], w["sources"], opts, n, w["seed"])
+    _cube_bins_within_4sigma(g["cube"], o["cube"], wmax=1.5)
+    # the transposed cube must NOT pass: the check has teeth
+    with pytest.raises(AssertionError):
+        _cube_bins_within_4sigma(np.ascontiguousarray(g["cube"][::-1, :, :]), o["cube"], wmax=1.5)
+
+
+def test_full_size_ifu_cube(thor):
+    """BASELINE.json config 4's 256 x 256 x 400 cube (105 MB of doubles, 210 MB of fixed point on the device): allocation,
+    fixed-point range and thor_tally_get at full size.  The same packets peeled into a 64 x 64 x 100 cube must give the
+    fine cube summed over 4 x 4 x 4 blocks: the sums are integers (2^-32 fixed point), so equality is exact wherever the
+    fp32 bin edges agree."""
+    n = 3000
+    w = W.turbulent_box(n=32, n_src=256, n_photons=n, peel_pix=256, peel_bins=400, cell_pc=1e-3)
+    w = dict(w, opts=dict(w["opts"], max_scatter=2000))
+    fine = thor.run_workload(w, raw=False)
+    coarse = thor.run_workload(dict(w, opts=dict(w["opts"], peel_nx=64, peel_ny=64, peel_nv=100)), raw=False)
+    cf, cc = fine["cube"], coarse["cube"]
+    assert cf.shape == (256, 256, 400) and cf.sum() > 0.2 * n
+    assert fine["counters"] == coarse["counters"]
+    reb = cf.reshape(64, 4, 64, 4, 100, 4).sum(axis=(1, 3, 5))
+    assert abs(reb.sum() - cc.sum()) <= 1e-6 * cc.sum()
+    assert np.count_nonzero(np.abs(reb - cc) > 1e-9) <= 0.002 * np.count_nonzero(cc) + 4   # bin-edge roundings only
+
+
+def test_beyond_l2_kernel_variant(thor, oracle):
+    """The walk kernel launched for grids beyond L2 (4 CTAs per SM, gather issued at the face crossing) — picked
+    automatically above 96 MB of fields, here a 176^3 cosmic web (109 MB): (i) its raw records equal, bit for bit, those
+    of the cache-resident variant forced through opts.walk_variant, and those of a run that finishes every packet inside
+    the walk kernel (drain_mode = 1); (ii) it agrees with the oracle statistically."""
+    n = 3000
+    w = W.cosmic_web(n=176, n_src=2048, n_photons=n, mean_n=1e-8, map_pix=16, v_max=200.0)
+    opts = dict(w["opts"], peel_on=0)
+    ctx = thor.Context.from_workload(w["grid"])
+    try:
+        ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
+        runs = {}
+        for tag, extra in (("auto", {}), ("v3", dict(walk_variant=3)), ("v4", dict(walk_variant=4)), ("nodrain", dict(drain_mode=1))):
+            ctx.run(n, w["seed"], dict(opts, raw_output=1, **extra))
+            runs[tag] = dict(raw=ctx.raw(), counters=ctx.counters(), spectrum=ctx.spectrum(), nscat_hist=ctx.nscat_hist())
+    finally:
+        ctx.close()
+    for tag in ("v3", "v4", "nodrain"):
+        assert runs["auto"]["raw"].tobytes() == runs[tag]["raw"].tobytes(), tag
+        assert runs["auto"]["counters"] == runs[tag]["counters"], tag
+    o = oracle.run(w["grid"], w["sources"], opts, n, w["seed"])
+    _conserved(runs["auto"], n)
+    _statistical_parity(runs["auto"], o, n, n)
+    assert runs["auto"]["counters"]["scatterings"] > n
+
+
+def test_drain_kernel_is_bit_identical(thor):
+    """The cooperative drain kernel (DESIGN.md 4.6) walks the packets the walk kernel parks once the photon counter is dry;
+    it must change no bit of any result: static and Hubble-drift walks, with peel-off and dust, against drain_mode = 1."""
+    cases = [dict(W.expanding_shell(n=32, n_photons=20_000), tag="shell"),
+             dict(W.static_slab(n_photons=3000), tag="slab"),
+             dict(W.turbulent_box(n=32, n_src=256, n_photons=3000, peel_pix=16, peel_bins=20, cell_pc=1e-3), tag="turb"),
+             dict(W.cosmic_web(n=32, n_src=256, n_photons=3000, mean_n=1e-8, map_pix=16, v_max=40.0), tag="web")]
+    for w in cases:
+        w["opts"] = dict(w["opts"], max_scatter=20_000)
+        a = thor.run_workload(w, drain_mode=0)
+        b = thor.run_workload(w, drain_mode=1)
+        assert a["raw"].tobytes() == b["raw"].tobytes(), w["tag"]
+        assert a["counters"] == b["counters"], w["tag"]
+        assert np.array_equal(a["spectrum"], b["spectrum"]) and np.array_equal(a["nscat_hist"], b["nscat_hist"])
+        if a["cube"] is not None:
+            assert np.array_equal(a["cube"], b["cube"]), w["tag"]
+
+
+def test_mean_scattering_count_within_one_percent(thor, oracle):
+    """BASELINE.json's bar as stated: mean scattering count within 1 % — on a rung where the standard error lets it bind
+    (reading A23): tau0 = 1e2, 4e5 packets per side, 3 SE = 0.6 %.  Plain |dmean| <= 1 %, no SE allowance."""
+    n = 400_000
+    w = W.static_sphere(n=32, tau0=1e2, T=10.0, n_photons=n)
+    g = thor.run_workload(w)
+    o = oracle.run(w["grid"], w["sources"], w["opts"], n, w["seed"])
+    mg, mo = g["raw"]["nscat"].astype(np.float64), o["raw"]["nscat"].astype(np.float64)
+    se = math.sqrt(mg.var() / n + mo.var() / n)
+    assert 3 * se < 0.008 * mo.mean(), (se, mo.mean())
+    assert abs(mg.mean() - mo.mean()) <= 0.01 * mo.mean(), (mg.mean(), mo.mean(), se)
+    assert stats.ks_2samp(g["raw"]["V"], o["raw"]["V"]).pvalue > 0.01
+    _bins_within_4sigma(g["spectrum"], o["spectrum"])
+    _bins_within_4sigma(g["nscat_hist"], o["nscat_hist"])
+
+
+@statistical()
+def test_long_core_chains_at_1e4K(thor, oracle):
+    """The regime config 2's bench time is spent in: chains of 1e5-1e6 CORE scatterings at T = 1e4 K (a = 4.7e-4) in fp32
+    against fp64, uncapped.  A uniform static sphere with tau0 = 3e5 puts EVERY packet there (<N> ~ 3e5), which the
+    dusty shell does for 0.3 % of its packets only.  (Picking the shell's long photon ids from a GPU run and walking the
+    same ids in the oracle would compare a sample selected for being long on one side with an unselected one: fp32 and
+    fp64 trajectories part ways after a few scatterings, reading A17.)"""
+    n = scaled(300)
+    w = W.static_sphere(n=32, tau0=3e5, T=1e4, n_photons=n)
+    g = thor.run_workload(w)
+    o = oracle.run(w["grid"], w["sources"], w["opts"], n, w["seed"])
+    _conserved(g, n)
+    assert g["counters"]["escaped"] == n and g["raw"]["nscat"].mean() > 1e5
+    _statistical_parity(g, o, n, n)
