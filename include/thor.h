@@ -43,6 +43,13 @@ typedef enum {
                                      arrays are not referenced after thor_grid_create returns.  Results are
                                      bit-identical to the borrowed SoA layout. */
 
+#define THOR_GRID_L2_PERSIST 0x400u /* with THOR_GRID_PACK: thor_sources_set puts an L2 access-policy window (persisting
+                                     lines) on the contiguous z-slabs of the packed grid that hold the most source
+                                     luminosity, as large as the device allows (BASELINE.json north_star; measured in
+                                     DESIGN.md 5).  Results do not depend on it */
+#define THOR_GRID_L2_FETCH32 0x800u /* cudaLimitMaxL2FetchGranularity = 32 B for this process: a cell gather needs one
+                                     32-byte sector; the default granularity pulls its neighbours as well */
+
 /* The dataset (uniform Cartesian grid, fields constant per cell).  Six SoA fp32 arrays, dense
  * row-major [nz][ny][nx] (x fastest): nHI [cm^-3], T [K], vx, vy, vz [km/s], and kdust [cm^-1], the dust ABSORPTION
  * coefficient (NULL = no dust; reading A21).  cell_cm = cell edge in cm.  A periodic axis of extent 1 is

@@ -4,6 +4,7 @@
 #include <cstring>
 #include <chrono>
 #include "walker.hpp"
+#include "gridless.hpp"
 
 using namespace orc;
 
@@ -172,6 +173,32 @@ double orc_run(int nx, int ny, int nz, int px, int py, int pz, double cell_cm,
     if (nscat_hist) std::memcpy(nscat_hist, res.nscat_hist, sizeof res.nscat_hist);
     if (counters) std::memcpy(counters, res.counters, sizeof res.counters);
     if (cube && !res.cube.empty()) std::memcpy(cube, res.cube.data(), res.cube.size() * 8);
+    if (raw) std::memcpy(raw, res.raw.data(), res.raw.size() * sizeof(RawRecord));
+    return std::chrono::duration<double>(t1 - t0).count();
+}
+
+// The same walk through a gridless dataset (gridless.hpp; PAPER.md 3.3): geometry 0 = shell / sphere, 1 = slab.
+double orc_run_gridless(int geometry, double r_in, double r_out, double length_cm, double n0, double alpha_rho, double T,
+                        double v_max, double alpha_v, double kdust0, double step_f,
+                        int64_t n_src, const float* src_pos, const float* src_lum, const float* src_sigma,
+                        const orc_opts_c* oc, uint64_t n_photons, uint64_t seed,
+                        uint64_t* spectrum, uint64_t* nscat_hist, uint64_t* counters, void* raw) {
+    Gridless d{geometry, r_in, r_out, length_cm, n0, alpha_rho, T, v_max, alpha_v, kdust0, step_f};
+    Sources s{n_src, src_pos, src_lum, src_sigma, {}};
+    Opts o;
+    o.phase_core = oc->phase_core; o.phase_wing = oc->phase_wing; o.phase_frame = oc->phase_frame;
+    o.phase_split_x = oc->phase_split_x; o.core_skip_mode = oc->core_skip_mode; o.x_crit = oc->x_crit;
+    o.spec_mode = oc->spec_mode; o.spec_T_ref = oc->spec_T_ref; o.spec_bins = oc->spec_bins;
+    o.spec_lo = oc->spec_lo; o.spec_hi = oc->spec_hi; o.v_max_kms = oc->v_max_kms;
+    o.photon_id_offset = oc->photon_id_offset; o.max_scatter = oc->max_scatter; o.max_crossings = oc->max_crossings;
+    GridlessWalker w(d, s, o);
+    Result res;
+    const auto t0 = std::chrono::steady_clock::now();
+    w.run(n_photons, seed, res, raw != nullptr);
+    const auto t1 = std::chrono::steady_clock::now();
+    if (spectrum) std::memcpy(spectrum, res.spectrum.data(), res.spectrum.size() * 8);
+    if (nscat_hist) std::memcpy(nscat_hist, res.nscat_hist, sizeof res.nscat_hist);
+    if (counters) std::memcpy(counters, res.counters, sizeof res.counters);
     if (raw) std::memcpy(raw, res.raw.data(), res.raw.size() * sizeof(RawRecord));
     return std::chrono::duration<double>(t1 - t0).count();
 }

@@ -11,7 +11,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "liboracle.so")
-_SOURCES = ["capi.cpp", "walker.hpp", "dda.hpp", "sampler.hpp", "voigt.hpp", "philox.hpp", "constants.hpp"]
+_SOURCES = ["capi.cpp", "walker.hpp", "gridless.hpp", "dda.hpp", "sampler.hpp", "voigt.hpp", "philox.hpp", "constants.hpp"]
 
 
 def build(force=False):
@@ -89,6 +89,8 @@ def lib():
         L.orc_raytrace.argtypes = [i32, i32, i32, d] + [P] * 6 + [i64, P, P, d, i32, d, d, P, P, P]
         L.orc_volume_render.restype = None
         L.orc_volume_render.argtypes = [i32, i32, i32, P, P, i64, P, P, i32, P, d, P]
+        L.orc_run_gridless.restype = d
+        L.orc_run_gridless.argtypes = [i32] + [d] * 10 + [i64, P, P, P, P, u64, u64] + [P] * 4
         L.orc_run.restype = d
         L.orc_run.argtypes = [i32] * 6 + [d] + [P] * 6 + [i64, P, P, P, P, u64, u64] + [P] * 5
         _lib = L
@@ -215,6 +217,50 @@ def run(grid, sources, opts, n_photons, seed, want_raw=True):
                          _ptr(spectrum), _ptr(hist), _ptr(counters), _ptr(cube), _ptr(raw))
     return dict(spectrum=spectrum, nscat_hist=hist, counters=dict(zip(COUNTER_NAMES, (int(c) for c in counters))),
                 cube=cube, raw=raw, seconds=secs)
+
+
+GRIDLESS_DEFAULTS = dict(geometry=0, r_in=0.0, r_out=1.0, length_cm=1.0, n0=0.0, alpha_rho=0.0, T=1e4, v_max=0.0, alpha_v=1.0,
+                         kdust0=0.0, step_f=0.01)
+
+
+def _opts_struct(opts):
+    o = dict(OPT_DEFAULTS)
+    unknown = set(opts) - set(o)
+    if unknown:
+        raise KeyError(f"unknown opts: {unknown}")
+    o.update(opts)
+    oc = _Opts()
+    for k, v in o.items():
+        if k == "k_obs":
+            oc.k_obs = (C.c_double * 3)(*v)
+        else:
+            setattr(oc, k, v)
+    return o, oc
+
+
+def run_gridless(dataset, sources, opts, n_photons, seed, want_raw=True):
+    """The walk through a gridless dataset (oracle/gridless.hpp).  dataset: dict over GRIDLESS_DEFAULTS (geometry 0 = shell /
+    sphere, 1 = slab; lengths in the dataset's unit of length_cm centimetres); sources: pos in that unit, relative to the
+    centre / midplane."""
+    dd = dict(GRIDLESS_DEFAULTS)
+    unknown = set(dataset) - set(dd)
+    if unknown:
+        raise KeyError(f"unknown gridless fields: {unknown}")
+    dd.update(dataset)
+    pos = np.ascontiguousarray(sources["pos"], np.float32).reshape(-1, 3)
+    lum = np.ascontiguousarray(sources["lum"], np.float32)
+    sig = np.ascontiguousarray(sources["sigma"], np.float32)
+    o, oc = _opts_struct(opts)
+    spectrum = np.zeros(o["spec_bins"] + 2, np.uint64)
+    hist = np.zeros(64, np.uint64)
+    counters = np.zeros(9, np.uint64)
+    raw = np.zeros(n_photons, RAW_DTYPE) if want_raw else None
+    secs = lib().orc_run_gridless(int(dd["geometry"]), *(float(dd[k]) for k in ("r_in", "r_out", "length_cm", "n0", "alpha_rho", "T",
+                                                                                  "v_max", "alpha_v", "kdust0", "step_f")),
+                                  pos.shape[0], _ptr(pos), _ptr(lum), _ptr(sig), C.addressof(oc), int(n_photons), int(seed),
+                                  _ptr(spectrum), _ptr(hist), _ptr(counters), _ptr(raw))
+    return dict(spectrum=spectrum, nscat_hist=hist, counters=dict(zip(COUNTER_NAMES, (int(c) for c in counters))),
+                raw=raw, seconds=secs)
 
 
 def raytrace(grid, origins, dirs, n_v=0, v_lo=0.0, v_hi=1.0, hubble_kms_per_cell=0.0):

@@ -36,6 +36,8 @@ struct thor_ctx {
     float* owned[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     float4* d_packed = nullptr;                 // THOR_GRID_PACK: the library's own one-sector-per-cell copy
     bool has_dust = false;
+    bool l2_persist = false;
+    size_t l2_window_max = 0;
     // sources
     long long n_src = 0;
     float* d_src_pos = nullptr;
@@ -108,6 +110,11 @@ extern "C" void thor_grid_destroy(thor_ctx* ctx) {
     if (ctx->d_cube) cudaFree(ctx->d_cube);
     if (ctx->d_raw) cudaFree(ctx->d_raw);
     if (ctx->d_pool) cudaFree(ctx->d_pool);
+    if (ctx->l2_persist) {                        // drop the access-policy window of the caller's stream
+        cudaStreamAttrValue av{};
+        cudaStreamSetAttribute(ctx->stream, cudaStreamAttributeAccessPolicyWindow, &av);
+        cudaCtxResetPersistingL2Cache();
+    }
     if (ctx->ev0) cudaEventDestroy(ctx->ev0);
     if (ctx->ev1) cudaEventDestroy(ctx->ev1);
     delete ctx;
@@ -186,6 +193,12 @@ extern "C" thor_status thor_grid_create(thor_ctx** out, int nx, int ny, int nz, 
         CU(cudaStreamSynchronize(ctx->stream));
     }
     ctx->has_dust = kdust != nullptr;
+    if (flags & THOR_GRID_L2_FETCH32) CU(cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, 32));
+    if ((flags & THOR_GRID_L2_PERSIST) && (flags & THOR_GRID_PACK) && prop.persistingL2CacheMaxSize > 0) {
+        CU(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)prop.persistingL2CacheMaxSize));
+        ctx->l2_persist = true;
+        ctx->l2_window_max = (size_t)prop.accessPolicyMaxWindowSize;
+    }
     if (flags & THOR_GRID_PACK) {
         CU(cudaMalloc(&ctx->d_packed, (size_t)ctx->n_cells * 2 * sizeof(float4)));
         CU(thor::launch_pack_fields(ctx->f[0], ctx->f[1], ctx->f[2], ctx->f[3], ctx->f[4], ctx->f[5], ctx->n_cells,
@@ -234,6 +247,36 @@ extern "C" thor_status thor_sources_set(thor_ctx* ctx, long long n_src, const fl
     CU(cudaMemcpyAsync(ctx->d_src_cdf, cdf.data(), (size_t)n_src * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     ctx->n_src = n_src;
+    if (ctx->l2_persist && ctx->d_packed) {
+        // L2-persistence window (BASELINE.json north_star): the run of z-slabs of the packed grid, as long as the device's
+        // window allows, that holds the most source luminosity — where packets are emitted and scatter first
+        const size_t slab_bytes = (size_t)ctx->g.nx * ctx->g.ny * 2 * sizeof(float4);
+        const size_t total = slab_bytes * (size_t)ctx->g.nz;
+        long long S = (long long)(ctx->l2_window_max / slab_bytes);
+        if (S > ctx->g.nz) S = ctx->g.nz;
+        if (S >= 1) {
+            std::vector<double> mass((size_t)ctx->g.nz, 0.0);
+            for (long long i = 0; i < n_src; ++i) {
+                int z = (int)pos_xyz[3 * i + 2];
+                if (z >= ctx->g.nz) z = ctx->g.nz - 1;
+                mass[(size_t)z] += lum[i];
+            }
+            double best = -1, run = 0;
+            long long z0 = 0;
+            for (long long z = 0; z < ctx->g.nz; ++z) {
+                run += mass[(size_t)z];
+                if (z >= S) run -= mass[(size_t)(z - S)];
+                if (z >= S - 1 && run > best) { best = run; z0 = z - S + 1; }
+            }
+            cudaStreamAttrValue av{};
+            av.accessPolicyWindow.base_ptr = reinterpret_cast<char*>(ctx->d_packed) + (size_t)z0 * slab_bytes;
+            av.accessPolicyWindow.num_bytes = (size_t)S * slab_bytes < total ? (size_t)S * slab_bytes : total;
+            av.accessPolicyWindow.hitRatio = 1.0f;
+            av.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+            av.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+            CU(cudaStreamSetAttribute(ctx->stream, cudaStreamAttributeAccessPolicyWindow, &av));
+        }
+    }
     return THOR_OK;
 }
 
@@ -296,7 +339,10 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
         for (int i = 0; i < 3; ++i) { i1[i] = h[i] - hk * k[i]; m2 += i1[i] * i1[i]; }
         for (int i = 0; i < 3; ++i) i1[i] /= std::sqrt(m2);
         i2[0] = k[1] * i1[2] - k[2] * i1[1]; i2[1] = k[2] * i1[0] - k[0] * i1[2]; i2[2] = k[0] * i1[1] - k[1] * i1[0];
-        for (int i = 0; i < 3; ++i) { p.kobs[i] = (float)k[i]; p.img1[i] = (float)i1[i]; p.img2[i] = (float)i2[i]; }
+        for (int i = 0; i < 3; ++i) {
+            p.kobs[i] = (float)k[i]; p.img1[i] = (float)i1[i]; p.img2[i] = (float)i2[i];
+            p.kobs_inv[i] = 1.0f / p.kobs[i];             // what __fdiv_rn(1, k) gives on the device
+        }
         p.peel_nx = o.peel_nx; p.peel_ny = o.peel_ny; p.peel_nv = o.peel_nv;
         p.peel_v_lo = (float)o.peel_v_lo;
         p.peel_inv_dv = (float)(o.peel_nv / (o.peel_v_hi - o.peel_v_lo));

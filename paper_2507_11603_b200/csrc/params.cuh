@@ -71,7 +71,7 @@ struct WalkParams {
     float spec_lo, spec_inv_width;       // bin = floor((val - lo) * inv_width), inv_width = bins / (hi - lo)
     float hubble, hubble_eps, v_max;
     int peel_on;
-    float kobs[3], img1[3], img2[3];
+    float kobs[3], kobs_inv[3], img1[3], img2[3];   // kobs_inv = 1 / kobs (IEEE single-precision quotients; +-inf for 0)
     int peel_nx, peel_ny, peel_nv;
     float peel_v_lo, peel_inv_dv;        // iv = floor((dv - lo) * inv_dv)
     float peel_inv_width;                // 1 / peel_width_cells

@@ -41,7 +41,7 @@ struct UparEnvelope {
 };
 
 #ifndef THOR_UPAR_X_LORENTZ
-#define THOR_UPAR_X_LORENTZ 0.3f
+#define THOR_UPAR_X_LORENTZ 0.7f
 #endif
 constexpr float UPAR_X_LORENTZ = THOR_UPAR_X_LORENTZ;   // below this a plain Lorentzian proposal accepts with H(a,x) >= e^{-x^2}
 constexpr float UPAR_U_MIN = -4.5f;       // left end of piece A (see below)

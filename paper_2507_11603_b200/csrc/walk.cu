@@ -31,7 +31,6 @@ constexpr int REFILL_MIN_LANES = THOR_REFILL_MIN_LANES;
 #define THOR_COOP_MAX_LANES 4
 #endif
 constexpr int COOP_MAX_LANES = THOR_COOP_MAX_LANES;     // cooperative drain when a warp has at most this many packets left
-constexpr int WALK_WARPS = WALK_THREADS / 32;
 constexpr int WIN_STRIDE = 20;                          // floats per window slot (16 used; 80 B keeps STS.128 conflict-free)
 constexpr int PK_WORDS = 48;                            // 32-bit words of a parked packet
 
@@ -118,7 +117,8 @@ __device__ __forceinline__ int park_load(const uint32_t* w, Packet& k) {
 //   q1 = (sin, cos of pi u.y; -ln u.x; dipole_mu(u.y))  trial: Lorentzian angle when psi0 = 0 | first FINISH block: tau', mu
 //   q2 = (sin, cos of 2 pi u.z; -ln u.w; 0)             first FINISH block: azimuth of k', |u_perp|^2
 //   q3 = (sin, cos of 2 pi u.x; 0; 0)                   second FINISH block: angle of u_perp
-__device__ __forceinline__ void coop_fill_window(float4* win, const BlockRng& rng, uint32_t k0, uint32_t k1, unsigned lane) {
+__device__ __forceinline__ void coop_fill_window(float4* win, const BlockRng& rng, uint32_t k0, uint32_t k1, unsigned lane,
+                                                 float4& my_u, float& my_sC, float& my_cC) {
     const uint32_t lo = rng.b_lo + lane, hi = rng.b_hi + (lo < rng.b_lo ? 1u : 0u);
     const U4 r = philox4x32_10(lo, hi, rng.id_lo, rng.id_hi, k0, k1);
     const float4 u = make_float4(u01(r.x), u01(r.y), u01(r.z), u01(r.w));
@@ -132,6 +132,7 @@ __device__ __forceinline__ void coop_fill_window(float4* win, const BlockRng& rn
     q3.z = 0.f; q3.w = 0.f;
     float4* slot = win + 5 * lane;
     slot[0] = u; slot[1] = q1; slot[2] = q2; slot[3] = q3;
+    my_u = u; my_sC = q1.x; my_cC = q1.y;
 }
 
 // The drain kernel: launched behind walk_kernel on the same stream.  Each warp pops one parked packet at a time from the
@@ -159,7 +160,9 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
         slot = __shfl_sync(0xffffffffu, slot, 0);
         if (slot >= n_pool) break;
         int st = park_load(p.pool + slot * PK_WORDS, k);      // every lane reads the same words: one broadcast per load
-        int c = 32;                                           // blocks of the window already consumed (32 = none left)
+        int c = 32;                                           // first unconsumed block of the window (32 = none left)
+        float4 my_u = make_float4(0.f, 0.f, 0.f, 0.f);        // this lane's own block of the window
+        float my_sC = 0.f, my_cC = 0.f;
         UparEnvelope env;
         env.mTot = -1.f;
         for (;;) {
@@ -172,21 +175,39 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
             }
             if (c + 3 > 32) {                                 // fewer than a trial + a FINISH left: a new window
                 __syncwarp();
-                coop_fill_window(win, k.rng, k0, k1, lane);
+                coop_fill_window(win, k.rng, k0, k1, lane, my_u, my_sC, my_cC);
                 __syncwarp();
                 c = 0;
             }
             if (st == LS_TRIAL) {
+                // every lane tries its OWN block; the packet takes the first acceptance at or after block c — exactly the
+                // trial the sequential rejection loop would have accepted, found in one step however many it rejects
                 if (env.mTot < 0.f) env = upar_envelope(k.cell.a, fabsf(k.x_in));
-                const float4 u = win[5 * c], q1 = win[5 * c + 1];
-                ++c;
-                k.rng.b_lo += 1u; k.rng.b_hi += (k.rng.b_lo == 0u);
-                ++k.rej_iters;
                 float uu;
-                const bool ok = upar_try<true>(env, k.cell.a, u, q1.x, q1.y, uu);
-                if (!(ok || ++k.trials >= (1u << 20))) continue;
+                const bool ok = upar_try<true>(env, k.cell.a, my_u, my_sC, my_cC, uu);
+                const unsigned acc = __ballot_sync(0xffffffffu, ok) & ~((1u << c) - 1u);
+                const uint32_t nrej = (uint32_t)((acc ? __ffs(acc) - 1 : 32) - c);   // rejections before the first acceptance
+                uint32_t ntr;                                 // blocks this step consumes
+                bool done_trial;
+                if (k.trials + nrej >= (1u << 20)) {          // fail-safe of the sequential loop: its 2^20-th rejection is taken
+                    ntr = (1u << 20) - k.trials;
+                    k.trials = 1u << 20;
+                    done_trial = true;
+                } else {
+                    k.trials += nrej;
+                    done_trial = acc != 0u;
+                    ntr = nrej + (done_trial ? 1u : 0u);
+                }
+                const int jj = c + (int)ntr - 1;              // the block whose u is taken, if any
+                k.rej_iters += ntr;
+                const uint32_t lo = k.rng.b_lo;
+                k.rng.b_lo += ntr; k.rng.b_hi += (k.rng.b_lo < lo);
+                c += (int)ntr;
+                if (!done_trial) continue;                    // the whole window rejected: refill, keep trying
+                uu = __shfl_sync(0xffffffffu, uu, jj);
                 k.upar = k.x_in < 0.f ? -uu : uu;
                 st = LS_FINISH;
+                if (c + 2 > 32) continue;                     // FINISH needs two more blocks: refill first
             }
             {   // LS_FINISH: blocks c, c + 1
                 const float4 u1 = win[5 * c], a1 = win[5 * c + 1], a2 = win[5 * c + 2];
@@ -257,7 +278,7 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
                     emit_packet(p, k, p.id_offset + i, k0, k1, dV);
                     if (PEEL) {
                         ++peel_rays;
-                        peel_ray<HUBBLE>(p, sh.voigt, k.ray,
+                        peel_ray<HUBBLE>(p, sh.voigt, k.ray, k.cell,
                                          dot3(k.cell.vx, k.cell.vy, k.cell.vz, p.kobs[0], p.kobs[1], p.kobs[2]) + dV, 1.f,
                                          peel_cells, true);
                     }

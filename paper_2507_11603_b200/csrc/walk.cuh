@@ -123,8 +123,8 @@ __device__ __forceinline__ float cell_opacity(const float2* s_tab, const Cell& c
 // (pixel of the starting point projected perpendicular to k_obs, spectral bin of dv = -V at the box face).  `add` is
 // false on the lanes that only shadow a packet in the cooperative drain (one lane tallies).
 template <bool HUBBLE>
-__device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, const Ray& at, float V_o, float phat,
-                                      uint32_t& n_cells, bool add) {
+__device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, const Ray& at, const Cell& own, float V_o,
+                                      float phat, uint32_t& n_cells, bool add) {
     const float px0 = (float)at.cx + at.fx - 0.5f * (float)p.g.nx;
     const float py0 = (float)at.cy + at.fy - 0.5f * (float)p.g.ny;
     const float pz0 = (float)at.cz + at.fz - 0.5f * (float)p.g.nz;
@@ -132,13 +132,17 @@ __device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, 
     const float py = fmaf(dot3(px0, py0, pz0, p.img2[0], p.img2[1], p.img2[2]), p.peel_inv_width, 0.5f) * (float)p.peel_ny;
     if (!(px >= 0.f && px < (float)p.peel_nx && py >= 0.f && py < (float)p.peel_ny)) return;
     Ray r = at;
-    ray_set_direction(r, p.kobs[0], p.kobs[1], p.kobs[2]);
+    r.kx = p.kobs[0]; r.ky = p.kobs[1]; r.kz = p.kobs[2];     // 1 / k_obs: IEEE quotients made once on the host
+    r.ix = p.kobs_inv[0]; r.iy = p.kobs_inv[1]; r.iz = p.kobs_inv[2];
     float tau = 0.f, V = V_o;
+    bool first = true;
     for (;;) {
         float len;
         const int ex = dda_next_face(r, p.g, len);
         if (!(len < CUDART_INF_F)) return;                    // reading A24: never reaches a box face -> dropped
-        const Cell c = load_cell(p, dda_linear(r, p.g));
+        // the ray starts in the packet's own cell, whose derived properties the packet already holds (most rays end there)
+        const Cell c = first ? own : load_cell(p, dda_linear(r, p.g));
+        first = false;
         const float vk = dot3(c.vx, c.vy, c.vz, r.kx, r.ky, r.kz);
         float dtau, s_hit, kt;
         integrate_segment<HUBBLE>(p, s_tab, c, V, vk, len, 3.0e38f, dtau, s_hit, kt);
@@ -311,7 +315,7 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
         const float V_o = fmaf(x_o, c.vth, dot3(c.vx, c.vy, c.vz, p.kobs[0], p.kobs[1], p.kobs[2]));
         ++peel_rays;
         // mix: the sampled branch weights the ray (unbiased; reading A27)
-        peel_ray<HUBBLE>(p, s_tab, k.ray, V_o, is_dipole ? 0.75f * fmaf(mu_o, mu_o, 1.f) : 1.f, peel_cells, add);
+        peel_ray<HUBBLE>(p, s_tab, k.ray, c, V_o, is_dipole ? 0.75f * fmaf(mu_o, mu_o, 1.f) : 1.f, peel_cells, add);
     }
     const float st = sqrtf(fmaxf(0.f, fmaf(-mu, mu, 1.f)));
     float nx = fmaf(st, fmaf(d.cphi, e1[0], d.sphi * e2[0]), mu * kx);

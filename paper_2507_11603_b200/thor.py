@@ -13,6 +13,7 @@ LIB_PATH = os.path.join(_HERE, "libthor_b200.so")
 STATUS = {0: "THOR_OK", 1: "THOR_ERR_ARG", 2: "THOR_ERR_STATE", 3: "THOR_ERR_OOM", 4: "THOR_ERR_CUDA",
           5: "THOR_ERR_UNSUPPORTED"}
 GRID_HOST, PERIODIC_X, PERIODIC_Y, PERIODIC_Z, GRID_NO_VALIDATE, GRID_PACK = 0x1, 0x10, 0x20, 0x40, 0x100, 0x200
+GRID_L2_PERSIST, GRID_L2_FETCH32 = 0x400, 0x800
 TALLY_SPECTRUM, TALLY_NSCAT_HIST, TALLY_COUNTERS, TALLY_CUBE, TALLY_RAW, TALLY_DEVICE_DST = 0, 1, 2, 3, 4, 0x100
 COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "cell_crossings", "rejection_iters",
                  "peel_rays", "peel_cells"]
@@ -116,10 +117,10 @@ class Context:
     kept referenced here) or numpy float32 arrays (host=True: copied to the device by the library)."""
 
     def __init__(self, nx, ny, nz, cell_cm, nHI, T, vx, vy, vz, kdust=None, periodic=(0, 0, 0), host=False,
-                 validate=True, pack=False):
+                 validate=True, pack=False, extra_flags=0):
         self._ctx = C.c_void_p()
         fields = [nHI, T, vx, vy, vz, kdust]
-        flags = _periodic_flags(periodic) | (0 if validate else GRID_NO_VALIDATE) | (GRID_PACK if pack else 0)
+        flags = _periodic_flags(periodic) | (0 if validate else GRID_NO_VALIDATE) | (GRID_PACK if pack else 0) | int(extra_flags)
         if host:
             self._keep = [None if a is None else np.ascontiguousarray(a, np.float32) for a in fields]
             ptrs = [None if a is None else a.ctypes.data_as(C.c_void_p) for a in self._keep]
@@ -145,7 +146,7 @@ class Context:
             self._keep = None              # THOR_GRID_PACK: the library holds its own copy; release ours
 
     @classmethod
-    def from_workload(cls, grid, host=False, device="cuda", pack=False):
+    def from_workload(cls, grid, host=False, device="cuda", pack=False, extra_flags=0):
         """grid: the dict made by paper_2507_11603_b200.workloads (numpy float32 fields) or .workloads_device (CUDA
         tensors, borrowed as they are)."""
         keys = ("nHI", "T", "vx", "vy", "vz", "kdust")
@@ -157,7 +158,7 @@ class Context:
                     (grid[k] if isinstance(grid[k], torch.Tensor) else
                      torch.from_numpy(np.ascontiguousarray(grid[k], np.float32)).to(device)) for k in keys]
         return cls(grid["nx"], grid["ny"], grid["nz"], grid["cell_cm"], *arrs,
-                   periodic=grid.get("periodic", (0, 0, 0)), host=host, pack=pack)
+                   periodic=grid.get("periodic", (0, 0, 0)), host=host, pack=pack, extra_flags=extra_flags)
 
     def close(self):
         if getattr(self, "_ctx", None) and self._ctx.value:

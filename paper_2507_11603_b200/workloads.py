@@ -151,7 +151,8 @@ def cosmic_web(n=64, n_src=4096, n_photons=10_000, seed=11, mean_n=1e-6, sigma_l
                cell_kpc=11.2, hubble_kms_per_mpc=203.6, map_pix=128, bins=1000, v_max=1233.0):
     """Config 5 at size n (1536 in BASELINE.json): lognormal overdensity (sigma_ln 1.5) on mean n_HI = 1e-6,
     T = 1e4 (1+delta)^0.6, Hubble flow as a frequency drift plus Gaussian peculiar velocities (3-D dispersion
-    100 km/s, k^-4), sources ∝ (1+delta)^2, stop at |V| > v_max (5 Å), surface-brightness map by peel-off along +z."""
+    100 km/s, k^-4), sources ∝ (1+delta)^2, stop at |V| > v_max (5 Å), surface-brightness map by peel-off along +z,
+    local core-skipping as in the paper's simulation runs (reading A28)."""
     rng = np.random.default_rng(seed)
     g = _gaussian_field(rng, n, -3.0)
     opd = np.exp(-0.5 * sigma_ln ** 2 + sigma_ln * g)              # 1 + delta, mean 1
@@ -168,7 +169,7 @@ def cosmic_web(n=64, n_src=4096, n_photons=10_000, seed=11, mean_n=1e-6, sigma_l
     hc = hubble_kms_per_mpc * cell_kpc * 1e-3
     grid = dict(nx=n, ny=n, nz=n, periodic=(0, 0, 0), cell_cm=cell_cm, nHI=nHI, T=T, vx=vx, vy=vy, vz=vz, kdust=None)
     src = dict(pos=pos.astype(np.float32), lum=np.ones(n_src, np.float32), sigma=np.zeros(n_src, np.float32))
-    opts = dict(phase_core=0, phase_wing=0, spec_mode=1, spec_bins=bins, spec_lo=-v_max, spec_hi=v_max,
+    opts = dict(phase_core=0, phase_wing=0, core_skip_mode=2, spec_mode=1, spec_bins=bins, spec_lo=-v_max, spec_hi=v_max,
                 hubble_kms_per_cell=float(np.float32(hc)), hubble_eps=0.25, v_max_kms=v_max,
                 peel_on=1, k_obs=(0.0, 0.0, 1.0), peel_nx=map_pix, peel_ny=map_pix, peel_nv=1,
                 peel_v_lo=-1e30, peel_v_hi=1e30, peel_width_cells=float(n), tau_peel_max=30.0)

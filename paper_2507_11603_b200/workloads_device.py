@@ -104,7 +104,7 @@ def cosmic_web(n=1536, n_src=1 << 22, n_photons=100_000_000, seed=11, mean_n=1e-
     hc = hubble_kms_per_mpc * cell_kpc * 1e-3
     grid = dict(nx=n, ny=n, nz=n, periodic=(0, 0, 0), cell_cm=cell_cm, nHI=nHI, T=T, vx=vx, vy=vy, vz=vz, kdust=None)
     src = dict(pos=pos, lum=np.ones(n_src, np.float32), sigma=np.zeros(n_src, np.float32))
-    opts = dict(phase_core=0, phase_wing=0, spec_mode=1, spec_bins=bins, spec_lo=-v_max, spec_hi=v_max,
+    opts = dict(phase_core=0, phase_wing=0, core_skip_mode=2, spec_mode=1, spec_bins=bins, spec_lo=-v_max, spec_hi=v_max,
                 hubble_kms_per_cell=float(np.float32(hc)), hubble_eps=0.25, v_max_kms=v_max,
                 peel_on=1, k_obs=(0.0, 0.0, 1.0), peel_nx=map_pix, peel_ny=map_pix, peel_nv=1,
                 peel_v_lo=-1e30, peel_v_hi=1e30, peel_width_cells=float(n), tau_peel_max=30.0)

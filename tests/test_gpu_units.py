@@ -155,29 +155,29 @@ def test_single_scatter_against_oracle(thor, oracle, a, x_in, x_crit, phase):
 
 
 def test_dda_linear_index_beyond_2_31(thor, oracle):
-    """a4 with 64-bit cell indices (BASELINE.json config 5 has 3.6e9 cells): 1e5 random rays through a VIRTUAL
-    2049 x 1024 x 1024 grid (2.15e9 cells; the trace reads no field) — hashes of the 64-bit linear indices and of the
-    fp32 segment lengths equal the oracle's."""
-    dims = (2049, 1024, 1024)
-    org, dirs = W.random_rays(100_000, dims, seed=17)
-    g = thor.unit_dda_trace(dims, (0, 0, 0), org, dirs, max_steps=1 << 14)
-    o = oracle.dda_trace(dims, (0, 0, 0), org, dirs, max_steps=1 << 14)
-    assert np.array_equal(g["count"], o["count"])
-    assert np.array_equal(g["hash_idx"], o["hash_idx"]) and np.array_equal(g["hash_len"], o["hash_len"])
-    # the grid really is beyond 2^31: a ray ending in the far corner visits indices above it
-    far = thor.unit_dda_trace(dims, (0, 0, 0), np.array([[2040.5, 1020.5, 1020.5]], np.float32),
+    """a4 with 64-bit cell indices (BASELINE.json config 5 has 3.6e9 cells): random rays through VIRTUAL grids of 2.15e9
+    and 4.3e9 cells (the trace reads no field; the second is beyond 2^32 as well) — hashes of the 64-bit linear indices
+    and of the fp32 segment lengths equal the oracle's."""
+    for dims, n_rays in (((2049, 1024, 1024), 60_000), ((1024, 1024, 4100), 40_000)):
+        org, dirs = W.random_rays(n_rays, dims, seed=17)
+        g = thor.unit_dda_trace(dims, (0, 0, 0), org, dirs, max_steps=1 << 14)
+        o = oracle.dda_trace(dims, (0, 0, 0), org, dirs, max_steps=1 << 14)
+        assert np.array_equal(g["count"], o["count"])
+        assert np.array_equal(g["hash_idx"], o["hash_idx"]) and np.array_equal(g["hash_len"], o["hash_len"])
+    # the grid really is beyond 2^32: a ray in the top slabs visits indices above it
+    far = thor.unit_dda_trace((1024, 1024, 4100), (0, 0, 0), np.array([[1000.5, 1000.5, 4097.5]], np.float32),
                               np.array([[0.6, 0.0, 0.8]], np.float32), max_steps=64, want_seq=True)
-    assert far["seq_idx"].max() > 2 ** 31
+    assert far["seq_idx"].min() > 2 ** 32
 
 
 def test_gathers_beyond_2_31_on_a_borrowed_grid(thor):
-    """A borrowed 2049 x 1024 x 1024 grid whose five field pointers alias ONE 8.6 GB device buffer holding an
-    index-dependent pattern: (i) thor_raytrace's column density along rays through cells above 2^31 equals
-    sum(buffer[idx] * len) over the index / length sequence of the DDA unit trace (itself pinned to the oracle above);
-    (ii) the walk emits from source cells above 2^31 with V = v_cell . k = buffer[idx] (kx + ky + kz) and crosses exactly
-    the cells the DDA counts."""
+    """A borrowed 1024 x 1024 x 2304 grid (2.4e9 cells) whose five field pointers alias ONE 9.7 GB device buffer holding an
+    index-dependent pattern; everything below happens in the slabs z >= 2048, whose linear indices exceed 2^31:
+    (i) thor_raytrace's column density equals sum(buffer[idx] * len) over the index / length sequence of the DDA unit
+    trace (itself pinned to the oracle above); (ii) the walk emits from source cells up there with
+    V = v_cell . k = buffer[idx] (kx + ky + kz) and crosses exactly the cells the DDA counts."""
     import torch
-    nx, ny, nz = 2049, 1024, 1024
+    nx, ny, nz = 1024, 1024, 2304
     N = nx * ny * nz
     buf = torch.empty(N, dtype=torch.float32, device="cuda")
     step = 1 << 27
@@ -187,18 +187,18 @@ def test_gathers_beyond_2_31_on_a_borrowed_grid(thor):
     f = buf.view(nz, ny, nx)
     ctx = thor.Context(nx, ny, nz, 1.0, f, f, f, f, f, None, validate=False)     # cell_cm = 1 cm: transparent
     try:
-        org = np.array([[2040.5, 1020.5, 1010.25], [1500.25, 900.5, 1000.75], [2048.5, 1023.5, 1023.5]], np.float32)
+        org = np.array([[1000.5, 1020.5, 2100.25], [500.25, 900.5, 2200.75], [1023.5, 1023.5, 2303.5]], np.float32)
         dirs = np.array([[0.6, 0.0, 0.8], [0.48, 0.6, 0.64], [-0.8, -0.6, 0.0]], np.float32)
         col = ctx.raytrace(org, dirs)["column"]
         for j in range(3):
             t = thor.unit_dda_trace((nx, ny, nz), (0, 0, 0), org[j:j + 1], dirs[j:j + 1], max_steps=4096, want_seq=True)
             idx = torch.from_numpy(t["seq_idx"]).cuda()
-            assert int(idx.max()) > 2 ** 31
+            assert int(idx.min()) > 2 ** 31
             vals = buf[idx].double().cpu().numpy()
             expect = float((vals * t["seq_len"].astype(np.float64)).sum())
             assert abs(col[j] - expect) <= 2e-5 * expect, (j, col[j], expect)
         n = 2000
-        src = np.array([[2040.5, 1020.5, 1010.25], [2047.5, 1000.5, 1023.5]], np.float32)
+        src = np.array([[1000.5, 1020.5, 2100.25], [1020.5, 700.5, 2290.5]], np.float32)
         ctx.sources_set(src, np.ones(2, np.float32), np.zeros(2, np.float32))
         ctx.run(n, 5, dict(spec_mode=1, spec_bins=10, spec_lo=-1e4, spec_hi=1e4, raw_output=1))
         raw, c = ctx.raw(), ctx.counters()
