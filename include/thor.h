@@ -61,6 +61,34 @@ thor_status thor_grid_create(thor_ctx **out, int nx, int ny, int nz, double cell
                              const float *kdust, unsigned flags, void *stream);
 void thor_grid_destroy(thor_ctx *ctx);
 
+/* The paper's GRIDLESS datasets (PAPER.md 3.3; power laws PAPER.md:380; step limiter PAPER.md:382):
+ * nothing is voxelised, boundaries are the analytic sphere(s) / planes.  Lengths are in the dataset's own unit of
+ * length_cm centimetres, relative to the centre (shell) or the midplane (slab).
+ *   THOR_GEOM_SHELL: gas in r_in <= r <= r_out (r_in = 0: a sphere), n_HI(r) = n0 (r/r_out)^alpha_rho [cm^-3],
+ *                    v(r) = v_max (r/r_out)^alpha_v radially outward [km/s], dust absorption kdust0 (r/r_out)^alpha_rho
+ *                    [cm^-1]; the cavity and the outside are empty; a packet ends when it leaves r_out.
+ *   THOR_GEOM_SLAB:  gas in |z| <= r_out, n_HI = n0, v_z = v_max z / r_out, dust kdust0; infinite in x and y.
+ * T [K] is uniform.  step_f: no step is longer than step_f * min(v_th / max|dv/dr|, max[rho / |d rho/dr|]) (0.01 in the
+ * paper; 0 = no limiter; a static homogeneous medium has none anyway); the gas of a step is that of its midpoint and the
+ * interaction site is linear within it (readings A29-A31).  The context then works with thor_sources_set
+ * (positions in length units, inside r_out), thor_run and thor_tally_get as a grid context does; thor_run refuses
+ * peel-off, Hubble drift and local core-skipping on it (THOR_ERR_UNSUPPORTED); the ray operators need a grid.
+ * THOR_ERR_ARG for a bad geometry, r_out <= r_in, T <= 0, negative n0 / kdust0, non-finite values. */
+#define THOR_GEOM_SHELL 0
+#define THOR_GEOM_SLAB 1
+typedef struct thor_gridless {
+    uint32_t struct_size;     /* = sizeof(thor_gridless) */
+    int32_t geometry;         /* THOR_GEOM_* */
+    double r_in, r_out;       /* length units; slab: r_out = half thickness, r_in ignored */
+    double length_cm;
+    double n0, alpha_rho;
+    double T;
+    double v_max, alpha_v;
+    double kdust0;
+    double step_f;
+} thor_gridless;
+thor_status thor_dataset_create_gridless(thor_ctx **out, const thor_gridless *dataset, void *stream);
+
 /* The generator: a list of point sources.  HOST arrays, copied: pos_xyz [n_src][3] in cell units
  * (grid spans [0,nx) x [0,ny) x [0,nz)), lum [n_src] >= 0 relative luminosities (a packet picks source j with
  * probability lum_j / sum, reading A18), sigma_kms [n_src] Gaussian line width in the source cell's gas frame

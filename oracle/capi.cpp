@@ -248,6 +248,61 @@ void orc_raytrace(int nx, int ny, int nz, double cell_cm, const float* nHI, cons
     }
 }
 
+// Sight lines as the paper draws them for the Lyα forest ("periodic boundary conditions", cells sub-sampled
+// "such that each ray step corresponds to a Hubble induced velocity-shift much smaller than the line width"): the ray
+// wraps at the periodic faces given and ends after max_len cell lengths (or at the first non-periodic face; max_len <= 0:
+// first box face as orc_raytrace); with hubble_eps > 0 each face-to-face segment is cut into
+// n_sub = ceil(|Hc len| / (hubble_eps v_th(T_cell))) sub-steps (the rule of reading A12), the gas frequency evaluated at
+// each sub-step's midpoint.
+void orc_raytrace_ex(int nx, int ny, int nz, int px, int py, int pz, double cell_cm, const float* nHI, const float* T,
+                     const float* vx, const float* vy, const float* vz, const float* kdust, int64_t n_rays, const float* org,
+                     const float* dir, double hubble, double hubble_eps, double max_len, int n_v, double v_lo, double v_hi,
+                     double* out_column, double* out_tmean, double* out_tau) {
+    const bool wrap = max_len > 0;
+    Grid g{{{nx, ny, nz}, {wrap && px != 0, wrap && py != 0, wrap && pz != 0}}, cell_cm, nHI, T, vx, vy, vz, kdust};
+    for (int64_t i = 0; i < n_rays; ++i) {
+        Ray<double> r;
+        const double pos[3] = {org[3 * i], org[3 * i + 1], org[3 * i + 2]};
+        dda_locate(r, g.dims, pos);
+        const double k[3] = {dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]};
+        r.set_direction(k);
+        double col = 0, tn = 0, s_path = 0;
+        if (out_tau) for (int j = 0; j < n_v; ++j) out_tau[i * n_v + j] = 0.0;
+        for (;;) {
+            double len;
+            const int ex = dda_next_face(r, g.dims, len);
+            if (std::isinf(len) && !wrap) break;
+            bool last = false;
+            if (wrap && s_path + len >= max_len) { len = max_len - s_path; last = true; }
+            const CellProps cp = fetch_cell(g, r.c);
+            col += cp.n * len;
+            tn += cp.n * cp.T * len;
+            if (out_tau && (cp.n > 0 || cp.kd > 0) && len > 0) {
+                const double vth = vth_kms(cp.T), a = voigt_a(cp.T);
+                int nsub = 1;
+                if (hubble_eps > 0 && hubble != 0 && cp.n > 0) {
+                    const double q = std::ceil(std::fabs(hubble * len) / (hubble_eps * vth));
+                    nsub = q < 1.0 ? 1 : (q > 1e6 ? 1000000 : (int)q);
+                }
+                const double ds = len / nsub;
+                for (int m = 0; m < nsub; ++m) {
+                    const double vgas = dot3(cp.v, k) + hubble * (s_path + (m + 0.5) * ds);
+                    for (int j = 0; j < n_v; ++j) {
+                        const double V = v_lo + (j + 0.5) * (v_hi - v_lo) / n_v;
+                        const double kl = cp.n > 0 ? cp.n * sigma0_cm2(cp.T) * voigt_H(a, (V - vgas) / vth) * cell_cm : 0.0;
+                        out_tau[i * n_v + j] += (kl + cp.kd * cell_cm) * ds;
+                    }
+                }
+            }
+            s_path += len;
+            if (last) break;
+            if (!dda_cross(r, g.dims, ex, len)) break;     // left through a non-periodic face
+        }
+        if (out_column) out_column[i] = col * cell_cm;
+        if (out_tmean) out_tmean[i] = col > 0 ? tn / col : 0.0;
+    }
+}
+
 // Pins of orc_raytrace and orc_volume_render (tests/test_oracle_raytrace.py), none through this file's DDA or Voigt:
 // density x analytic chord, two-slab weighted mean, N sigma_0 H by scipy's Faddeeva function with a bulk-velocity shift,
 // Hubble-swept line against adaptive quadrature; volume rendering: c (1 - e^{-mu L}) in a uniform medium, two slabs seen

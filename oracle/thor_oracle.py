@@ -87,6 +87,8 @@ def lib():
         L.orc_dda_trace.argtypes = [i32] * 6 + [i64, P, P, i64, i32, P, P, P, P, P]
         L.orc_raytrace.restype = None
         L.orc_raytrace.argtypes = [i32, i32, i32, d] + [P] * 6 + [i64, P, P, d, i32, d, d, P, P, P]
+        L.orc_raytrace_ex.restype = None
+        L.orc_raytrace_ex.argtypes = [i32] * 6 + [d] + [P] * 6 + [i64, P, P, d, d, d, i32, d, d, P, P, P]
         L.orc_volume_render.restype = None
         L.orc_volume_render.argtypes = [i32, i32, i32, P, P, i64, P, P, i32, P, d, P]
         L.orc_run_gridless.restype = d
@@ -280,6 +282,34 @@ def raytrace(grid, origins, dirs, n_v=0, v_lo=0.0, v_hi=1.0, hubble_kms_per_cell
     if tau is not None:
         out["tau"] = tau
     return out
+
+
+def raytrace_ex(grid, origins, dirs, n_v=0, v_lo=0.0, v_hi=1.0, hubble_kms_per_cell=0.0, hubble_eps=0.25, max_length_cells=0.0):
+    """Sight lines with periodic wrap-around up to max_length_cells and Hubble sub-sampling of Eq. 11."""
+    f = lambda k: None if grid.get(k) is None else np.ascontiguousarray(grid[k], np.float32)
+    nHI, T, vx, vy, vz, kd = (f(k) for k in ("nHI", "T", "vx", "vy", "vz", "kdust"))
+    org = np.ascontiguousarray(origins, np.float32).reshape(-1, 3)
+    dr = np.ascontiguousarray(dirs, np.float32).reshape(-1, 3)
+    n = org.shape[0]
+    col = np.zeros(n, np.float64)
+    tm = np.zeros(n, np.float64)
+    tau = np.zeros((n, n_v), np.float64) if n_v > 0 else None
+    per = grid.get("periodic", (0, 0, 0))
+    lib().orc_raytrace_ex(int(grid["nx"]), int(grid["ny"]), int(grid["nz"]), int(per[0]), int(per[1]), int(per[2]),
+                          float(grid["cell_cm"]), _ptr(nHI), _ptr(T), _ptr(vx), _ptr(vy), _ptr(vz), _ptr(kd), n, _ptr(org), _ptr(dr),
+                          float(hubble_kms_per_cell), float(hubble_eps), float(max_length_cells), int(n_v), float(v_lo), float(v_hi),
+                          _ptr(col), _ptr(tm), _ptr(tau))
+    out = dict(column=col, tmean=tm)
+    if tau is not None:
+        out["tau"] = tau
+    return out
+
+
+def slice_field(grid, points, field):
+    """Slice operator: the value of `field` in the cell holding each point — by definition a plain lookup."""
+    pts = np.asarray(points, np.float64).reshape(-1, 3)
+    idx = [np.clip(np.floor(pts[:, a]).astype(np.int64), 0, grid[("nx", "ny", "nz")[a]] - 1) for a in range(3)]
+    return np.asarray(grid[field])[idx[2], idx[1], idx[0]].astype(np.float64)
 
 
 def volume_render(grid, origins, dirs, peaks, n_ref=0.0):

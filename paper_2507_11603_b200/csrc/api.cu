@@ -37,6 +37,8 @@ struct thor_ctx {
     float4* d_packed = nullptr;                 // THOR_GRID_PACK: the library's own one-sector-per-cell copy
     bool has_dust = false;
     bool l2_persist = false;
+    bool gridless = false;
+    thor_gridless gl{};
     size_t l2_window_max = 0;
     // sources
     long long n_src = 0;
@@ -214,6 +216,48 @@ extern "C" thor_status thor_grid_create(thor_ctx** out, int nx, int ny, int nz, 
     return THOR_OK;
 }
 
+extern "C" thor_status thor_dataset_create_gridless(thor_ctx** out, const thor_gridless* d, void* stream) {
+    if (!out) return fail(nullptr, THOR_ERR_ARG, "thor_dataset_create_gridless: out is NULL");
+    *out = nullptr;
+    if (!d || d->struct_size != sizeof(thor_gridless)) return fail(nullptr, THOR_ERR_ARG, "thor_dataset_create_gridless: struct_size is not set");
+    if (d->geometry != THOR_GEOM_SHELL && d->geometry != THOR_GEOM_SLAB) return fail(nullptr, THOR_ERR_ARG, "thor_dataset_create_gridless: unknown geometry");
+    const double vals[] = {d->r_in, d->r_out, d->length_cm, d->n0, d->alpha_rho, d->T, d->v_max, d->alpha_v, d->kdust0, d->step_f};
+    for (double v : vals) if (!std::isfinite(v)) return fail(nullptr, THOR_ERR_ARG, "thor_dataset_create_gridless: non-finite value");
+    const double r_in = d->geometry == THOR_GEOM_SLAB ? 0.0 : d->r_in;
+    if (!(d->r_out > 0) || !(r_in >= 0) || !(d->r_out > r_in) || !(d->length_cm > 0) || !(d->T > 0) || !(d->n0 >= 0) ||
+        !(d->kdust0 >= 0) || !(d->step_f >= 0))
+        return fail(nullptr, THOR_ERR_ARG, "thor_dataset_create_gridless: need r_out > r_in >= 0, length_cm > 0, T > 0, n0 >= 0, kdust0 >= 0, step_f >= 0");
+    if (d->geometry == THOR_GEOM_SHELL && r_in == 0.0 && (d->alpha_rho < 0 || (d->alpha_v < 0 && d->v_max != 0)))
+        return fail(nullptr, THOR_ERR_ARG, "thor_dataset_create_gridless: a negative power law needs r_in > 0");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, THOR_ERR_UNSUPPORTED, "thor_dataset_create_gridless: no CUDA device (this library has no CPU fallback)");
+    }
+    thor_ctx* ctx = new (std::nothrow) thor_ctx;
+    if (!ctx) return fail(nullptr, THOR_ERR_OOM, "thor_dataset_create_gridless: host allocation failed");
+    struct Guard { thor_ctx* c; ~Guard() { if (c) thor_grid_destroy(c); } } guard{ctx};
+    CU(cudaGetDevice(&ctx->device));
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, ctx->device));
+    if (prop.major != 10)
+        return fail(nullptr, THOR_ERR_UNSUPPORTED, std::string("thor_dataset_create_gridless: device '") + prop.name + "' is not sm_100");
+    ctx->n_sm = prop.multiProcessorCount;
+    ctx->stream = (cudaStream_t)stream;
+    ctx->gridless = true;
+    ctx->gl = *d;
+    ctx->gl.r_in = r_in;
+    ctx->g.nx = ctx->g.ny = ctx->g.nz = 1;
+    ctx->cell_cm = d->length_cm;
+    ctx->has_dust = d->kdust0 > 0;
+    CU(cudaMalloc(&ctx->d_small, SMALL_TOTAL * sizeof(unsigned long long)));
+    CU(cudaEventCreate(&ctx->ev0));
+    CU(cudaEventCreate(&ctx->ev1));
+    guard.c = nullptr;
+    *out = ctx;
+    return THOR_OK;
+}
+
 extern "C" thor_status thor_sources_set(thor_ctx* ctx, long long n_src, const float* pos_xyz, const float* lum,
                                         const float* sigma_kms) {
     if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_sources_set: ctx is NULL");
@@ -222,6 +266,11 @@ extern "C" thor_status thor_sources_set(thor_ctx* ctx, long long n_src, const fl
     std::vector<double> cdf((size_t)n_src);
     double tot = 0;
     for (long long i = 0; i < n_src; ++i) {
+        if (ctx->gridless) {
+            const double x = pos_xyz[3 * i], y = pos_xyz[3 * i + 1], z = pos_xyz[3 * i + 2];
+            const bool in = ctx->gl.geometry == THOR_GEOM_SLAB ? std::fabs(z) <= ctx->gl.r_out : x * x + y * y + z * z <= ctx->gl.r_out * ctx->gl.r_out;
+            if (!in || !std::isfinite(x) || !std::isfinite(y)) return fail(ctx, THOR_ERR_ARG, "thor_sources_set: source " + std::to_string(i) + " lies outside the dataset");
+        } else
         for (int ax = 0; ax < 3; ++ax) {
             const float p = pos_xyz[3 * i + ax];
             if (!(p >= 0.f && p <= (float)n[ax])) return fail(ctx, THOR_ERR_ARG, "thor_sources_set: source " + std::to_string(i) + " lies outside the grid");
@@ -314,6 +363,32 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     p.c_a = (float)K.c_a; p.c_vth = (float)K.c_vth; p.inv_c_vth = (float)(1.0 / K.c_vth);
     p.cell_cm = (float)ctx->cell_cm;
     p.max_crossings = (o.max_crossings && o.max_crossings < 0xffffffffull) ? (unsigned)o.max_crossings : 0xffffffffu;
+    p.gl_geom = -1;
+    if (ctx->gridless) {
+        const thor_gridless& d = ctx->gl;
+        if (o.peel_on || o.hubble_kms_per_cell != 0 || o.core_skip_mode == 2)
+            return fail(ctx, THOR_ERR_UNSUPPORTED, "thor_run: peel-off, Hubble drift and local core-skipping need a grid dataset");
+        const double vth = K.c_vth * std::sqrt(d.T);
+        // step limiter l_max = f min(l_v, l_rho) (reading A29)
+        double lv = INFINITY, lrho = INFINITY;
+        if (d.geometry == THOR_GEOM_SLAB) {
+            if (d.v_max != 0) lv = vth * d.r_out / std::fabs(d.v_max);
+        } else {
+            if (d.v_max != 0 && d.alpha_v != 0) {
+                const double rm = d.alpha_v >= 1.0 ? d.r_out : std::fmax(d.r_in, 1e-300);
+                lv = vth / (std::fabs(d.alpha_v * d.v_max) * std::pow(rm / d.r_out, d.alpha_v - 1.0) / d.r_out);
+            }
+            if (d.alpha_rho != 0) lrho = d.r_out / std::fabs(d.alpha_rho);
+        }
+        const double lm = std::fmin(lv, lrho);
+        p.gl_geom = d.geometry;
+        p.gl_rin = d.r_in; p.gl_rout = d.r_out;
+        p.gl_lmax = (d.step_f > 0 && std::isfinite(lm)) ? (float)(d.step_f * lm) : INFINITY;
+        p.gl_nsig0 = (float)(d.n0 * K.c_sig / std::sqrt(d.T) * d.length_cm);
+        p.gl_kd0 = (float)(d.kdust0 * d.length_cm);
+        p.gl_alpha_rho = (float)d.alpha_rho; p.gl_vmax = (float)d.v_max; p.gl_alpha_v = (float)d.alpha_v;
+        p.gl_a = (float)(K.c_a / std::sqrt(d.T)); p.gl_vth = (float)vth; p.gl_inv_vth = (float)(1.0 / vth);
+    }
     p.n_src = ctx->n_src; p.src_pos = ctx->d_src_pos; p.src_sigma = ctx->d_src_sigma; p.src_cdf = ctx->d_src_cdf;
     p.phase_core = o.phase_core; p.phase_wing = o.phase_wing; p.phase_frame = o.phase_frame;
     p.phase_split_x = (float)o.phase_split_x;
@@ -414,6 +489,7 @@ extern "C" thor_status thor_raytrace(thor_ctx* ctx, long long n_rays, const floa
                                      double hubble_kms_per_cell, int n_v, double v_lo, double v_hi, float* out_column,
                                      float* out_tmean, float* out_tau) {
     if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_raytrace: ctx is NULL");
+    if (ctx->gridless) return fail(ctx, THOR_ERR_UNSUPPORTED, "thor_raytrace: needs a grid dataset");
     if (n_rays <= 0 || !org_xyz || !dir_xyz) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: no rays");
     if (!out_column && !out_tmean && !out_tau) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: no output requested");
     if (out_tau && (n_v <= 0 || !(v_hi > v_lo))) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: bad velocity axis");
@@ -436,6 +512,7 @@ extern "C" thor_status thor_raytrace(thor_ctx* ctx, long long n_rays, const floa
 extern "C" thor_status thor_volume_render(thor_ctx* ctx, long long n_rays, const float* org_xyz, const float* dir_xyz,
                                           int n_peaks, const float* peaks, double n_ref, float* out_rgba) {
     if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_volume_render: ctx is NULL");
+    if (ctx->gridless) return fail(ctx, THOR_ERR_UNSUPPORTED, "thor_volume_render: needs a grid dataset");
     if (n_rays <= 0 || !org_xyz || !dir_xyz || !out_rgba) return fail(ctx, THOR_ERR_ARG, "thor_volume_render: no rays or no output");
     if (!peaks || n_peaks < 1 || n_peaks > THOR_MAX_TF_PEAKS) return fail(ctx, THOR_ERR_ARG, "thor_volume_render: n_peaks out of range");
     if (!(n_ref >= 0.0) || !std::isfinite(n_ref)) return fail(ctx, THOR_ERR_ARG, "thor_volume_render: bad n_ref");

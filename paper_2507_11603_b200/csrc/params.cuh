@@ -92,6 +92,13 @@ struct WalkParams {
     uint32_t* pool;                      // [slots][PK_WORDS] parked packet states, or nullptr = no drain kernel
     unsigned long long* pool_count;      // packets parked
     unsigned long long* pool_next;       // next slot to pop
+    // gridless dataset (PAPER.md 3.3: spherical shell / infinite slab with power-law density and velocity); gl_geom < 0 = grid
+    int gl_geom;                         // -1 grid, 0 shell / sphere, 1 slab
+    double gl_rin, gl_rout;              // length units
+    float gl_lmax;                       // step limiter l_max, +inf = none
+    float gl_nsig0, gl_kd0;              // n0 sigma_0(T) length_cm and kdust0 length_cm: optical depths per length unit at r_out
+    float gl_alpha_rho, gl_vmax, gl_alpha_v;
+    float gl_a, gl_vth, gl_inv_vth;      // the one temperature of the dataset
     int walk_variant;                    // 0 = by grid size, 3 / 4 = force the cache-resident / beyond-L2 kernel (tests)
 };
 

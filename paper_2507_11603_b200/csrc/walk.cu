@@ -80,6 +80,7 @@ __device__ __forceinline__ void tally_packet(const WalkParams& p, BlockTallies& 
 // lanes step the packet redundantly — same instructions, same operands, warp-uniform control flow — reading the window
 // instead of computing.  Blocks are consumed in the packet's own order (trial, trial, ..., finish, finish), so the walk
 // is bit-identical to the staged loop's.  Packets of the warp take turns, one window each.
+template <bool GL>
 __device__ __forceinline__ void park_store(uint32_t* w, const Packet& k, int state) {
     w[0] = (uint32_t)k.ray.cx; w[1] = (uint32_t)k.ray.cy; w[2] = (uint32_t)k.ray.cz;
     w[3] = __float_as_uint(k.ray.fx); w[4] = __float_as_uint(k.ray.fy); w[5] = __float_as_uint(k.ray.fz);
@@ -93,8 +94,15 @@ __device__ __forceinline__ void park_store(uint32_t* w, const Packet& k, int sta
     w[27] = __float_as_uint(k.x_in); w[28] = __float_as_uint(k.upar);
     w[29] = k.nscat; w[30] = k.crossings; w[31] = k.rej_iters; w[32] = k.trials;
     w[33] = (k.stale ? 1u : 0u) | (k.inv_ok ? 2u : 0u); w[34] = (uint32_t)state;
+    if (GL) {
+        const unsigned long long x = (unsigned long long)__double_as_longlong(k.gx), y = (unsigned long long)__double_as_longlong(k.gy),
+                                 z = (unsigned long long)__double_as_longlong(k.gz);
+        w[36] = (uint32_t)x; w[37] = (uint32_t)(x >> 32); w[38] = (uint32_t)y; w[39] = (uint32_t)(y >> 32);
+        w[40] = (uint32_t)z; w[41] = (uint32_t)(z >> 32);
+    }
 }
 
+template <bool GL>
 __device__ __forceinline__ int park_load(const uint32_t* w, Packet& k) {
     k.ray.cx = (int)w[0]; k.ray.cy = (int)w[1]; k.ray.cz = (int)w[2];
     k.ray.fx = __uint_as_float(w[3]); k.ray.fy = __uint_as_float(w[4]); k.ray.fz = __uint_as_float(w[5]);
@@ -108,6 +116,11 @@ __device__ __forceinline__ int park_load(const uint32_t* w, Packet& k) {
     k.x_in = __uint_as_float(w[27]); k.upar = __uint_as_float(w[28]);
     k.nscat = w[29]; k.crossings = w[30]; k.rej_iters = w[31]; k.trials = w[32];
     k.stale = (w[33] & 1u) != 0u; k.inv_ok = (w[33] & 2u) != 0u;
+    if (GL) {
+        k.gx = __longlong_as_double((long long)(((unsigned long long)w[37] << 32) | w[36]));
+        k.gy = __longlong_as_double((long long)(((unsigned long long)w[39] << 32) | w[38]));
+        k.gz = __longlong_as_double((long long)(((unsigned long long)w[41] << 32) | w[40]));
+    }
     return (int)w[34];
 }
 
@@ -138,7 +151,7 @@ __device__ __forceinline__ void coop_fill_window(float4* win, const BlockRng& rn
 // The drain kernel: launched behind walk_kernel on the same stream.  Each warp pops one parked packet at a time from the
 // global pool and walks it to its end, all 32 lanes on that one packet (see above).  4 warps per CTA — one per SM
 // sub-partition — and a register budget of its own (the walk kernel is held to 80 registers by its occupancy).
-template <bool HUBBLE, bool PEEL>
+template <bool HUBBLE, bool PEEL, bool GL>
 __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_constant__ WalkParams p) {
     __shared__ BlockTallies sh;
     __shared__ float4 s_win[DRAIN_WARPS][32 * WIN_STRIDE / 4];
@@ -159,7 +172,7 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
         if (lane == 0) slot = atomicAdd(p.pool_next, 1ull);
         slot = __shfl_sync(0xffffffffu, slot, 0);
         if (slot >= n_pool) break;
-        int st = park_load(p.pool + slot * PK_WORDS, k);      // every lane reads the same words: one broadcast per load
+        int st = park_load<GL>(p.pool + slot * PK_WORDS, k);      // every lane reads the same words: one broadcast per load
         int c = 32;                                           // first unconsumed block of the window (32 = none left)
         float4 my_u = make_float4(0.f, 0.f, 0.f, 0.f);        // this lane's own block of the window
         float my_sC = 0.f, my_cC = 0.f;
@@ -167,7 +180,7 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
         env.mTot = -1.f;
         for (;;) {
             if (st == LS_MARCH) {
-                const int ev = march_step<HUBBLE, false>(p, sh.voigt, k);
+                const int ev = GL ? march_step_gridless(p, sh.voigt, k) : march_step<HUBBLE, false>(p, sh.voigt, k);
                 if (ev == EV_CROSSED) continue;
                 if (ev != EV_HIT) { if (lane == 0) tally_packet(p, sh, ev, k); break; }
                 st = LS_TRIAL;
@@ -238,7 +251,7 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
         if (sh.spectrum[i]) atomicAdd(p.spectrum + i, (unsigned long long)sh.spectrum[i]);
 }
 
-template <bool HUBBLE, bool PEEL, int MIN_CTAS>
+template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL>
 __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __grid_constant__ WalkParams p) {
     __shared__ BlockTallies sh;
     if (threadIdx.x == 0) atomicMin(p.t_start, global_timer_ns());
@@ -274,11 +287,12 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
                 if (i >= p.n_photons) {
                     state = LS_OUT;
                 } else {
-                    float dV;
-                    emit_packet(p, k, p.id_offset + i, k0, k1, dV);
+                    float dV = 0.f;
+                    if (GL) emit_packet_gridless(p, k, p.id_offset + i, k0, k1);
+                    else emit_packet(p, k, p.id_offset + i, k0, k1, dV);
                     if (PEEL) {
                         ++peel_rays;
-                        peel_ray<HUBBLE>(p, sh.voigt, k.ray, k.cell,
+                        peel_ray<HUBBLE, false>(p, sh.voigt, k.ray, k.cell,
                                          dot3(k.cell.vx, k.cell.vy, k.cell.vz, p.kobs[0], p.kobs[1], p.kobs[2]) + dV, 1.f,
                                          peel_cells, true);
                     }
@@ -300,14 +314,14 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
                 unsigned long long base = 0;
                 if (lane == 0) base = atomicAdd(p.pool_count, (unsigned long long)__popc(live));
                 base = __shfl_sync(0xffffffffu, base, 0);
-                if (act) park_store(p.pool + (base + __popc(live & ((1u << lane) - 1u))) * PK_WORDS, k, state);
+                if (act) park_store<GL>(p.pool + (base + __popc(live & ((1u << lane) - 1u))) * PK_WORDS, k, state);
                 break;
             }
         }
 
         // ---- a4-a7: one cell step for every marching lane ----
         if (state == LS_MARCH) {
-            const int ev = march_step<HUBBLE, EARLY>(p, sh.voigt, k);
+            const int ev = GL ? march_step_gridless(p, sh.voigt, k) : march_step<HUBBLE, EARLY>(p, sh.voigt, k);
             if (ev == EV_HIT) { env.mTot = -1.f; state = LS_TRIAL; }   // envelope not built yet
             else if (ev != EV_CROSSED) { tally_packet(p, sh, ev, k); state = LS_IDLE; }
         }
@@ -483,26 +497,26 @@ cudaError_t launch_volume_render(const WalkParams& p, const TransferFn& tf, long
 // issue-bound, 4 CTAs (64 registers, 32 warps) when it does not and the walk needs more gathers in flight
 // (+18 % on the 512^3 gather workload, -6 % on the cache-resident sphere); 2 CTAs with peel-off (<= 128 registers).
 // The drain kernel follows on the same stream: a persistent grid of 4-warp CTAs whose warps pop parked packets.
-template <bool HUBBLE, bool PEEL, int MIN_CTAS>
+template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL = false>
 static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {
     int per_sm = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, walk_kernel<HUBBLE, PEEL, MIN_CTAS>, WALK_THREADS, 0);
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, walk_kernel<HUBBLE, PEEL, MIN_CTAS, GL>, WALK_THREADS, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     long long blocks = (long long)n_sm * per_sm;
     const long long need = (long long)((p.n_photons + 31) / 32);   // few packets: spread the warps over the SMs
     if (need < blocks) blocks = need < 1 ? 1 : need;
     if (blocks_out) *blocks_out = (int)blocks;
-    walk_kernel<HUBBLE, PEEL, MIN_CTAS><<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(p);
+    walk_kernel<HUBBLE, PEEL, MIN_CTAS, GL><<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess || !p.pool) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, drain_kernel<HUBBLE, PEEL>, DRAIN_THREADS, 0);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, drain_kernel<HUBBLE, PEEL, GL>, DRAIN_THREADS, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     long long dblocks = (long long)n_sm * per_sm;
     const long long cap = (blocks * (WALK_THREADS / 32) * COOP_MAX_LANES + DRAIN_WARPS - 1) / DRAIN_WARPS;   // one warp per slot
     if (cap < dblocks) dblocks = cap;
-    drain_kernel<HUBBLE, PEEL><<<(unsigned)dblocks, DRAIN_THREADS, 0, stream>>>(p);
+    drain_kernel<HUBBLE, PEEL, GL><<<(unsigned)dblocks, DRAIN_THREADS, 0, stream>>>(p);
     return cudaGetLastError();
 }
 
@@ -511,6 +525,7 @@ long long walk_pool_slots(int n_sm) { return (long long)n_sm * 4 * (WALK_THREADS
 int walk_pool_words() { return PK_WORDS; }
 
 cudaError_t launch_walk(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {
+    if (p.gl_geom >= 0) return launch_variant<false, false, THOR_WALK_MIN_CTAS, true>(p, n_sm, stream, blocks_out);
     const bool hub = p.hubble != 0.f, peel = p.peel_on != 0;
     const double cells = (double)p.g.nx * p.g.ny * p.g.nz;
     const double grid_bytes = cells * (p.packed ? 32.0 : (p.has_dust ? 24.0 : 20.0));

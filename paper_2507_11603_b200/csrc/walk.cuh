@@ -123,8 +123,8 @@ __device__ __forceinline__ float cell_opacity(const float2* s_tab, const Cell& c
 // (pixel of the starting point projected perpendicular to k_obs, spectral bin of dv = -V at the box face).  `add` is
 // false on the lanes that only shadow a packet in the cooperative drain (one lane tallies).
 template <bool HUBBLE>
-__device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, const Ray& at, const Cell& own, float V_o,
-                                      float phat, uint32_t& n_cells, bool add) {
+__device__ __forceinline__ void peel_ray_body(const WalkParams& p, const float2* s_tab, const Ray& at, const Cell& own, float V_o,
+                                              float phat, uint32_t& n_cells, bool add) {
     const float px0 = (float)at.cx + at.fx - 0.5f * (float)p.g.nx;
     const float py0 = (float)at.cy + at.fy - 0.5f * (float)p.g.ny;
     const float pz0 = (float)at.cz + at.fz - 0.5f * (float)p.g.nz;
@@ -145,10 +145,12 @@ __device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, 
         first = false;
         const float vk = dot3(c.vx, c.vy, c.vz, r.kx, r.ky, r.kz);
         float dtau, s_hit, kt;
-        integrate_segment<HUBBLE>(p, s_tab, c, V, vk, len, 3.0e38f, dtau, s_hit, kt);
+        // the ray is dropped beyond tau_peel_max (reading A13): asking the segment for no more than what is left to the
+        // cap lets it stop at the sub-step that reaches it instead of integrating the whole cell
+        ++n_cells;
+        if (integrate_segment<HUBBLE>(p, s_tab, c, V, vk, len, fmaf(p.tau_peel_max - tau, 1.0000002f, 1e-30f), dtau, s_hit, kt)) return;
         tau += dtau;
         if (HUBBLE) V = fmaf(-p.hubble, len, V);
-        ++n_cells;
         if (tau > p.tau_peel_max) return;
         // peel rays leave through the first box face they meet, periodic or not
         const float ke = ex == 0 ? r.kx : ex == 1 ? r.ky : r.kz;
@@ -164,6 +166,24 @@ __device__ __noinline__ void peel_ray(const WalkParams& p, const float2* s_tab, 
     if (q && add) atomicAdd(p.cube + ((size_t)(int)py * p.peel_nx + (int)px) * p.peel_nv + iv, q);
 }
 
+// INLINE: the drain kernel has registers to spare and walks one packet per warp, where a call's spills are pure latency.
+template <bool HUBBLE, bool INLINE>
+__device__ __forceinline__ void peel_ray(const WalkParams& p, const float2* s_tab, const Ray& at, const Cell& own, float V_o,
+                                         float phat, uint32_t& n_cells, bool add);
+
+template <bool HUBBLE>
+__device__ __noinline__ void peel_ray_call(const WalkParams& p, const float2* s_tab, const Ray& at, const Cell& own, float V_o,
+                                           float phat, uint32_t& n_cells, bool add) {
+    peel_ray_body<HUBBLE>(p, s_tab, at, own, V_o, phat, n_cells, add);
+}
+
+template <bool HUBBLE, bool INLINE>
+__device__ __forceinline__ void peel_ray(const WalkParams& p, const float2* s_tab, const Ray& at, const Cell& own, float V_o,
+                                         float phat, uint32_t& n_cells, bool add) {
+    if (INLINE) peel_ray_body<HUBBLE>(p, s_tab, at, own, V_o, phat, n_cells, add);
+    else peel_ray_call<HUBBLE>(p, s_tab, at, own, V_o, phat, n_cells, add);
+}
+
 // ---- one packet, and the steps of its life as functions shared by every code variant that walks it ----
 struct Packet {
     Ray ray;
@@ -175,6 +195,8 @@ struct Packet {
     uint32_t nscat, crossings, rej_iters, trials;
     bool stale;                  // cell must be (re)gathered / derived before use
     bool inv_ok;                 // 1/k of the current direction is in `ray`
+    double gx, gy, gz;           // gridless datasets only: position in length units (fp64: a line-centre mean free path
+                                 // is 1e-6 ... 1e-9 of the radius, below fp32 spacing); unused and optimised away on grids
 };
 
 enum : int { EV_CROSSED = 0, EV_HIT = 1, EV_ESCAPED = 2, EV_TERMINATED = 3, EV_CAPPED = 4, EV_ABSORBED = 5, EV_SCATTERED = 6 };
@@ -263,6 +285,123 @@ __device__ __forceinline__ int march_step(const WalkParams& p, const float2* s_t
     return EV_CROSSED;
 }
 
+// ---- gridless datasets (PAPER.md 3.3; readings A29-A31): analytic shell / sphere / slab ----
+// Geometry in fp64 (positions, boundary distances), physics in fp32 as on grids.  B200's FP64 pipe makes the handful of
+// double operations per step cheap; there is no cell to anchor an fp32 offset to.
+
+// Gas of a step: the dataset's properties at position r (the step's midpoint, reading A30) into the packet's Cell.
+__device__ __forceinline__ void gl_props(const WalkParams& p, double x, double y, double z, Cell& c) {
+    c.a = p.gl_a; c.vth = p.gl_vth; c.inv_vth = p.gl_inv_vth;
+    c.vx = 0.f; c.vy = 0.f; c.vz = 0.f;
+    if (p.gl_geom == 1) {
+        const bool in = fabs(z) <= p.gl_rout;
+        c.nsig = in ? p.gl_nsig0 : 0.f;
+        c.kd = in ? p.gl_kd0 : 0.f;
+        if (in) c.vz = p.gl_vmax * (float)(z / p.gl_rout);
+        return;
+    }
+    const double rr = sqrt(fma(z, z, fma(y, y, x * x)));
+    if (rr < p.gl_rin || rr > p.gl_rout) { c.nsig = 0.f; c.kd = 0.f; return; }
+    const float q = (float)(rr / p.gl_rout);
+    const float w = p.gl_alpha_rho == 0.f ? 1.f : __powf(q, p.gl_alpha_rho);
+    c.nsig = p.gl_nsig0 * w;
+    c.kd = p.gl_kd0 * w;
+    if (rr > 0.0 && p.gl_vmax != 0.f) {
+        const float vm = p.gl_vmax * (p.gl_alpha_v == 1.f ? q : __powf(q, p.gl_alpha_v)) / (float)rr;
+        c.vx = vm * (float)x; c.vy = vm * (float)y; c.vz = vm * (float)z;
+    }
+}
+
+__device__ __forceinline__ void emit_packet_gridless(const WalkParams& p, Packet& k, unsigned long long id, uint32_t k0, uint32_t k1) {
+    k.rng.init(id);
+    const float4 e1 = k.rng.next4(k0, k1), e2 = k.rng.next4(k0, k1);   // (src, mu, phi, g1), (g2, tau, -, -)
+    const double us = (double)e1.x;
+    long long lo = 0, hi = p.n_src - 1;
+    while (lo < hi) { const long long mid = (lo + hi) >> 1; if (us < p.src_cdf[mid]) hi = mid; else lo = mid + 1; }
+    const float mu0 = fmaf(2.f, e1.y, -1.f);
+    float sp, cp;
+    sincos_uniform(e1.z, sp, cp);
+    const float st0 = sqrtf(fmaxf(0.f, fmaf(-mu0, mu0, 1.f)));
+    const float gauss = sqrtf(2.f * neg_log(e1.w)) * cos_uniform(e2.x);
+    k.gx = (double)p.src_pos[3 * lo]; k.gy = (double)p.src_pos[3 * lo + 1]; k.gz = (double)p.src_pos[3 * lo + 2];
+    ray_set_k(k.ray, st0 * cp, st0 * sp, mu0);
+    k.inv_ok = false; k.stale = false;
+    gl_props(p, k.gx, k.gy, k.gz, k.cell);
+    k.V = dot3(k.cell.vx, k.cell.vy, k.cell.vz, k.ray.kx, k.ray.ky, k.ray.kz) + p.src_sigma[lo] * gauss;
+    k.nscat = 0; k.crossings = 0; k.rej_iters = 0; k.trials = 0;
+    k.tau_rem = neg_log(e2.y);
+}
+
+// One step (readings A29-A31): to the next boundary ahead but at most l_max; gas of the midpoint; interaction site linear
+// within the step.  Same events as march_step; `crossings` counts steps.
+__device__ __forceinline__ int march_step_gridless(const WalkParams& p, const float2* s_tab, Packet& k) {
+    const double kx = (double)k.ray.kx, ky = (double)k.ray.ky, kz = (double)k.ray.kz;
+    const double R = p.gl_rout;
+    double db;
+    bool in_gas = true;
+    if (p.gl_geom == 1) {
+        db = kz > 0.0 ? (R - k.gz) / kz : (kz < 0.0 ? (-R - k.gz) / kz : (double)CUDART_INF_F);
+    } else {
+        const double b = fma(k.gz, kz, fma(k.gy, ky, k.gx * kx));
+        const double r2 = fma(k.gz, k.gz, fma(k.gy, k.gy, k.gx * k.gx));
+        if (p.gl_rin == 0.0 && p.gl_lmax == CUDART_INF_F && p.gl_alpha_rho == 0.f && p.gl_vmax == 0.f) {
+            // homogeneous static sphere: the gas does not depend on the step, so the interaction site s = tau / kappa is
+            // known before the boundary is; (|r| + s)^2 <= R^2 is implied by r^2 + s^2 + 2 s R <= R^2: no square root
+            gl_props(p, k.gx, k.gy, k.gz, k.cell);
+            const float kt0 = cell_opacity(s_tab, k.cell, k.V, 0.f);
+            if (kt0 > 0.f) {
+                const double s = (double)(k.tau_rem / kt0);
+                if (fma(s, s + 2.0 * R, r2) <= R * R) {
+                    k.gx = fma(s, kx, k.gx); k.gy = fma(s, ky, k.gy); k.gz = fma(s, kz, k.gz);
+                    k.hit_kt = kt0; k.x_in = k.V * k.cell.inv_vth; k.trials = 0u;
+                    return EV_HIT;
+                }
+            }
+        }
+        if (r2 < p.gl_rin * p.gl_rin) {
+            in_gas = false;
+            db = -b + sqrt(fmax(0.0, fma(b, b, -(r2 - p.gl_rin * p.gl_rin))));
+        } else {
+            db = -1.0;
+            if (p.gl_rin > 0.0 && b < 0.0) {
+                const double disc = fma(b, b, -(r2 - p.gl_rin * p.gl_rin));
+                if (disc > 0.0) { const double t = -b - sqrt(disc); if (t >= 0.0) db = t; }
+            }
+            if (db < 0.0) db = -b + sqrt(fmax(0.0, fma(b, b, -(r2 - R * R))));
+        }
+    }
+    const bool inf_step = !(db < (double)CUDART_INF_F) && p.gl_lmax == CUDART_INF_F;   // slab, k_z = 0, no limiter (A24)
+    const double len = inf_step ? 0.0 : (in_gas ? fmin(db, (double)p.gl_lmax) : db);
+    float kt = 0.f, vk = 0.f;
+    if (in_gas) {
+        gl_props(p, fma(0.5 * len, kx, k.gx), fma(0.5 * len, ky, k.gy), fma(0.5 * len, kz, k.gz), k.cell);
+        vk = dot3(k.cell.vx, k.cell.vy, k.cell.vz, k.ray.kx, k.ray.ky, k.ray.kz);
+        kt = cell_opacity(s_tab, k.cell, k.V, vk);
+    }
+    if (kt > 0.f && (inf_step || kt * (float)len >= k.tau_rem)) {
+        const double s = (double)(k.tau_rem / kt);
+        k.gx = fma(s, kx, k.gx); k.gy = fma(s, ky, k.gy); k.gz = fma(s, kz, k.gz);
+        k.hit_kt = kt; k.x_in = (k.V - vk) * k.cell.inv_vth; k.trials = 0u;
+        return EV_HIT;
+    }
+    if (inf_step) return EV_CAPPED;
+    k.tau_rem -= kt * (float)len;
+    k.gx = fma(len, kx, k.gx); k.gy = fma(len, ky, k.gy); k.gz = fma(len, kz, k.gz);
+    ++k.crossings;
+    if (len >= db) {                                          // a boundary: leaving the dataset ends the packet (A31)
+        if (p.gl_geom == 1) return EV_ESCAPED;
+        const double rr = sqrt(fma(k.gz, k.gz, fma(k.gy, k.gy, k.gx * k.gx)));
+        const double bb = fma(k.gz, kz, fma(k.gy, ky, k.gx * kx));
+        const bool at_inner = p.gl_rin > 0.0 && rr < p.gl_rin * (1.0 + 1e-12);
+        if (bb > 0.0 && rr >= R * (1.0 - 1e-12) && !at_inner) return EV_ESCAPED;
+        const double nudge = 1e-12 * R;                       // step across the inner sphere
+        k.gx = fma(nudge, kx, k.gx); k.gy = fma(nudge, ky, k.gy); k.gz = fma(nudge, kz, k.gz);
+    }
+    if (p.v_max > 0.f && fabsf(k.V) > p.v_max) return EV_TERMINATED;
+    if (k.crossings >= p.max_crossings) return EV_CAPPED;
+    return EV_CROSSED;
+}
+
 // The random numbers of one FINISH, turned into what the event needs.  Draws: (tau, mu, phi, perp1), (perp2, dust, mix, -).
 struct FinDraws {
     float tau_next;              // -ln s1.x
@@ -315,7 +454,7 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
         const float V_o = fmaf(x_o, c.vth, dot3(c.vx, c.vy, c.vz, p.kobs[0], p.kobs[1], p.kobs[2]));
         ++peel_rays;
         // mix: the sampled branch weights the ray (unbiased; reading A27)
-        peel_ray<HUBBLE>(p, s_tab, k.ray, c, V_o, is_dipole ? 0.75f * fmaf(mu_o, mu_o, 1.f) : 1.f, peel_cells, add);
+        peel_ray<HUBBLE, PRE>(p, s_tab, k.ray, c, V_o, is_dipole ? 0.75f * fmaf(mu_o, mu_o, 1.f) : 1.f, peel_cells, add);
     }
     const float st = sqrtf(fmaxf(0.f, fmaf(-mu, mu, 1.f)));
     float nx = fmaf(st, fmaf(d.cphi, e1[0], d.sphi * e2[0]), mu * kx);

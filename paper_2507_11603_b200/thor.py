@@ -19,7 +19,7 @@ COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "
                  "peel_rays", "peel_cells"]
 RAW_DTYPE = np.dtype([("V", "<f4"), ("nscat", "<u4"), ("status", "<i4"), ("kx", "<f4"), ("ky", "<f4"), ("kz", "<f4")])
 
-EXPORTS = ["thor_grid_create", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run",
+EXPORTS = ["thor_grid_create", "thor_dataset_create_gridless", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run",
            "thor_last_run_ms", "thor_last_run_feed_ms", "thor_last_run_max_nscat", "thor_raytrace", "thor_volume_render", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_dda_trace",
            "thor_unit_voigt", "thor_unit_scatter"]
 
@@ -49,6 +49,15 @@ class Opts(C.Structure):
     ]
 
 
+class Gridless(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("geometry", C.c_int32), ("r_in", C.c_double), ("r_out", C.c_double),
+                ("length_cm", C.c_double), ("n0", C.c_double), ("alpha_rho", C.c_double), ("T", C.c_double),
+                ("v_max", C.c_double), ("alpha_v", C.c_double), ("kdust0", C.c_double), ("step_f", C.c_double)]
+
+
+GRIDLESS_DEFAULTS = dict(geometry=0, r_in=0.0, r_out=1.0, length_cm=1.0, n0=0.0, alpha_rho=0.0, T=1e4, v_max=0.0, alpha_v=1.0,
+                         kdust0=0.0, step_f=0.01)
+
 _lib = None
 
 
@@ -62,6 +71,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         P, i32, i64, u32, u64, d, f = C.c_void_p, C.c_int, C.c_longlong, C.c_uint, C.c_uint64, C.c_double, C.c_float
         L.thor_grid_create.argtypes = [C.POINTER(P), i32, i32, i32, d, P, P, P, P, P, P, u32, P]
+        L.thor_dataset_create_gridless.argtypes = [C.POINTER(P), C.POINTER(Gridless), P]
         L.thor_grid_destroy.argtypes = [P]
         L.thor_grid_destroy.restype = None
         L.thor_sources_set.argtypes = [P, i64, P, P, P]
@@ -144,6 +154,19 @@ class Context:
         _check(lib().thor_grid_create(C.byref(self._ctx), nx, ny, nz, float(cell_cm), *ptrs, flags, stream))
         if pack:
             self._keep = None              # THOR_GRID_PACK: the library holds its own copy; release ours
+
+    @classmethod
+    def gridless(cls, **dataset):
+        """A gridless shell / sphere / slab dataset (thor_dataset_create_gridless); keys of GRIDLESS_DEFAULTS."""
+        unknown = set(dataset) - set(GRIDLESS_DEFAULTS)
+        if unknown:
+            raise KeyError(f"unknown gridless fields: {unknown}")
+        d = Gridless(struct_size=C.sizeof(Gridless), **{**GRIDLESS_DEFAULTS, **dataset})
+        self = cls.__new__(cls)
+        self._ctx = C.c_void_p()
+        self._keep = None
+        _check(lib().thor_dataset_create_gridless(C.byref(self._ctx), C.byref(d), _stream()))
+        return self
 
     @classmethod
     def from_workload(cls, grid, host=False, device="cuda", pack=False, extra_flags=0):
@@ -269,8 +292,9 @@ class Context:
 
 
 def run_workload(w, n_photons=None, host=False, raw=True, pack=False, **opt_overrides):
-    """Convenience: build a Context from a workloads.* dict, run it, return the tallies as a dict."""
-    ctx = Context.from_workload(w["grid"], host=host, pack=pack)
+    """Convenience: build a Context from a workloads.* dict (or dict(dataset=<gridless fields>, ...)), run it, return the
+    tallies as a dict."""
+    ctx = Context.gridless(**w["dataset"]) if "dataset" in w else Context.from_workload(w["grid"], host=host, pack=pack)
     try:
         ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
         n = w["n_photons"] if n_photons is None else n_photons

@@ -179,3 +179,70 @@ def test_volume_render_matches_quadrature_of_eq12(oracle):
         assert out[:3] == pytest.approx(C, rel=1e-7)
         assert out[3] == pytest.approx(1 - math.exp(-tau_at[-1]), rel=1e-7)
         assert 0.05 < out[3] < 0.999
+
+
+# ---------------------------------------------------------------- round 2: periodic sight lines, Hubble sub-sampling
+def test_forest_sightline_subsampled_against_quadrature(oracle):
+    """cells are sub-sampled so that a ray step shifts the line by much less than its width.  Uniform static gas
+    swept by H_c = 2.28 km/s per cell (BASELINE.json config 5's drift): tau(V) = n sigma_0 Delta Int_0^L H(a, (V - H_c s) / v_th) ds
+    by scipy quad, to 1e-3 — at T = 1e3 K (0.56 v_th per cell; there even one midpoint per cell is accurate, the midpoint rule
+    converging exponentially on a Gaussian) and at T = 60 K (2.3 v_th per cell), where one midpoint per cell fails by far."""
+    from scipy import integrate, special
+    for T, coarse_fails in ((1e3, False), (60.0, True)):
+        _forest_case(oracle, T, coarse_fails)
+
+
+def _forest_case(oracle, T, coarse_fails):
+    from scipy import integrate, special
+    Hc, L = 2.28, 40
+    shape = (2, 2, L)
+    tau_cell = 0.8
+    n = tau_cell / (oracle.sigma0_cm2(T) * W.PC_CM)
+    z = np.zeros(shape[::-1], np.float32)
+    grid = dict(nx=2, ny=2, nz=L, periodic=(0, 0, 0), cell_cm=W.PC_CM, nHI=np.full(shape[::-1], n, np.float32),
+                T=np.full(shape[::-1], T, np.float32), vx=z, vy=z, vz=z, kdust=None)
+    org, dr = np.array([[1.0, 1.0, 0.0]], np.float32), np.array([[0.0, 0.0, 1.0]], np.float32)
+    vth, a = oracle.vth_kms(T), oracle.voigt_a(T)
+    n_v, v_lo, v_hi = 24, 20.0, 70.0
+    fine = oracle.raytrace_ex(grid, org, dr, n_v, v_lo, v_hi, Hc, hubble_eps=0.25)["tau"][0]
+    coarse = oracle.raytrace(grid, org, dr, n_v, v_lo, v_hi, Hc)["tau"][0]
+    tau_real = float(np.float32(n)) * oracle.sigma0_cm2(T) * W.PC_CM
+    worst_c = 0.0
+    for j in range(n_v):
+        V = v_lo + (j + 0.5) * (v_hi - v_lo) / n_v
+        exact = tau_real * integrate.quad(lambda s: special.wofz((V - Hc * s) / vth + 1j * a).real, 0, L, points=[V / Hc],
+                                          epsabs=1e-12, epsrel=1e-10, limit=400)[0]
+        assert abs(fine[j] - exact) < 1e-3 * exact, (j, fine[j], exact)
+        worst_c = max(worst_c, abs(coarse[j] - exact) / exact)
+    assert (worst_c > 3e-2) == coarse_fails, worst_c
+
+
+def test_periodic_sightline_wraps(oracle):
+    """PAPER.md:520 "periodic boundary conditions": a ray of stated length wraps at periodic faces.  Pins: an axis-aligned ray
+    of 2.5 box lengths collects 2.5 times the row's column; an oblique ray through the periodic box equals the same ray
+    through the box tiled 3 x 3 x 3 without wrapping; a non-periodic axis still ends the ray."""
+    rng = np.random.default_rng(3)
+    N = 6
+    f = lambda: rng.random((N, N, N)).astype(np.float32) + 0.1
+    grid = dict(nx=N, ny=N, nz=N, periodic=(1, 1, 1), cell_cm=1.0, nHI=f(), T=f() * 1e4, vx=f() * 20, vy=f() * 20, vz=f() * 20, kdust=None)
+    r = oracle.raytrace_ex(grid, np.array([[0.0, 2.5, 3.5]], np.float32), np.array([[1.0, 0.0, 0.0]], np.float32), max_length_cells=15.0)
+    row = grid["nHI"][3, 2, :].astype(np.float64)
+    assert abs(r["column"][0] - (2 * row.sum() + row[:3].sum())) < 1e-9
+    org = np.array([[1.25, 4.5, 0.75]], np.float32)              # exact in fp32 also after adding N
+    dr = np.array([[0.48, -0.6, 0.64]], np.float32)
+    tiled = {k: (np.tile(grid[k], (3, 3, 3)) if isinstance(grid[k], np.ndarray) else grid[k]) for k in grid}
+    tiled.update(nx=3 * N, ny=3 * N, nz=3 * N, periodic=(0, 0, 0))
+    a = oracle.raytrace_ex(grid, org, dr, 8, -60.0, 60.0, 1.5, 0.25, max_length_cells=9.0)
+    b = oracle.raytrace_ex(tiled, org + N, dr, 8, -60.0, 60.0, 1.5, 0.25, max_length_cells=9.0)
+    assert abs(a["column"][0] - b["column"][0]) < 1e-9 * b["column"][0]
+    assert np.allclose(a["tau"], b["tau"], rtol=1e-9)
+    c = oracle.raytrace_ex(dict(grid, periodic=(0, 0, 0)), org, dr, max_length_cells=9.0)
+    assert c["column"][0] < a["column"][0]                         # not periodic: ends at the first face
+
+
+def test_slice_is_a_lookup(oracle):
+    """PAPER.md:189 slices: the field value of the cell holding each point of the plane."""
+    rng = np.random.default_rng(4)
+    g = dict(nx=5, ny=4, nz=3, T=rng.random((3, 4, 5)).astype(np.float32))
+    pts = np.array([[0.2, 0.9, 2.99], [4.99, 3.0, 0.0], [2.5, 1.5, 1.5]])
+    assert np.array_equal(oracle.slice_field(g, pts, "T"), [g["T"][2, 0, 0], g["T"][0, 3, 4], g["T"][1, 1, 2]])
