@@ -302,8 +302,14 @@ def run_operators(args):
         return ms
 
     def e2e_step():
-        launch(h_org.cuda(non_blocking=True), h_dir.cuda(non_blocking=True))
-        h_out.copy_(out, non_blocking=True)
+        # the C-ABI call with HOST buffers: the library copies rays in and the image out inside the call
+        ho, hd, hout = (C.c_void_p(t.data_ptr()) for t in (h_org, h_dir, h_out))
+        if render:
+            st = L.thor_volume_render_ex(ctx._ctx, n_rays, ho, hd, len(peaks), peaks.ctypes.data_as(C.c_void_p), 0.0, hout, thor.RAYS_HOST)
+        else:
+            ro = thor.RayOpts(struct_size=C.sizeof(thor.RayOpts), flags=thor.RAYS_HOST)
+            st = L.thor_raytrace_ex(ctx._ctx, n_rays, ho, hd, C.byref(ro), hout, None, None)
+        assert st == 0, thor.lib().thor_last_error(ctx._ctx)
 
     timed(lambda: launch(d_org, d_dir), max(args.warmup, 3))
     sampler = ClockSampler(local)

@@ -210,6 +210,39 @@ thor_status thor_raytrace(thor_ctx *ctx, long long n_rays, const float *org_xyz,
 thor_status thor_volume_render(thor_ctx *ctx, long long n_rays, const float *org_xyz, const float *dir_xyz,
                                int n_peaks, const float *peaks, double n_ref, float *out_rgba);
 
+/* The same operators with the sight lines of the paper's Lyα-forest application and with HOST buffers.
+ *   max_length_cells > 0: the ray wraps at the faces the grid was declared periodic on and ends after that path length
+ *                         (in cell lengths), or at the first non-periodic face; 0: ends at the first box face.
+ *   hubble_eps > 0:       Eq. 11 is sub-sampled: each face-to-face segment is cut into ceil(|H len| / (hubble_eps v_th))
+ *                         sub-steps with the Hubble term at each sub-step's midpoint ("each ray step ... much smaller than
+ *                         the line width"; the rule of reading A12); 0: one midpoint per segment, as thor_raytrace.
+ *   flags & THOR_RAYS_HOST: org_xyz, dir_xyz and every output are HOST pointers; the library stages them through device
+ *                         buffers of its own inside the call (else DEVICE pointers, as thor_raytrace). */
+#define THOR_RAYS_HOST 0x1u
+typedef struct thor_ray_opts {
+    uint32_t struct_size;             /* = sizeof(thor_ray_opts) */
+    uint32_t flags;                   /* THOR_RAYS_HOST */
+    double hubble_kms_per_cell, hubble_eps;
+    double max_length_cells;
+    int32_t n_v;
+    double v_lo, v_hi;
+} thor_ray_opts;
+thor_status thor_raytrace_ex(thor_ctx *ctx, long long n_rays, const float *org_xyz, const float *dir_xyz,
+                             const thor_ray_opts *opts, float *out_column, float *out_tmean, float *out_tau);
+thor_status thor_volume_render_ex(thor_ctx *ctx, long long n_rays, const float *org_xyz, const float *dir_xyz,
+                                  int n_peaks, const float *peaks, double n_ref, float *out_rgba, unsigned flags);
+
+/* Slice operator: out[i] = the value of one field in the cell that holds point pos_xyz[i] (cell units,
+ * clamped into the grid).  field: THOR_FIELD_*.  pos_xyz / out are DEVICE pointers, or HOST with THOR_RAYS_HOST.
+ * THOR_ERR_ARG for NULL / empty input, an unknown field, or kdust on a grid without dust. */
+#define THOR_FIELD_NHI 0
+#define THOR_FIELD_T 1
+#define THOR_FIELD_VX 2
+#define THOR_FIELD_VY 3
+#define THOR_FIELD_VZ 4
+#define THOR_FIELD_KDUST 5
+thor_status thor_slice(thor_ctx *ctx, long long n_points, const float *pos_xyz, int field, float *out, unsigned flags);
+
 /* Static-lifetime or context-owned text of the last error (ctx may be NULL for create-time errors). */
 const char *thor_last_error(const thor_ctx *ctx);
 

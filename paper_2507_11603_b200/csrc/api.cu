@@ -18,8 +18,9 @@ int walk_pool_words();
 cudaError_t launch_volume_render(const WalkParams& p, const TransferFn& tf, long long n_rays, const float* org,
                                  const float* dir, float* out_rgba, cudaStream_t stream);
 cudaError_t launch_raytrace(const WalkParams& p, long long n_rays, const float* org, const float* dir, float hubble,
-                            int n_v, float v_lo, float dv, float* out_column, float* out_tmean, float* out_tau,
-                            cudaStream_t stream);
+                            float hubble_eps, float max_len, int n_v, float v_lo, float dv, float* out_column,
+                            float* out_tmean, float* out_tau, cudaStream_t stream);
+cudaError_t launch_slice(const WalkParams& p, long long n, const float* pos, int field, float* out, cudaStream_t stream);
 cudaError_t launch_pack_fields(const float* nHI, const float* T, const float* vx, const float* vy, const float* vz,
                                const float* kdust, long long n, float4* out, cudaStream_t stream);
 cudaError_t launch_validate_fields(const float* nHI, const float* T, const float* vx, const float* vy, const float* vz,
@@ -485,15 +486,8 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     return THOR_OK;
 }
 
-extern "C" thor_status thor_raytrace(thor_ctx* ctx, long long n_rays, const float* org_xyz, const float* dir_xyz,
-                                     double hubble_kms_per_cell, int n_v, double v_lo, double v_hi, float* out_column,
-                                     float* out_tmean, float* out_tau) {
-    if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_raytrace: ctx is NULL");
-    if (ctx->gridless) return fail(ctx, THOR_ERR_UNSUPPORTED, "thor_raytrace: needs a grid dataset");
-    if (n_rays <= 0 || !org_xyz || !dir_xyz) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: no rays");
-    if (!out_column && !out_tmean && !out_tau) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: no output requested");
-    if (out_tau && (n_v <= 0 || !(v_hi > v_lo))) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: bad velocity axis");
-    if (!std::isfinite(hubble_kms_per_cell)) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: bad Hubble term");
+// grid part of the kernel parameter block, shared by the ray operators
+static thor::WalkParams grid_params(const thor_ctx* ctx) {
     const thor::LyaConstants K = thor::lya_constants();
     thor::WalkParams p{};
     p.g = ctx->g;
@@ -502,15 +496,80 @@ extern "C" thor_status thor_raytrace(thor_ctx* ctx, long long n_rays, const floa
     p.sig_cell = (float)(K.c_sig * ctx->cell_cm);
     p.c_a = (float)K.c_a; p.c_vth = (float)K.c_vth; p.inv_c_vth = (float)(1.0 / K.c_vth);
     p.cell_cm = (float)ctx->cell_cm;
+    p.gl_geom = -1;
+    return p;
+}
+
+// HOST <-> DEVICE staging of the ray operators' buffers (THOR_RAYS_HOST): device twins owned for the length of one call.
+struct Staged {
+    std::vector<void*> dev;
+    ~Staged() { for (void* d : dev) if (d) cudaFree(d); }
+    cudaError_t in(const void* host, size_t bytes, cudaStream_t st, const float** out) {
+        void* d = nullptr;
+        cudaError_t e = cudaMalloc(&d, bytes);
+        if (e != cudaSuccess) return e;
+        dev.push_back(d);
+        *out = static_cast<const float*>(d);
+        return cudaMemcpyAsync(d, host, bytes, cudaMemcpyHostToDevice, st);
+    }
+    cudaError_t out(size_t bytes, float** out_dev) {
+        void* d = nullptr;
+        cudaError_t e = cudaMalloc(&d, bytes);
+        if (e != cudaSuccess) return e;
+        dev.push_back(d);
+        *out_dev = static_cast<float*>(d);
+        return cudaSuccess;
+    }
+};
+
+extern "C" thor_status thor_raytrace_ex(thor_ctx* ctx, long long n_rays, const float* org_xyz, const float* dir_xyz,
+                                        const thor_ray_opts* o, float* out_column, float* out_tmean, float* out_tau) {
+    if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_raytrace: ctx is NULL");
+    if (ctx->gridless) return fail(ctx, THOR_ERR_UNSUPPORTED, "thor_raytrace: needs a grid dataset");
+    if (!o || o->struct_size != sizeof(thor_ray_opts)) return fail(ctx, THOR_ERR_ARG, "thor_raytrace_ex: opts->struct_size is not set");
+    if (n_rays <= 0 || !org_xyz || !dir_xyz) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: no rays");
+    if (!out_column && !out_tmean && !out_tau) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: no output requested");
+    if (out_tau && (o->n_v <= 0 || !(o->v_hi > o->v_lo))) return fail(ctx, THOR_ERR_ARG, "thor_raytrace: bad velocity axis");
+    if (!std::isfinite(o->hubble_kms_per_cell) || !(o->hubble_eps >= 0) || !(o->max_length_cells >= 0) || !std::isfinite(o->max_length_cells))
+        return fail(ctx, THOR_ERR_ARG, "thor_raytrace: bad Hubble term / sub-sampling / length");
+    const thor::WalkParams p = grid_params(ctx);
     CU(cudaSetDevice(ctx->device));
-    CU(thor::launch_raytrace(p, n_rays, org_xyz, dir_xyz, (float)hubble_kms_per_cell, out_tau ? n_v : 0, (float)v_lo,
-                             out_tau ? (float)((v_hi - v_lo) / n_v) : 0.f, out_column, out_tmean, out_tau, ctx->stream));
+    const bool host = (o->flags & THOR_RAYS_HOST) != 0;
+    const int n_v = out_tau ? o->n_v : 0;
+    Staged st;
+    const float *d_org = org_xyz, *d_dir = dir_xyz;
+    float *d_col = out_column, *d_tm = out_tmean, *d_tau = out_tau;
+    if (host) {
+        CU(st.in(org_xyz, (size_t)n_rays * 12, ctx->stream, &d_org));
+        CU(st.in(dir_xyz, (size_t)n_rays * 12, ctx->stream, &d_dir));
+        if (out_column) CU(st.out((size_t)n_rays * 4, &d_col));
+        if (out_tmean) CU(st.out((size_t)n_rays * 4, &d_tm));
+        if (out_tau) CU(st.out((size_t)n_rays * n_v * 4, &d_tau));
+    }
+    CU(thor::launch_raytrace(p, n_rays, d_org, d_dir, (float)o->hubble_kms_per_cell, (float)o->hubble_eps,
+                             (float)o->max_length_cells, n_v, (float)o->v_lo, n_v ? (float)((o->v_hi - o->v_lo) / n_v) : 0.f,
+                             d_col, d_tm, d_tau, ctx->stream));
+    if (host) {
+        if (out_column) CU(cudaMemcpyAsync(out_column, d_col, (size_t)n_rays * 4, cudaMemcpyDeviceToHost, ctx->stream));
+        if (out_tmean) CU(cudaMemcpyAsync(out_tmean, d_tm, (size_t)n_rays * 4, cudaMemcpyDeviceToHost, ctx->stream));
+        if (out_tau) CU(cudaMemcpyAsync(out_tau, d_tau, (size_t)n_rays * n_v * 4, cudaMemcpyDeviceToHost, ctx->stream));
+    }
     CU(cudaStreamSynchronize(ctx->stream));
     return THOR_OK;
 }
 
-extern "C" thor_status thor_volume_render(thor_ctx* ctx, long long n_rays, const float* org_xyz, const float* dir_xyz,
-                                          int n_peaks, const float* peaks, double n_ref, float* out_rgba) {
+extern "C" thor_status thor_raytrace(thor_ctx* ctx, long long n_rays, const float* org_xyz, const float* dir_xyz,
+                                     double hubble_kms_per_cell, int n_v, double v_lo, double v_hi, float* out_column,
+                                     float* out_tmean, float* out_tau) {
+    thor_ray_opts o{};
+    o.struct_size = (uint32_t)sizeof o;
+    o.hubble_kms_per_cell = hubble_kms_per_cell;
+    o.n_v = n_v; o.v_lo = v_lo; o.v_hi = v_hi;
+    return thor_raytrace_ex(ctx, n_rays, org_xyz, dir_xyz, &o, out_column, out_tmean, out_tau);
+}
+
+extern "C" thor_status thor_volume_render_ex(thor_ctx* ctx, long long n_rays, const float* org_xyz, const float* dir_xyz,
+                                             int n_peaks, const float* peaks, double n_ref, float* out_rgba, unsigned flags) {
     if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_volume_render: ctx is NULL");
     if (ctx->gridless) return fail(ctx, THOR_ERR_UNSUPPORTED, "thor_volume_render: needs a grid dataset");
     if (n_rays <= 0 || !org_xyz || !dir_xyz || !out_rgba) return fail(ctx, THOR_ERR_ARG, "thor_volume_render: no rays or no output");
@@ -532,13 +591,46 @@ extern "C" thor_status thor_volume_render(thor_ctx* ctx, long long n_rays, const
         tf.amp[q] = (float)(n_ref > 0.0 ? (double)k[5] / n_ref : (double)k[5]);
         tf.r[q] = k[2]; tf.g[q] = k[3]; tf.b[q] = k[4];
     }
-    thor::WalkParams p{};
-    p.g = ctx->g;
-    p.nHI = ctx->f[0]; p.T = ctx->f[1]; p.vx = ctx->f[2]; p.vy = ctx->f[3]; p.vz = ctx->f[4]; p.kdust = ctx->f[5];
-    p.packed = ctx->d_packed; p.has_dust = ctx->has_dust ? 1 : 0;
-    p.cell_cm = (float)ctx->cell_cm;
+    const thor::WalkParams p = grid_params(ctx);
     CU(cudaSetDevice(ctx->device));
-    CU(thor::launch_volume_render(p, tf, n_rays, org_xyz, dir_xyz, out_rgba, ctx->stream));
+    const bool host = (flags & THOR_RAYS_HOST) != 0;
+    Staged st;
+    const float *d_org = org_xyz, *d_dir = dir_xyz;
+    float* d_out = out_rgba;
+    if (host) {
+        CU(st.in(org_xyz, (size_t)n_rays * 12, ctx->stream, &d_org));
+        CU(st.in(dir_xyz, (size_t)n_rays * 12, ctx->stream, &d_dir));
+        CU(st.out((size_t)n_rays * 16, &d_out));
+    }
+    CU(thor::launch_volume_render(p, tf, n_rays, d_org, d_dir, d_out, ctx->stream));
+    if (host) CU(cudaMemcpyAsync(out_rgba, d_out, (size_t)n_rays * 16, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return THOR_OK;
+}
+
+extern "C" thor_status thor_volume_render(thor_ctx* ctx, long long n_rays, const float* org_xyz, const float* dir_xyz,
+                                          int n_peaks, const float* peaks, double n_ref, float* out_rgba) {
+    return thor_volume_render_ex(ctx, n_rays, org_xyz, dir_xyz, n_peaks, peaks, n_ref, out_rgba, 0u);
+}
+
+extern "C" thor_status thor_slice(thor_ctx* ctx, long long n_points, const float* pos_xyz, int field, float* out, unsigned flags) {
+    if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_slice: ctx is NULL");
+    if (ctx->gridless) return fail(ctx, THOR_ERR_UNSUPPORTED, "thor_slice: needs a grid dataset");
+    if (n_points <= 0 || !pos_xyz || !out) return fail(ctx, THOR_ERR_ARG, "thor_slice: no points or no output");
+    if (field < THOR_FIELD_NHI || field > THOR_FIELD_KDUST) return fail(ctx, THOR_ERR_ARG, "thor_slice: unknown field");
+    if (field == THOR_FIELD_KDUST && !ctx->has_dust) return fail(ctx, THOR_ERR_ARG, "thor_slice: the grid has no dust field");
+    const thor::WalkParams p = grid_params(ctx);
+    CU(cudaSetDevice(ctx->device));
+    const bool host = (flags & THOR_RAYS_HOST) != 0;
+    Staged st;
+    const float* d_pos = pos_xyz;
+    float* d_out = out;
+    if (host) {
+        CU(st.in(pos_xyz, (size_t)n_points * 12, ctx->stream, &d_pos));
+        CU(st.out((size_t)n_points * 4, &d_out));
+    }
+    CU(thor::launch_slice(p, n_points, d_pos, field, d_out, ctx->stream));
+    if (host) CU(cudaMemcpyAsync(out, d_out, (size_t)n_points * 4, cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return THOR_OK;
 }

@@ -6,7 +6,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(os.path.dirname(HERE), "libthor_b200.so")
 HASH = LIB + ".srchash"
-SOURCES = ["api.cu", "walk.cu", "unit_kernels.cu"]
+SOURCES = ["api.cu", "walk.cu", "rayops.cu", "unit_kernels.cu"]
 DEPS = SOURCES + ["walk.cuh", "params.cuh", "philox.cuh", "dda.cuh", "voigt.cuh", "voigt_table.inc", "sampler.cuh",
                   os.path.join("..", "..", "include", "thor.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--shared",

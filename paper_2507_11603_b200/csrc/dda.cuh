@@ -185,4 +185,15 @@ __device__ __forceinline__ bool march_cross(RayMarch& m, const GridDims& g, bool
     return (unsigned)m.cx < (unsigned)g.nx && (unsigned)m.cy < (unsigned)g.ny && (unsigned)m.cz < (unsigned)g.nz;
 }
 
+// The same crossing for a sight line that wraps at periodic faces: an exit through a periodic face re-enters
+// at the opposite one (cell and linear index wrapped); a non-periodic face ends the ray as above.
+__device__ __forceinline__ bool march_cross_wrap(RayMarch& m, const GridDims& g, bool ex_x, bool ex_y, float len) {
+    if (march_cross(m, g, ex_x, ex_y, len)) return true;
+    const bool ex_z = !ex_x && !ex_y;
+    if (ex_x && (g.periodic & 1u)) { const int w = m.cx < 0 ? g.nx : -g.nx; m.cx += w; m.idx += w; return true; }
+    if (ex_y && (g.periodic & 2u)) { const int w = m.cy < 0 ? g.ny : -g.ny; m.cy += w; m.idx += (int64_t)w * g.nx; return true; }
+    if (ex_z && (g.periodic & 4u)) { const int w = m.cz < 0 ? g.nz : -g.nz; m.cz += w; m.idx += (int64_t)w * g.nx * g.ny; return true; }
+    return false;
+}
+
 }  // namespace thor

@@ -371,126 +371,6 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
 }
 
 
-// (n_HI, T) alone: 8 B of the cell's packed sector, or two SoA loads.
-__device__ __forceinline__ void load_nT(const WalkParams& p, int64_t i, float& n, float& T) {
-    if (p.packed) { const float2 q = __ldg(reinterpret_cast<const float2*>(p.packed + 2 * i)); n = q.x; T = q.y; }
-    else { n = __ldg(p.nHI + i); T = __ldg(p.T + i); }
-}
-
-// ---- ray-tracing operators on the same DDA + gather + Voigt (PAPER.md 3.5) ----
-// One thread per ray, marched from its origin to the first box face.  Projection (PAPER.md 3.5.1): Q = Int q w ds with
-// q = n_HI, w = 1 (column density, cm^-2) and q = T, w = n_HI (density-weighted temperature Q / Q^).  Absorption
-// spectrum (PAPER.md 3.5.2, Eq. 11): tau(V_j) = Int n sigma(nu(s), T) ds with the gas seeing the sight-line
-// frequency shifted by its line-of-sight velocity v.k and the Hubble term H s; piecewise-constant cells, midpoint of
-// each segment for the Hubble term.
-__global__ void raytrace_kernel(const __grid_constant__ WalkParams p, long long n_rays, const float* __restrict__ org,
-                                const float* __restrict__ dir, float hubble, int n_v, float v_lo, float dv,
-                                float* __restrict__ out_column, float* __restrict__ out_tmean, float* __restrict__ out_tau) {
-    __shared__ float2 s_tab[VOIGT_NODES];
-    voigt_table_load(s_tab);
-    __syncthreads();
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n_rays) return;
-    RayMarch r;
-    const float kx = dir[3 * i], ky = dir[3 * i + 1], kz = dir[3 * i + 2];
-    march_init(r, p.g, org[3 * i], org[3 * i + 1], org[3 * i + 2], kx, ky, kz);
-    float col = 0.f, tn = 0.f, s_path = 0.f;
-    float* tau = out_tau ? out_tau + i * n_v : nullptr;
-    if (tau) for (int j = 0; j < n_v; ++j) tau[j] = 0.f;
-    for (;;) {
-        bool ex_x, ex_y;
-        const float len = march_next_face(r, ex_x, ex_y);
-        if (!(len < CUDART_INF_F)) break;
-        Cell c;
-        if (tau) c = load_cell_raw(p, r.idx);
-        else load_nT(p, r.idx, c.nsig, c.a);                  // projections need 8 B of the cell only
-        const float n = c.nsig, T = c.a;
-        col = fmaf(n, len, col);
-        tn = fmaf(n * T, len, tn);
-        if (tau) {
-            derive_cell(p, c);
-            const float vgas = fmaf(hubble, fmaf(0.5f, len, s_path), dot3(c.vx, c.vy, c.vz, kx, ky, kz));
-            if (c.nsig > 0.f || c.kd > 0.f)
-                for (int j = 0; j < n_v; ++j) {
-                    const float V = fmaf((float)j + 0.5f, dv, v_lo);
-                    const float kl = c.nsig > 0.f ? c.nsig * voigt_H(s_tab, c.a, (V - vgas) * c.inv_vth) : 0.f;
-                    tau[j] = fmaf(kl + c.kd, len, tau[j]);
-                }
-        }
-        s_path += len;
-        if (!march_cross(r, p.g, ex_x, ex_y, len)) break;     // rays end at the first box face, periodic or not
-    }
-    if (out_column) out_column[i] = col * p.cell_cm;
-    if (out_tmean) out_tmean[i] = col > 0.f ? tn / col : 0.f;
-}
-
-cudaError_t launch_raytrace(const WalkParams& p, long long n_rays, const float* org, const float* dir, float hubble,
-                            int n_v, float v_lo, float dv, float* out_column, float* out_tmean, float* out_tau,
-                            cudaStream_t stream) {
-    raytrace_kernel<<<(unsigned)((n_rays + 127) / 128), 128, 0, stream>>>(p, n_rays, org, dir, hubble, n_v, v_lo, dv,
-                                                                         out_column, out_tmean, out_tau);
-    return cudaGetLastError();
-}
-
-// Volume rendering (PAPER.md 3.5.3, Eq. 12) on the same march: front-to-back compositing with the exact integral of
-// each piecewise-constant segment, C += Tr c (1 - e^{-mu l}), Tr *= e^{-mu l}.  The transfer function (Gaussian peaks
-// in log10 T) arrives by value: per peak {centre in log2 T, -log2(e) / (2 s^2) in log2 units, R, G, B, A / n_ref}.
-__device__ __forceinline__ float ex2_approx(float x) {
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
-__global__ void __launch_bounds__(128) volume_render_kernel(const __grid_constant__ WalkParams p, const __grid_constant__ TransferFn tf,
-                                     long long n_rays, const float* __restrict__ org, const float* __restrict__ dir,
-                                     float4* __restrict__ out_rgba) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n_rays) return;
-    RayMarch r;
-    march_init(r, p.g, org[3 * i], org[3 * i + 1], org[3 * i + 2], dir[3 * i], dir[3 * i + 1], dir[3 * i + 2]);
-    float cr = 0.f, cg = 0.f, cb = 0.f, tr = 1.f;
-    for (;;) {
-        bool ex_x, ex_y;
-        const float len = march_next_face(r, ex_x, ex_y);
-        if (!(len < CUDART_INF_F)) break;
-        float n, T;
-        load_nT(p, r.idx, n, T);
-        const float w = tf.weight_by_density ? n : 1.f;
-        if (w > 0.f && T > 0.f) {
-            const float lt = __log2f(T);
-            float mu = 0.f, er = 0.f, eg = 0.f, eb = 0.f;
-#pragma unroll
-            for (int q = 0; q < MAX_TF_PEAKS; ++q) {
-                if (q >= tf.n_peaks) break;                     // uniform: n_peaks is a kernel parameter
-                const float z = lt - tf.centre[q];
-                const float ag = tf.amp[q] * ex2_approx(tf.neg_inv_2s2[q] * z * z);
-                mu += ag;
-                er = fmaf(ag, tf.r[q], er);
-                eg = fmaf(ag, tf.g[q], eg);
-                eb = fmaf(ag, tf.b[q], eb);
-            }
-            mu *= w;
-            if (mu > 0.f) {
-                const float att = ex2_approx(-1.4426950408889634f * mu * len);
-                const float f = tr * (1.f - att) * w / mu;      // Tr (1 - e^{-mu l}) / mu, times w for the emission
-                cr = fmaf(f, er, cr);
-                cg = fmaf(f, eg, cg);
-                cb = fmaf(f, eb, cb);
-                tr *= att;
-            }
-        }
-        if (!march_cross(r, p.g, ex_x, ex_y, len)) break;
-    }
-    out_rgba[i] = make_float4(cr, cg, cb, 1.f - tr);
-}
-
-cudaError_t launch_volume_render(const WalkParams& p, const TransferFn& tf, long long n_rays, const float* org,
-                                 const float* dir, float* out_rgba, cudaStream_t stream) {
-    volume_render_kernel<<<(unsigned)((n_rays + 127) / 128), 128, 0, stream>>>(p, tf, n_rays, org, dir,
-                                                                              reinterpret_cast<float4*>(out_rgba));
-    return cudaGetLastError();
-}
-
 // Launch configuration: one persistent grid, blocks = SMs x resident blocks per SM.  The kernel is specialised at
 // compile time on (Hubble drift, peel-off) so that the common static, no-peel walk carries neither, and on the
 // register budget: 3 CTAs of 256 threads per SM (<= 80 registers) when the grid fits the 126 MB L2 and the walk is

@@ -20,7 +20,7 @@ COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "
 RAW_DTYPE = np.dtype([("V", "<f4"), ("nscat", "<u4"), ("status", "<i4"), ("kx", "<f4"), ("ky", "<f4"), ("kz", "<f4")])
 
 EXPORTS = ["thor_grid_create", "thor_dataset_create_gridless", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run",
-           "thor_last_run_ms", "thor_last_run_feed_ms", "thor_last_run_max_nscat", "thor_raytrace", "thor_volume_render", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_dda_trace",
+           "thor_last_run_ms", "thor_last_run_feed_ms", "thor_last_run_max_nscat", "thor_raytrace", "thor_raytrace_ex", "thor_volume_render", "thor_volume_render_ex", "thor_slice", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_dda_trace",
            "thor_unit_voigt", "thor_unit_scatter"]
 
 
@@ -47,6 +47,15 @@ class Opts(C.Structure):
         ("raw_output", C.c_int32), ("accumulate", C.c_int32),
         ("max_crossings", C.c_uint64), ("walk_variant", C.c_int32), ("drain_mode", C.c_int32),
     ]
+
+
+class RayOpts(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("flags", C.c_uint32), ("hubble_kms_per_cell", C.c_double), ("hubble_eps", C.c_double),
+                ("max_length_cells", C.c_double), ("n_v", C.c_int32), ("v_lo", C.c_double), ("v_hi", C.c_double)]
+
+
+RAYS_HOST = 0x1
+FIELDS = dict(nHI=0, T=1, vx=2, vy=3, vz=4, kdust=5)
 
 
 class Gridless(C.Structure):
@@ -83,6 +92,9 @@ def lib():
         L.thor_last_run_max_nscat.argtypes = [P, C.POINTER(C.c_ulonglong)]
         L.thor_raytrace.argtypes = [P, i64, P, P, d, i32, d, d, P, P, P]
         L.thor_volume_render.argtypes = [P, i64, P, P, i32, P, d, P]
+        L.thor_raytrace_ex.argtypes = [P, i64, P, P, C.POINTER(RayOpts), P, P, P]
+        L.thor_volume_render_ex.argtypes = [P, i64, P, P, i32, P, d, P, u32]
+        L.thor_slice.argtypes = [P, i64, P, i32, P, u32]
         L.thor_tally_get.argtypes = [P, i32, P, C.c_size_t, C.POINTER(C.c_size_t)]
         L.thor_last_error.argtypes = [P]
         L.thor_last_error.restype = C.c_char_p
@@ -216,36 +228,39 @@ class Context:
         _check(lib().thor_last_run_ms(self._ctx, C.byref(ms)), self._ctx)
         return ms.value
 
-    def raytrace(self, origins, dirs, n_v=0, v_lo=0.0, v_hi=1.0, hubble_kms_per_cell=0.0):
-        """Projection / absorption spectra along rays (thor_raytrace).  Returns dict(column, tmean[, tau])."""
-        import torch
-        org = torch.from_numpy(np.ascontiguousarray(origins, np.float32)).cuda()
-        dr = torch.from_numpy(np.ascontiguousarray(dirs, np.float32)).cuda()
+    def raytrace(self, origins, dirs, n_v=0, v_lo=0.0, v_hi=1.0, hubble_kms_per_cell=0.0, hubble_eps=0.0, max_length_cells=0.0):
+        """Projection / absorption spectra along rays (thor_raytrace_ex with HOST buffers: the library does the copies).
+        Returns dict(column, tmean[, tau])."""
+        org = np.ascontiguousarray(origins, np.float32).reshape(-1, 3)
+        dr = np.ascontiguousarray(dirs, np.float32).reshape(-1, 3)
         n = org.shape[0]
-        col = torch.empty(n, dtype=torch.float32, device="cuda")
-        tm = torch.empty(n, dtype=torch.float32, device="cuda")
-        tau = torch.empty((n, n_v), dtype=torch.float32, device="cuda") if n_v > 0 else None
-        _check(lib().thor_raytrace(self._ctx, n, C.c_void_p(org.data_ptr()), C.c_void_p(dr.data_ptr()),
-                                   float(hubble_kms_per_cell), int(n_v), float(v_lo), float(v_hi),
-                                   C.c_void_p(col.data_ptr()), C.c_void_p(tm.data_ptr()),
-                                   C.c_void_p(tau.data_ptr()) if tau is not None else None), self._ctx)
-        out = dict(column=col.cpu().numpy(), tmean=tm.cpu().numpy())
+        col, tm = np.empty(n, np.float32), np.empty(n, np.float32)
+        tau = np.empty((n, n_v), np.float32) if n_v > 0 else None
+        o = RayOpts(struct_size=C.sizeof(RayOpts), flags=RAYS_HOST, hubble_kms_per_cell=float(hubble_kms_per_cell),
+                    hubble_eps=float(hubble_eps), max_length_cells=float(max_length_cells), n_v=int(n_v), v_lo=float(v_lo), v_hi=float(v_hi))
+        p = lambda a: None if a is None else a.ctypes.data_as(C.c_void_p)
+        _check(lib().thor_raytrace_ex(self._ctx, n, p(org), p(dr), C.byref(o), p(col), p(tm), p(tau)), self._ctx)
+        out = dict(column=col, tmean=tm)
         if tau is not None:
-            out["tau"] = tau.cpu().numpy()
+            out["tau"] = tau
         return out
 
     def volume_render(self, origins, dirs, peaks, n_ref=0.0):
-        """Volume rendering along rays (thor_volume_render, Eq. 12).  Returns float32[n][4] = (C_R, C_G, C_B, opacity)."""
-        import torch
-        org = torch.from_numpy(np.ascontiguousarray(origins, np.float32)).cuda()
-        dr = torch.from_numpy(np.ascontiguousarray(dirs, np.float32)).cuda()
+        """Volume rendering along rays (thor_volume_render_ex, Eq. 12; HOST buffers).  Returns float32[n][4] = (C_R, C_G, C_B, opacity)."""
+        org = np.ascontiguousarray(origins, np.float32).reshape(-1, 3)
+        dr = np.ascontiguousarray(dirs, np.float32).reshape(-1, 3)
         pk = np.ascontiguousarray(peaks, np.float32).reshape(-1, 6)
-        n = org.shape[0]
-        out = torch.empty((n, 4), dtype=torch.float32, device="cuda")
-        _check(lib().thor_volume_render(self._ctx, n, C.c_void_p(org.data_ptr()), C.c_void_p(dr.data_ptr()),
-                                        pk.shape[0], pk.ctypes.data_as(C.c_void_p), float(n_ref),
-                                        C.c_void_p(out.data_ptr())), self._ctx)
-        return out.cpu().numpy()
+        out = np.empty((org.shape[0], 4), np.float32)
+        p = lambda a: a.ctypes.data_as(C.c_void_p)
+        _check(lib().thor_volume_render_ex(self._ctx, org.shape[0], p(org), p(dr), pk.shape[0], p(pk), float(n_ref), p(out), RAYS_HOST), self._ctx)
+        return out
+
+    def slice(self, points, field):
+        """Slice operator (thor_slice): the value of `field` ('nHI', 'T', 'vx', 'vy', 'vz', 'kdust') in the cell holding each point."""
+        pts = np.ascontiguousarray(points, np.float32).reshape(-1, 3)
+        out = np.empty(pts.shape[0], np.float32)
+        _check(lib().thor_slice(self._ctx, pts.shape[0], pts.ctypes.data_as(C.c_void_p), FIELDS[field], out.ctypes.data_as(C.c_void_p), RAYS_HOST), self._ctx)
+        return out
 
     def last_run_max_nscat(self):
         n = C.c_ulonglong()

@@ -133,3 +133,79 @@ def test_marcher_degenerate_rays(thor, oracle):
         assert np.allclose(g["tau"], o["tau"], rtol=5e-4, atol=1e-7 * o["tau"].max())
         assert np.allclose(gv, ov, rtol=2e-4, atol=1e-6)
         assert (o["column"] == 0).any() and (o["column"] > 0).any()      # outward rays from a corner see nothing
+
+
+# ---------------------------------------------------------------- round 2: forest sight lines, slices, thin renders
+@pytest.mark.parametrize("pack", [False, True])
+def test_periodic_subsampled_sightlines_parity(thor, oracle, pack):
+    """sight lines through the periodic box, wrapping at the faces up to a stated length, Eq. 11 sub-sampled so
+    that a step shifts the line by <= 0.25 v_th — against the oracle's orc_raytrace_ex on the same rays."""
+    n = 32
+    w = W.cosmic_web(n=n, n_src=16, n_photons=1, mean_n=3e-9, map_pix=8)
+    grid = dict(w["grid"], periodic=(1, 1, 1), T=(w["grid"]["T"] * 0.02).astype(np.float32))     # ~200 K: H_c ~ 1.3 v_th per cell
+    org, dirs = W.random_rays(1500, (n, n, n), seed=8)
+    hc = w["opts"]["hubble_kms_per_cell"]
+    ctx = thor.Context.from_workload(grid, pack=pack)
+    try:
+        g = ctx.raytrace(org, dirs, n_v=40, v_lo=-100.0, v_hi=400.0, hubble_kms_per_cell=hc, hubble_eps=0.25, max_length_cells=2.5 * n)
+        g1 = ctx.raytrace(org, dirs, n_v=40, v_lo=-100.0, v_hi=400.0, hubble_kms_per_cell=hc, hubble_eps=0.0, max_length_cells=2.5 * n)
+    finally:
+        ctx.close()
+    o = oracle.raytrace_ex(grid, org, dirs, 40, -100.0, 400.0, hc, 0.25, 2.5 * n)
+    rel = np.abs(g["column"] - o["column"]) / o["column"]
+    assert np.quantile(rel, 0.999) < 3e-5 and rel.max() < 1e-2
+    scale = o["tau"].max(axis=1, keepdims=True) + 1e-30
+    err = np.abs(g["tau"] - o["tau"]) / scale
+    assert np.quantile(err, 0.999) < 1e-4 and err.max() < 1e-2
+    # every ray went the full 2.5 box lengths: columns well above any single crossing of the box
+    single = oracle.raytrace(dict(grid, periodic=(0, 0, 0)), org, dirs)["column"]
+    assert np.all(o["column"] > single * (1 - 1e-9)) and np.median(o["column"] / single) > 2.0
+    # and the sub-sampling matters at this temperature: one midpoint per segment is off by far more than the parity bar
+    assert (np.abs(g1["tau"] - o["tau"]) / scale).max() > 1e-2
+
+
+def test_slice_and_host_buffers(thor, oracle):
+    """Slice operator = plain lookup, exact; and the HOST-buffer flag of the ray operators gives the very
+    bits the DEVICE-pointer entry points give."""
+    import ctypes as C
+    import torch
+    w = W.turbulent_box(n=24, n_src=16, n_photons=1, peel_pix=4, peel_bins=4)
+    grid = dict(w["grid"], kdust=(w["grid"]["nHI"] * 1e-20).astype(np.float32))
+    rng = np.random.default_rng(2)
+    pts = (rng.random((5000, 3)) * 24).astype(np.float32)
+    org, dirs = W.random_rays(800, (24, 24, 24), seed=4)
+    for pack in (False, True):
+        ctx = thor.Context.from_workload(grid, pack=pack)
+        try:
+            for f in ("nHI", "T", "vx", "vy", "vz", "kdust"):
+                assert np.array_equal(ctx.slice(pts, f).astype(np.float64), oracle.slice_field(grid, pts, f)), (f, pack)
+            host = ctx.raytrace(org, dirs, n_v=8, v_lo=-50.0, v_hi=50.0)
+            d = lambda a: torch.from_numpy(a).cuda()
+            o_, d_ = d(org), d(dirs)
+            col, tau = torch.empty(800, device="cuda"), torch.empty((800, 8), device="cuda")
+            p = lambda t: C.c_void_p(t.data_ptr())
+            assert thor.lib().thor_raytrace(ctx._ctx, 800, p(o_), p(d_), 0.0, 8, -50.0, 50.0, p(col), None, p(tau)) == 0
+            assert np.array_equal(col.cpu().numpy(), host["column"]) and np.array_equal(tau.cpu().numpy(), host["tau"])
+        finally:
+            ctx.close()
+
+
+def test_volume_render_thin_regime(thor, oracle):
+    """Optically thin renders (total tau 1e-4 ... 1e-2, per-segment mu l down to 1e-6): 1 - e^{-y} must not be formed by
+    subtracting an approximate exponential from one: colour and opacity agree with the fp64 oracle to 1e-4."""
+    n = 48
+    w = W.cosmic_web(n=n, n_src=16, n_photons=1, mean_n=1e-9, map_pix=8)
+    org, dirs = W.random_rays(3000, (n, n, n), seed=6)
+    peaks = TF_PEAKS.copy()
+    peaks[:, 5] *= 2e-4                                   # amplitudes: tau per cell ~1e-6 ... 1e-4
+    ctx = thor.Context.from_workload(w["grid"])
+    try:
+        g = ctx.volume_render(org, dirs, peaks).astype(np.float64)
+    finally:
+        ctx.close()
+    o = oracle.volume_render(w["grid"], org, dirs, peaks)
+    assert 1e-5 < np.median(o[:, 3]) < 1e-2
+    sel = o[:, 3] > 1e-6
+    rel = np.abs(g[sel] - o[sel]) / np.maximum(np.abs(o[sel]), 1e-12)
+    assert np.quantile(rel[:, 3], 0.999) < 1e-4, np.quantile(rel[:, 3], 0.999)
+    assert np.quantile(rel[:, :3], 0.999) < 1e-4
