@@ -89,6 +89,8 @@ void orc_sample_mu(int phase, uint64_t seed, uint64_t id, int64_t n, double* out
     for (int64_t i = 0; i < n; ++i) out[i] = sample_mu(phase, s, nullptr);
 }
 double orc_dipole_mu(double r) { return dipole_mu(r); }
+double orc_hg_mu(double g, double r) { return hg_mu(g, r); }
+double orc_hg_value(double g, double mu) { return hg_value(g, mu); }
 
 // One full scattering at gas-frame x_in for direction k_in = +z: returns x_out and k_out (for pins P9/P10).
 void orc_scatter_once(double a, double x_in, double x_crit, int phase, uint64_t seed, uint64_t id, int64_t n,
@@ -140,9 +142,12 @@ struct orc_opts_c {
     int32_t peel_nx, peel_ny, peel_nv;
     double peel_v_lo, peel_v_hi, peel_width_cells, tau_peel_max;
     uint64_t photon_id_offset, max_scatter, max_crossings;
+    double dust_albedo, dust_g;
+    int32_t doublet_on;
+    double doublet_dv_kms, doublet_sigma_ratio, doublet_a_ratio;
 };
 
-// Outputs (any may be NULL): spectrum u64[spec_bins+2], nscat_hist u64[64], counters u64[9],
+// Outputs (any may be NULL): spectrum u64[spec_bins+2], nscat_hist u64[64], counters u64[10],
 // cube f64[peel_ny*peel_nx*peel_nv], raw: RawRecord[n_photons] (24 bytes each).  Returns seconds of wall time
 // spent in the walk itself.
 double orc_run(int nx, int ny, int nz, int px, int py, int pz, double cell_cm,
@@ -164,6 +169,8 @@ double orc_run(int nx, int ny, int nz, int px, int py, int pz, double cell_cm,
     o.peel_v_lo = oc->peel_v_lo; o.peel_v_hi = oc->peel_v_hi; o.peel_width_cells = oc->peel_width_cells;
     o.tau_peel_max = oc->tau_peel_max;
     o.photon_id_offset = oc->photon_id_offset; o.max_scatter = oc->max_scatter; o.max_crossings = oc->max_crossings;
+    o.dust_albedo = oc->dust_albedo; o.dust_g = oc->dust_g; o.doublet_on = oc->doublet_on;
+    o.doublet_dv_kms = oc->doublet_dv_kms; o.doublet_sigma_ratio = oc->doublet_sigma_ratio; o.doublet_a_ratio = oc->doublet_a_ratio;
     Walker w(g, s, o);
     Result res;
     const auto t0 = std::chrono::steady_clock::now();
@@ -191,6 +198,7 @@ double orc_run_gridless(int geometry, double r_in, double r_out, double length_c
     o.spec_mode = oc->spec_mode; o.spec_T_ref = oc->spec_T_ref; o.spec_bins = oc->spec_bins;
     o.spec_lo = oc->spec_lo; o.spec_hi = oc->spec_hi; o.v_max_kms = oc->v_max_kms;
     o.photon_id_offset = oc->photon_id_offset; o.max_scatter = oc->max_scatter; o.max_crossings = oc->max_crossings;
+    o.dust_albedo = oc->dust_albedo; o.dust_g = oc->dust_g;
     GridlessWalker w(d, s, o);
     Result res;
     const auto t0 = std::chrono::steady_clock::now();

@@ -192,7 +192,23 @@ private:
             if (done) break;
             if (d_.kdust0 > 0.0) {                               // dust with probability kappa_dust / kappa_total
                 const double rr = rng.uniform();
-                if (rr * (k_line + k_dust) < k_dust) { status = ST_ABSORBED; break; }
+                if (rr * (k_line + k_dust) < k_dust) {
+                    // PAPER.md 2.3.2: scattered with probability albedo (Eq. 8; Henyey-Greenstein, Eq. 9), else destroyed
+                    if (!(o_.dust_albedo > 0.0) || !(rng.uniform() < o_.dust_albedo)) { status = ST_ABSORBED; break; }
+                    const double mu = hg_mu(o_.dust_g, rng.uniform());
+                    const double phi = 2.0 * PI * rng.uniform();
+                    double e1[3], e2[3];
+                    ortho_basis(k, e1, e2);
+                    const double vk0 = dot3(gs.v, k);
+                    const double st = std::sqrt(std::fmax(0.0, 1.0 - mu * mu));
+                    double kn[3];
+                    for (int i = 0; i < 3; ++i) kn[i] = mu * k[i] + st * (std::cos(phi) * e1[i] + std::sin(phi) * e2[i]);
+                    const double nrm = 1.0 / std::sqrt(dot3(kn, kn));
+                    for (int i = 0; i < 3; ++i) k[i] = kn[i] * nrm;
+                    V = V - vk0 + dot3(gs.v, k);                 // coherent in the bulk frame of the step's gas (A33)
+                    res.counters[CT_DUST_SCATTERINGS]++;
+                    continue;
+                }
             }
             // ---- resonant scattering in the gas of the step (PAPER.md 2.3.1), as in walker.hpp step 5
             const double vk = dot3(gs.v, k);

@@ -134,6 +134,16 @@ inline double sample_mu(int phase, DrawStream& rng, int* used_dipole) {
     return ph == PHASE_DIPOLE ? dipole_mu(r) : 2.0 * r - 1.0;
 }
 
+// Henyey-Greenstein phase function of dust scattering, Eq. 9: P_HG(mu) = (1/2)(1 - g^2)/(1 + g^2 - 2 g mu)^(3/2),
+// g = <mu>.  Its CDF inverts in closed form: mu = (1 + g^2 - ((1 - g^2)/(1 - g + 2 g r))^2) / (2 g); isotropic for g = 0.
+inline double hg_mu(double g, double r) {
+    if (std::fabs(g) < 1e-6) return 2.0 * r - 1.0;
+    const double q = (1.0 - g * g) / (1.0 - g + 2.0 * g * r);
+    return (1.0 + g * g - q * q) / (2.0 * g);
+}
+// 2 P_HG(mu): the phase function normalised so that isotropic scattering gives 1 (the convention of phase_value below).
+inline double hg_value(double g, double mu) { return (1.0 - g * g) / std::pow(1.0 + g * g - 2.0 * g * mu, 1.5); }
+
 // Normalised phase function toward a fixed direction, for peel-off: P^(mu) = 1 or 3/4 (1 + mu^2).
 inline double phase_value(int resolved_dipole, double mu) { return resolved_dipole ? 0.75 * (1.0 + mu * mu) : 1.0; }
 

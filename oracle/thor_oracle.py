@@ -39,6 +39,8 @@ class _Opts(C.Structure):
         ("peel_v_lo", C.c_double), ("peel_v_hi", C.c_double), ("peel_width_cells", C.c_double),
         ("tau_peel_max", C.c_double),
         ("photon_id_offset", C.c_uint64), ("max_scatter", C.c_uint64), ("max_crossings", C.c_uint64),
+        ("dust_albedo", C.c_double), ("dust_g", C.c_double), ("doublet_on", C.c_int32),
+        ("doublet_dv_kms", C.c_double), ("doublet_sigma_ratio", C.c_double), ("doublet_a_ratio", C.c_double),
     ]
 
 
@@ -48,11 +50,12 @@ OPT_DEFAULTS = dict(
     hubble_kms_per_cell=0.0, hubble_eps=0.25, v_max_kms=0.0,
     peel_on=0, k_obs=(0.0, 0.0, 1.0), peel_nx=0, peel_ny=0, peel_nv=0, peel_v_lo=0.0, peel_v_hi=1.0,
     peel_width_cells=0.0, tau_peel_max=30.0, photon_id_offset=0, max_scatter=0, max_crossings=0,
+    dust_albedo=0.0, dust_g=0.0, doublet_on=0, doublet_dv_kms=0.0, doublet_sigma_ratio=0.0, doublet_a_ratio=1.0,
 )
 
 RAW_DTYPE = np.dtype([("V", "<f4"), ("nscat", "<u4"), ("status", "<i4"), ("kx", "<f4"), ("ky", "<f4"), ("kz", "<f4")])
 COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "cell_crossings", "rejection_iters",
-                 "peel_rays", "peel_cells"]
+                 "peel_rays", "peel_cells", "dust_scatterings"]
 
 _lib = None
 
@@ -83,6 +86,10 @@ def lib():
         L.orc_sample_mu.argtypes = [i32, u64, u64, i64, P]
         L.orc_dipole_mu.restype = d
         L.orc_dipole_mu.argtypes = [d]
+        L.orc_hg_mu.restype = d
+        L.orc_hg_mu.argtypes = [d, d]
+        L.orc_hg_value.restype = d
+        L.orc_hg_value.argtypes = [d, d]
         L.orc_scatter_once.argtypes = [d, d, d, i32, u64, u64, i64, P, P]
         L.orc_dda_trace.argtypes = [i32] * 6 + [i64, P, P, i64, i32, P, P, P, P, P]
         L.orc_raytrace.restype = None
@@ -112,6 +119,8 @@ def x_cw_b25(a): return lib().orc_x_cw_b25(float(a))
 def upar_pdf(a, x, u): return lib().orc_upar_pdf(float(a), float(x), float(u))
 def upar_u0(a, x): return lib().orc_upar_u0(float(a), float(x))
 def dipole_mu(r): return lib().orc_dipole_mu(float(r))
+def hg_mu(g, r): return lib().orc_hg_mu(float(g), float(r))
+def hg_value(g, mu): return lib().orc_hg_value(float(g), float(mu))
 def u32_to_uniform(r): return lib().orc_u32_to_uniform(int(r))
 
 
@@ -209,7 +218,7 @@ def run(grid, sources, opts, n_photons, seed, want_raw=True):
             setattr(oc, k, v)
     spectrum = np.zeros(o["spec_bins"] + 2, np.uint64)
     hist = np.zeros(64, np.uint64)
-    counters = np.zeros(9, np.uint64)
+    counters = np.zeros(len(COUNTER_NAMES), np.uint64)
     cube = np.zeros((o["peel_ny"], o["peel_nx"], o["peel_nv"]), np.float64) if o["peel_on"] else None
     raw = np.zeros(n_photons, RAW_DTYPE) if want_raw else None
     per = grid.get("periodic", (0, 0, 0))
@@ -255,7 +264,7 @@ def run_gridless(dataset, sources, opts, n_photons, seed, want_raw=True):
     o, oc = _opts_struct(opts)
     spectrum = np.zeros(o["spec_bins"] + 2, np.uint64)
     hist = np.zeros(64, np.uint64)
-    counters = np.zeros(9, np.uint64)
+    counters = np.zeros(len(COUNTER_NAMES), np.uint64)
     raw = np.zeros(n_photons, RAW_DTYPE) if want_raw else None
     secs = lib().orc_run_gridless(int(dd["geometry"]), *(float(dd[k]) for k in ("r_in", "r_out", "length_cm", "n0", "alpha_rho", "T",
                                                                                   "v_max", "alpha_v", "kdust0", "step_f")),

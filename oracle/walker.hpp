@@ -56,7 +56,7 @@ struct Sources {
 
 enum Status { ST_ESCAPED = 0, ST_ABSORBED = 1, ST_TERMINATED = 2, ST_CAPPED = 3 };
 enum Counter { CT_ESCAPED = 0, CT_ABSORBED, CT_TERMINATED, CT_CAPPED, CT_SCATTERINGS, CT_CROSSINGS, CT_REJ_ITERS,
-               CT_PEEL_RAYS, CT_PEEL_CELLS, CT_COUNT };
+               CT_PEEL_RAYS, CT_PEEL_CELLS, CT_DUST_SCATTERINGS, CT_COUNT };
 
 struct Opts {
     int phase_core = PHASE_ISOTROPIC, phase_wing = PHASE_ISOTROPIC;
@@ -80,6 +80,13 @@ struct Opts {
     uint64_t photon_id_offset = 0;
     uint64_t max_scatter = 0;       // 0 = no cap
     uint64_t max_crossings = 0;     // cap on cell crossings per packet; 0 = the built-in limit 2^32 - 1 (reading A26)
+    // dust scattering (PAPER.md 2.3.2, Eq. 8-9): with albedo > 0 kdust is the dust EXTINCTION coefficient; an interaction
+    // with dust scatters with probability albedo (Henyey-Greenstein, asymmetry g), else absorbs (reading A32)
+    double dust_albedo = 0.0, dust_g = 0.0;
+    // doublet: a second transition of the same species, its line centre dv km/s from the first, with
+    // sigma_0 and a scaled by the two ratios; cross-sections add, a scattering happens in ONE line (reading A34)
+    int doublet_on = 0;
+    double doublet_dv_kms = 0.0, doublet_sigma_ratio = 0.0, doublet_a_ratio = 1.0;
 };
 
 struct RawRecord { float V; uint32_t nscat; int32_t status; float kx, ky, kz; };
@@ -113,16 +120,25 @@ inline double kappa_line(const Grid& g, const CellProps& p, double V, const doub
     return p.n * sigma0_cm2(p.T) * voigt_H(voigt_a(p.T), x) * g.cell_cm;
 }
 
+// The doublet's second line (reading A34): centre at dv, sigma_0 and a scaled by the ratios.
+struct Doublet { bool on; double dv, rs, ra; };
+inline double kappa_line2(const Grid& g, const CellProps& p, double V, const double k[3], const Doublet& d) {
+    if (!d.on || p.n <= 0.0) return 0.0;
+    const double vth = vth_kms(p.T);
+    const double x = (V - d.dv - dot3(p.v, k)) / vth;
+    return p.n * sigma0_cm2(p.T) * d.rs * voigt_H(voigt_a(p.T) * d.ra, x) * g.cell_cm;
+}
+
 // Optical depth of one segment of length len (cell units) starting at velocity offset V0, or the distance at
 // which tau_need is reached.  Without Hubble drift this is kappa * len (piecewise-constant cells).
 // With drift (V falls by Hc per cell length), sub-cell stepping per reading A12: n_sub = 1 if
 // min|x| over the segment > 6, else ceil(|dV| / (eps v_th)); midpoint rule; interaction site linear in the
 // sub-step.  Returns true on interaction; then s_hit = distance, kappa_hit_* = opacities at the site.
-struct SegmentOut { double tau; bool hit; double s_hit; double k_line, k_dust; };
+struct SegmentOut { double tau; bool hit; double s_hit; double k_line, k_dust, k_line2; };
 
 inline SegmentOut integrate_segment(const Grid& g, const CellProps& p, double V0, const double k[3], double len,
-                                    double tau_need, double Hc, double eps) {
-    SegmentOut o{0.0, false, 0.0, 0.0, 0.0};
+                                    double tau_need, double Hc, double eps, const Doublet& db = Doublet{false, 0, 0, 1}) {
+    SegmentOut o{0.0, false, 0.0, 0.0, 0.0, 0.0};
     const double kdust = p.kd * g.cell_cm;
     o.k_dust = kdust;
     if (p.n <= 0.0 && kdust <= 0.0) return o;
@@ -141,13 +157,15 @@ inline SegmentOut integrate_segment(const Grid& g, const CellProps& p, double V0
     for (int j = 0; j < nsub; ++j) {
         const double Vmid = Hc != 0.0 ? V0 - Hc * (j + 0.5) * ds : V0;   // no 0 * inf when ds = +inf (reading A24)
         const double kl = kappa_line(g, p, Vmid, k);
-        const double kt = kl + kdust;
+        const double kl2 = kappa_line2(g, p, Vmid, k, db);
+        const double kt = kl + kl2 + kdust;
         const double dtau = kt * ds;
         if (o.tau + dtau >= tau_need && kt > 0.0) {
             o.hit = true;
             o.s_hit = (j ? j * ds : 0.0) + (tau_need - o.tau) / kt;       // linear within the step
             if (o.s_hit > len) o.s_hit = len;
             o.k_line = kl;
+            o.k_line2 = kl2;
             o.tau = tau_need;
             return o;
         }
@@ -174,7 +192,8 @@ inline void ortho_basis(const double k[3], double e1[3], double e2[3]) {
 
 class Walker {
 public:
-    Walker(const Grid& g, Sources& s, const Opts& o) : g_(g), s_(s), o_(o) {
+    Walker(const Grid& g, Sources& s, const Opts& o) : g_(g), s_(s), o_(o),
+        db_{o.doublet_on != 0, o.doublet_dv_kms, o.doublet_sigma_ratio, o.doublet_a_ratio} {
         s_.prepare();
         if (o_.peel_on) {
             double n2 = dot3(o_.k_obs, o_.k_obs);
@@ -207,6 +226,7 @@ private:
     Sources& s_;
     Opts o_;
     double kobs_[3], img1_[3], img2_[3];
+    Doublet db_;
 
     // Step 6: contribution escaping toward the observer from position (ray cell/offset) at
     // velocity offset V_o with phase weight P^:  w = P^ exp(-tau_obs), tau_obs integrated along k_obs to the box
@@ -228,7 +248,7 @@ private:
             const int ex = dda_next_face(r, g_.dims, len);
             if (std::isinf(len)) return;                      // reading A24: never reaches a box face -> dropped
             const CellProps cp = fetch_cell(g_, r.c);
-            const SegmentOut so = integrate_segment(g_, cp, V, kobs_, len, 1e300, o_.hubble_kms_per_cell, o_.hubble_eps);
+            const SegmentOut so = integrate_segment(g_, cp, V, kobs_, len, 1e300, o_.hubble_kms_per_cell, o_.hubble_eps, db_);
             tau += so.tau;
             V -= o_.hubble_kms_per_cell * len;
             res.counters[CT_PEEL_CELLS]++;
@@ -285,7 +305,7 @@ private:
                 double len;
                 const int ex = dda_next_face(ray, g_.dims, len);
                 cp = fetch_cell(g_, ray.c);
-                so = integrate_segment(g_, cp, V, k, len, tau_target - tau_acc, Hc, o_.hubble_eps);
+                so = integrate_segment(g_, cp, V, k, len, tau_target - tau_acc, Hc, o_.hubble_eps, db_);
                 if (so.hit) {
                     dda_advance_within(ray, g_.dims, so.s_hit);
                     if (Hc != 0.0) V -= Hc * so.s_hit;
@@ -302,21 +322,44 @@ private:
                 if (++ncross >= cross_cap) { status = ST_CAPPED; done = true; break; }
             }
             if (done) break;
-            // ---- Step 4: which interaction: dust with probability kappa_dust / kappa_total.
-            if (g_.kdust) {
+            // ---- Step 4: which interaction: interaction i with probability tau_i / tau — dust, line 1, line 2.
+            int line = 0;
+            if (g_.kdust || db_.on) {
                 const double r = rng.uniform();
-                if (r * (so.k_line + so.k_dust) < so.k_dust) { status = ST_ABSORBED; break; }
+                const double kt = so.k_line + so.k_line2 + so.k_dust;
+                if (r * kt < so.k_dust) {
+                    // dust (PAPER.md 2.3.2): scattered with probability albedo (Eq. 8), else destroyed
+                    if (!(o_.dust_albedo > 0.0) || !(rng.uniform() < o_.dust_albedo)) { status = ST_ABSORBED; break; }
+                    const double mu = hg_mu(o_.dust_g, rng.uniform());          // Eq. 9
+                    const double phi = 2.0 * PI * rng.uniform();
+                    double e1[3], e2[3];
+                    ortho_basis(k, e1, e2);
+                    const double vk = dot3(cp.v, k);
+                    // grains move with the gas and are heavy: the frequency is unchanged in the cell's bulk frame (A33)
+                    if (o_.peel_on) peel(ray, V - vk + dot3(cp.v, kobs_), hg_value(o_.dust_g, dot3(k, kobs_)), res);
+                    const double st = std::sqrt(std::fmax(0.0, 1.0 - mu * mu));
+                    double kn[3];
+                    for (int i = 0; i < 3; ++i) kn[i] = mu * k[i] + st * (std::cos(phi) * e1[i] + std::sin(phi) * e2[i]);
+                    const double nrm = 1.0 / std::sqrt(dot3(kn, kn));
+                    for (int i = 0; i < 3; ++i) k[i] = kn[i] * nrm;
+                    ray.set_direction(k);
+                    V = V - vk + dot3(cp.v, k);
+                    res.counters[CT_DUST_SCATTERINGS]++;
+                    continue;
+                }
+                if (db_.on && r * kt >= so.k_dust + so.k_line) line = 1;
             }
-            // ---- Step 5: resonant scattering (§2.3.1).
+            // ---- Step 5: resonant scattering (§2.3.1) in the chosen line: frequencies relative to ITS centre.
+            const double dv_line = line ? db_.dv : 0.0;
             const double vth = vth_kms(cp.T);
-            const double a = voigt_a(cp.T);
+            const double a = voigt_a(cp.T) * (line ? db_.ra : 1.0);
             const double vk = dot3(cp.v, k);
-            const double x_in = (V - vk) / vth;
+            const double x_in = (V - dv_line - vk) / vth;
             const double upar = sample_upar(a, x_in, rng, &res.counters[CT_REJ_ITERS]);
             double x_crit = 0.0;
             if (o_.core_skip_mode == 1) x_crit = o_.x_crit;
             else if (o_.core_skip_mode == 2) {
-                const double atau = a * cp.n * sigma0_cm2(cp.T) * g_.cell_cm * 0.5;
+                const double atau = a * cp.n * sigma0_cm2(cp.T) * (line ? db_.rs : 1.0) * g_.cell_cm * 0.5;
                 x_crit = atau >= 1.0 ? 0.2 * std::cbrt(atau) : 0.0;
             }
             double up1, up2;
@@ -331,7 +374,7 @@ private:
             if (o_.peel_on) {
                 const double mu_o = dot3(k, kobs_);
                 const double x_o = x_in - upar + upar * mu_o + up1 * dot3(e1, kobs_) + up2 * dot3(e2, kobs_);
-                peel(ray, x_o * vth + dot3(cp.v, kobs_), phase_value(is_dipole, mu_o), res);
+                peel(ray, x_o * vth + dot3(cp.v, kobs_) + dv_line, phase_value(is_dipole, mu_o), res);
             }
             const double st = std::sqrt(std::fmax(0.0, 1.0 - mu * mu));
             const double cph = std::cos(phi), sph = std::sin(phi);
@@ -343,7 +386,7 @@ private:
             const double x_out = x_in - upar + upar * mu + st * (up1 * cph + up2 * sph);
             for (int i = 0; i < 3; ++i) k[i] = kn[i];
             ray.set_direction(k);
-            V = x_out * vth + dot3(cp.v, k);
+            V = x_out * vth + dot3(cp.v, k) + dv_line;
             ++nscat;
             res.counters[CT_SCATTERINGS]++;
             if (o_.v_max_kms > 0 && std::fabs(V) > o_.v_max_kms) { status = ST_TERMINATED; break; }
