@@ -71,6 +71,14 @@ def make_workload(name, n_photons=None, device="cuda"):
         note = dict(scaled_from="configs[0]: tau0 1e5 -> 1e4, 1e3 -> 1e6 packets")
     elif name == "slab":     # configs[2] as stated
         w = W.static_slab(n_photons=1_000_000)
+    elif name == "neufeld":  # the paper's own benchmark problem (Table 2): homogeneous static sphere, tau0 = 1e6,
+        # T = 2e4 K, 2e5 packets injected at line centre, no core-skipping — on the gridless dataset the paper uses
+        T, tau0 = 2e4, 1e6
+        w = dict(name="neufeld_sphere_gridless_tau1e6", n_photons=200_000, seed=1,
+                 dataset=dict(geometry=0, r_in=0.0, r_out=1.0, length_cm=W.PC_CM, T=T,
+                              n0=tau0 / (W.RECIPE_SIGMA0_T4 / (T / 1e4) ** 0.5 * W.PC_CM)),
+                 sources=dict(pos=np.zeros((1, 3), np.float32), lum=np.ones(1, np.float32), sigma=np.zeros(1, np.float32)),
+                 opts=dict(phase_core=0, phase_wing=0, spec_mode=0, spec_T_ref=T, spec_bins=400, spec_lo=-60.0, spec_hi=60.0))
     elif name == "gather":   # the cell-gather regime: configs[4]'s recipe at 512^3 made optically thin (mean n_HI 1e-11), so
         # packets stream through ~340 cells each and the walk is bound by the HBM gathers, not by scatterings
         w = W.cosmic_web(n=512, n_src=1 << 16, n_photons=4_000_000, map_pix=2048, mean_n=1e-11)
@@ -149,7 +157,11 @@ def _oracle_worker(args):
     secs = 0.0
     off = first
     while secs < budget_s:
-        r = thor_oracle.run(w["grid"], w["sources"], dict(w["opts"], photon_id_offset=off), chunk, w["seed"], want_raw=False)
+        o = dict(w["opts"], photon_id_offset=off)
+        if "dataset" in w:
+            r = thor_oracle.run_gridless(w["dataset"], w["sources"], o, chunk, w["seed"], want_raw=False)
+        else:
+            r = thor_oracle.run(w["grid"], w["sources"], o, chunk, w["seed"], want_raw=False)
         secs += r["seconds"]
         scat += r["counters"]["scatterings"]
         cross += r["counters"]["cell_crossings"]
@@ -232,7 +244,7 @@ def run_reference(args):
 
 def workload_label(name):
     return {"web1536": "cosmic_web_n1536", "web512": "cosmic_web_n512", "turb512": "turbulent_box_n512",
-            "shell": "expanding_shell_n128", "sphere": "static_sphere_n32_tau10000_T10", "slab": "static_slab_nz256_tau1e+07",
+            "shell": "expanding_shell_n128", "sphere": "static_sphere_n32_tau10000_T10", "slab": "static_slab_nz256_tau1e+07", "neufeld": "neufeld_sphere_gridless_tau1e6",
             "gather": "cosmic_web_n512_thin_gather"}.get(name, name)
 
 def run_operators(args):
@@ -374,7 +386,8 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
     n = w["n_photons"]
     opts = dict(w["opts"], raw_output=0)
     t_gen = time.perf_counter()
-    ctx = thor.Context.from_workload(w["grid"], pack=pack)         # fields resident in HBM before the timed region
+    gridless = "dataset" in w
+    ctx = thor.Context.gridless(**w["dataset"]) if gridless else thor.Context.from_workload(w["grid"], pack=pack, extra_flags=args.grid_flags)   # resident before the timed region
     ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     spec_dev = torch.zeros(opts["spec_bins"] + 2, dtype=torch.int64, device="cuda")
@@ -421,13 +434,13 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
     assert packets == n * world * steps, (packets, n, world, steps)
     secs = step_ms * 1e-3
     crossings = c["cell_crossings"] + c["peel_cells"]
-    g = w["grid"]
+    g = w.get("grid") or dict(nx=0, ny=0, nz=0)
     out = {
         "metric": "lya_scatterings_per_sec", "value": c["scatterings"] / secs, "unit": "scatterings/s",
         "packets_per_sec": packets / secs, "cell_crossings_per_sec": crossings / secs,
         "steps": steps, "warmup": warmup, "ms_per_step": step_ms / steps,
         "config": {"workload": workload_label(name), "grid": [g["nx"], g["ny"], g["nz"]], "n_photons_per_step_per_gpu": n,
-                   "layout": "packed 32 B/cell (THOR_GRID_PACK)" if pack else "SoA fp32, borrowed",
+                   "layout": "gridless (analytic sphere, fp64 geometry)" if gridless else "packed 32 B/cell (THOR_GRID_PACK)" if pack else "SoA fp32, borrowed",
                    "parallelism": f"photon-id shards x{world}, grid replicated",
                    "l2": "flushed between timed iterations (256 MB memset)",
                    "scatterings_per_packet": c["scatterings"] / packets,
@@ -481,7 +494,7 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
     # goes host -> device (thor_sources_set), the tallies come back device -> host (thor_tally_get), all inside the timed
     # region.  Small grids are re-created from host arrays each step as well; the 72.5 GB grid stays resident (dataset).
     if want_e2e:
-        regrid = not isinstance(g["nHI"], torch.Tensor)
+        regrid = not gridless and not isinstance(g["nHI"], torch.Tensor)
         src = w["sources"]
         h2d = sum(np.asarray(src[k]).nbytes for k in ("pos", "lum", "sigma"))
         if regrid:
@@ -541,6 +554,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-subs", action="store_true", help="skip the `workloads` sub-dict")
     ap.add_argument("--sub-steps", type=int, default=2)
+    ap.add_argument("--grid-flags", type=lambda v: int(v, 0), default=0, help="extra thor_grid_create flags (0x400 L2 persistence window, 0x800 32-byte L2 fetch granularity)")
     ap.add_argument("--pack", type=int, default=-1, help="THOR_GRID_PACK (1/0); default: on for the gather workload")
     args = ap.parse_args()
     if args.workload in ("project", "render"):

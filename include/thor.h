@@ -135,6 +135,15 @@ typedef struct thor_opts {
     int32_t drain_mode;               /* 0 (default): once the photon counter is dry, warps left with <= 4 packets hand them
                                          to the cooperative drain kernel; 1: the walk kernel finishes every
                                          packet itself.  Results do not depend on it */
+    double dust_albedo;               /* PAPER.md 2.3.2, Eq. 8: with albedo > 0 kdust is the dust EXTINCTION coefficient and an
+                                         interaction with dust scatters with this probability, else destroys (0: absorption
+                                         only, as before; the paper's fiducial value is 0.32) */
+    double dust_g;                    /* asymmetry g = <mu> of the Henyey-Greenstein phase function, Eq. 9 (fiducial 0.73) */
+    int32_t doublet_on;               /* a second transition of the same species: cross-sections add, each
+                                         scattering happens in one line, chosen with probability tau_i / tau */
+    double doublet_dv_kms;            /* its line centre, km/s from the first line's */
+    double doublet_sigma_ratio;       /* sigma_0 of line 2 / sigma_0 of line 1 (the ratio of oscillator strengths) */
+    double doublet_a_ratio;           /* Voigt parameter of line 2 / that of line 1 */
 } thor_opts;
 
 void thor_opts_default(thor_opts *o);
@@ -170,7 +179,8 @@ thor_status thor_last_run_max_nscat(const thor_ctx *ctx, unsigned long long *n);
 #define THOR_TALLY_DEVICE_DST 0x100 /* OR into kind: dst is a DEVICE pointer (CUBE then yields uint64 fixed point) */
 
 enum { THOR_CT_ESCAPED = 0, THOR_CT_ABSORBED, THOR_CT_TERMINATED, THOR_CT_CAPPED, THOR_CT_SCATTERINGS,
-       THOR_CT_CROSSINGS, THOR_CT_REJ_ITERS, THOR_CT_PEEL_RAYS, THOR_CT_PEEL_CELLS, THOR_N_COUNTERS };
+       THOR_CT_CROSSINGS, THOR_CT_REJ_ITERS, THOR_CT_PEEL_RAYS, THOR_CT_PEEL_CELLS, THOR_CT_DUST_SCATTERINGS,
+       THOR_N_COUNTERS };
 
 typedef struct thor_raw_record {
     float V;          /* lab-frame velocity offset from line centre at the end, km/s */

@@ -53,6 +53,7 @@ struct thor_ctx {
     thor::RawRecord* d_raw = nullptr;
     size_t raw_cap = 0;
     uint32_t* d_pool = nullptr;                 // parked packets for the drain kernel
+    unsigned int* d_pool_order = nullptr;
     // last run
     bool have_run = false;
     thor_opts last{};
@@ -99,6 +100,7 @@ extern "C" void thor_opts_default(thor_opts* o) {
     o->k_obs[2] = 1.0;
     o->peel_v_hi = 1.0;
     o->tau_peel_max = 30.0;
+    o->doublet_a_ratio = 1.0;
 }
 
 extern "C" void thor_grid_destroy(thor_ctx* ctx) {
@@ -113,6 +115,7 @@ extern "C" void thor_grid_destroy(thor_ctx* ctx) {
     if (ctx->d_cube) cudaFree(ctx->d_cube);
     if (ctx->d_raw) cudaFree(ctx->d_raw);
     if (ctx->d_pool) cudaFree(ctx->d_pool);
+    if (ctx->d_pool_order) cudaFree(ctx->d_pool_order);
     if (ctx->l2_persist) {                        // drop the access-policy window of the caller's stream
         cudaStreamAttrValue av{};
         cudaStreamSetAttribute(ctx->stream, cudaStreamAttributeAccessPolicyWindow, &av);
@@ -350,6 +353,9 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     if (o.spec_mode != 0 && o.spec_mode != 1) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_mode must be 0 or 1");
     if (o.spec_mode == 0 && !(o.spec_T_ref > 0)) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_T_ref must be > 0");
     if ((o.walk_variant != 0 && o.walk_variant != 3 && o.walk_variant != 4) || (o.drain_mode != 0 && o.drain_mode != 1)) return fail(ctx, THOR_ERR_ARG, "thor_run: bad walk_variant / drain_mode");
+    if (!(o.dust_albedo >= 0 && o.dust_albedo <= 1) || !(o.dust_g >= -1 && o.dust_g <= 1)) return fail(ctx, THOR_ERR_ARG, "thor_run: dust_albedo must be in [0, 1] and dust_g in [-1, 1]");
+    if (o.doublet_on && (!std::isfinite(o.doublet_dv_kms) || !(o.doublet_sigma_ratio >= 0) || !(o.doublet_a_ratio > 0) || !std::isfinite(o.doublet_sigma_ratio) || !std::isfinite(o.doublet_a_ratio)))
+        return fail(ctx, THOR_ERR_ARG, "thor_run: bad doublet options");
     if (!(o.hubble_eps > 0) || !(o.v_max_kms >= 0) || !std::isfinite(o.hubble_kms_per_cell)) return fail(ctx, THOR_ERR_ARG, "thor_run: bad Hubble / v_max options");
     // reading A26: on a grid periodic on all three axes nothing ends a packet in empty gas; without a crossing cap the
     // persistent kernel would never return (a fully frozen 1x1x1 grid has only infinite segments: reading A24 caps those)
@@ -367,8 +373,8 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     p.gl_geom = -1;
     if (ctx->gridless) {
         const thor_gridless& d = ctx->gl;
-        if (o.peel_on || o.hubble_kms_per_cell != 0 || o.core_skip_mode == 2)
-            return fail(ctx, THOR_ERR_UNSUPPORTED, "thor_run: peel-off, Hubble drift and local core-skipping need a grid dataset");
+        if (o.peel_on || o.hubble_kms_per_cell != 0 || o.core_skip_mode == 2 || o.doublet_on)
+            return fail(ctx, THOR_ERR_UNSUPPORTED, "thor_run: peel-off, Hubble drift, local core-skipping and doublets need a grid dataset");
         const double vth = K.c_vth * std::sqrt(d.T);
         // step limiter l_max = f min(l_v, l_rho) (reading A29)
         double lv = INFINITY, lrho = INFINITY;
@@ -428,10 +434,16 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     }
     p.id_offset = o.photon_id_offset; p.n_photons = n_photons; p.seed = seed; p.max_scatter = o.max_scatter;
     p.walk_variant = o.walk_variant;
+    p.dust_albedo = (float)o.dust_albedo; p.dust_g = (float)o.dust_g;
+    p.doublet_on = o.doublet_on ? 1 : 0;
+    p.db_dv = (float)o.doublet_dv_kms; p.db_rs = (float)o.doublet_sigma_ratio; p.db_ra = (float)o.doublet_a_ratio;
     CU(cudaSetDevice(ctx->device));
     if (o.drain_mode == 0 && !ctx->d_pool)
         CU(cudaMalloc(&ctx->d_pool, (size_t)thor::walk_pool_slots(ctx->n_sm) * thor::walk_pool_words() * sizeof(uint32_t)));
+    if (o.drain_mode == 0 && !ctx->d_pool_order)
+        CU(cudaMalloc(&ctx->d_pool_order, (size_t)thor::walk_pool_slots(ctx->n_sm) * sizeof(unsigned int)));
     p.pool = o.drain_mode == 0 ? ctx->d_pool : nullptr;
+    p.pool_order = ctx->d_pool_order;
     const bool keep = o.accumulate && ctx->have_run;
     if (cube_elems != ctx->cube_elems) {
         if (ctx->d_cube) { cudaFree(ctx->d_cube); ctx->d_cube = nullptr; }

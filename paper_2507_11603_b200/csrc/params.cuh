@@ -25,7 +25,7 @@ inline LyaConstants lya_constants() {
 }
 
 enum : int { CT_ESCAPED = 0, CT_ABSORBED, CT_TERMINATED, CT_CAPPED, CT_SCATTERINGS, CT_CROSSINGS, CT_REJ_ITERS,
-             CT_PEEL_RAYS, CT_PEEL_CELLS, N_COUNTERS };
+             CT_PEEL_RAYS, CT_PEEL_CELLS, CT_DUST_SCATTERINGS, N_COUNTERS };
 
 struct RawRecord { float V; uint32_t nscat; int32_t status; float kx, ky, kz; };
 
@@ -92,6 +92,7 @@ struct WalkParams {
     uint32_t* pool;                      // [slots][PK_WORDS] parked packet states, or nullptr = no drain kernel
     unsigned long long* pool_count;      // packets parked
     unsigned long long* pool_next;       // next slot to pop
+    unsigned int* pool_order;            // [slots]: pool slots by decreasing scattering count (longest first)
     // gridless dataset (PAPER.md 3.3: spherical shell / infinite slab with power-law density and velocity); gl_geom < 0 = grid
     int gl_geom;                         // -1 grid, 0 shell / sphere, 1 slab
     double gl_rin, gl_rout;              // length units
@@ -99,6 +100,10 @@ struct WalkParams {
     float gl_nsig0, gl_kd0;              // n0 sigma_0(T) length_cm and kdust0 length_cm: optical depths per length unit at r_out
     float gl_alpha_rho, gl_vmax, gl_alpha_v;
     float gl_a, gl_vth, gl_inv_vth;      // the one temperature of the dataset
+    // dust scattering (Eq. 8-9) and the doublet's second line
+    float dust_albedo, dust_g;
+    int doublet_on;
+    float db_dv, db_rs, db_ra;           // line 2: centre offset [km/s], sigma_0 ratio, a ratio
     int walk_variant;                    // 0 = by grid size, 3 / 4 = force the cache-resident / beyond-L2 kernel (tests)
 };
 

@@ -202,6 +202,18 @@ __device__ __forceinline__ float sample_mu(int phase, float r_mix, float r, floa
     return fminf(fmaxf(mu, -1.f), 1.f);
 }
 
+// Henyey-Greenstein phase function of dust scattering, Eq. 9, by closed-form inversion of its CDF:
+// mu = (1 + g^2 - ((1 - g^2) / (1 - g + 2 g r))^2) / (2 g); isotropic for g = 0.  hg_value = 2 P_HG (isotropic -> 1).
+__device__ __forceinline__ float hg_mu(float g, float r) {
+    if (fabsf(g) < 1e-6f) return fmaf(2.f, r, -1.f);
+    const float q = fmaf(-g, g, 1.f) / fmaf(2.f * g, r, 1.f - g);
+    return fminf(fmaxf(fmaf(-q, q, fmaf(g, g, 1.f)) / (2.f * g), -1.f), 1.f);
+}
+__device__ __forceinline__ float hg_value(float g, float mu) {
+    const float d = fmaf(-2.f * g, mu, fmaf(g, g, 1.f));
+    return fmaf(-g, g, 1.f) * rsqrtf(d) / d;
+}
+
 // Orthonormal basis (e1, e2) perpendicular to the unit vector k, branch-free (Duff et al. 2017 construction: with
 // sg = sign(kz), a = -1/(sg + kz), b = kx ky a:  e1 = (1 + sg kx^2 a, sg b, -sg kx),  e2 = (b, sg + ky^2 a, -ky)).
 // Any right-handed choice gives the same distribution of k' because the azimuth is uniform.

@@ -94,6 +94,7 @@ __device__ __forceinline__ void park_store(uint32_t* w, const Packet& k, int sta
     w[27] = __float_as_uint(k.x_in); w[28] = __float_as_uint(k.upar);
     w[29] = k.nscat; w[30] = k.crossings; w[31] = k.rej_iters; w[32] = k.trials;
     w[33] = (k.stale ? 1u : 0u) | (k.inv_ok ? 2u : 0u); w[34] = (uint32_t)state;
+    w[35] = __float_as_uint(k.hit_k2); w[42] = (uint32_t)k.line;
     if (GL) {
         const unsigned long long x = (unsigned long long)__double_as_longlong(k.gx), y = (unsigned long long)__double_as_longlong(k.gy),
                                  z = (unsigned long long)__double_as_longlong(k.gz);
@@ -116,6 +117,7 @@ __device__ __forceinline__ int park_load(const uint32_t* w, Packet& k) {
     k.x_in = __uint_as_float(w[27]); k.upar = __uint_as_float(w[28]);
     k.nscat = w[29]; k.crossings = w[30]; k.rej_iters = w[31]; k.trials = w[32];
     k.stale = (w[33] & 1u) != 0u; k.inv_ok = (w[33] & 2u) != 0u;
+    k.hit_k2 = __uint_as_float(w[35]); k.line = (int)w[42];
     if (GL) {
         k.gx = __longlong_as_double((long long)(((unsigned long long)w[37] << 32) | w[36]));
         k.gy = __longlong_as_double((long long)(((unsigned long long)w[39] << 32) | w[38]));
@@ -148,6 +150,22 @@ __device__ __forceinline__ void coop_fill_window(float4* win, const BlockRng& rn
     my_u = u; my_sC = q1.x; my_cC = q1.y;
 }
 
+// Longest first: a packet that has already scattered the most is the one most likely to go on the longest (the
+// scattering counts are heavy-tailed), and the launch ends when its longest packet does.  order[r] = the pool slot with the
+// r-th largest scattering count so far (ties by slot); one thread per slot, a scan of the pool's counts each.
+__global__ void pool_order_kernel(const __grid_constant__ WalkParams p) {
+    const unsigned long long n = *p.pool_count;
+    const unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t mine = p.pool[i * PK_WORDS + 29];          // word 29 = nscat (park_store)
+    unsigned int rank = 0;
+    for (unsigned long long j = 0; j < n; ++j) {
+        const uint32_t o = __ldg(p.pool + j * PK_WORDS + 29);
+        rank += (o > mine || (o == mine && j < i)) ? 1u : 0u;
+    }
+    p.pool_order[rank] = (unsigned int)i;
+}
+
 // The drain kernel: launched behind walk_kernel on the same stream.  Each warp pops one parked packet at a time from the
 // global pool and walks it to its end, all 32 lanes on that one packet (see above).  4 warps per CTA — one per SM
 // sub-partition — and a register budget of its own (the walk kernel is held to 80 registers by its occupancy).
@@ -165,13 +183,15 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
     const uint32_t k0 = (uint32_t)p.seed, k1 = (uint32_t)(p.seed >> 32);
     float4* win = s_win[threadIdx.x >> 5];
     const unsigned long long n_pool = *p.pool_count;
-    uint32_t pr = 0, pc = 0;
+    uint32_t pr = 0, pc = 0, ds = 0;
+    const int need0 = p.doublet_on ? 4 : 3;                   // blocks one scattering takes at least: [select,] trial, 2 x finish
     Packet k;
     for (;;) {
         unsigned long long slot = 0;
         if (lane == 0) slot = atomicAdd(p.pool_next, 1ull);
         slot = __shfl_sync(0xffffffffu, slot, 0);
         if (slot >= n_pool) break;
+        slot = p.pool_order[slot];
         int st = park_load<GL>(p.pool + slot * PK_WORDS, k);      // every lane reads the same words: one broadcast per load
         int c = 32;                                           // first unconsumed block of the window (32 = none left)
         float4 my_u = make_float4(0.f, 0.f, 0.f, 0.f);        // this lane's own block of the window
@@ -183,21 +203,28 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
                 const int ev = GL ? march_step_gridless(p, sh.voigt, k) : march_step<HUBBLE, false>(p, sh.voigt, k);
                 if (ev == EV_CROSSED) continue;
                 if (ev != EV_HIT) { if (lane == 0) tally_packet(p, sh, ev, k); break; }
-                st = LS_TRIAL;
+                st = p.doublet_on ? LS_SELECT : LS_TRIAL;
                 env.mTot = -1.f;
             }
-            if (c + 3 > 32) {                                 // fewer than a trial + a FINISH left: a new window
+            if (c + need0 > 32) {                                 // fewer than a trial + a FINISH left: a new window
                 __syncwarp();
                 coop_fill_window(win, k.rng, k0, k1, lane, my_u, my_sC, my_cC);
                 __syncwarp();
                 c = 0;
             }
+            if (st == LS_SELECT) {                            // doublet: which interaction, from one more block
+                const float4 u = win[5 * c];
+                ++c;
+                k.rng.b_lo += 1u; k.rng.b_hi += (k.rng.b_lo == 0u);
+                select_line(p, k, u.x);
+                st = k.line < 0 ? LS_FINISH : LS_TRIAL;
+            }
             if (st == LS_TRIAL) {
                 // every lane tries its OWN block; the packet takes the first acceptance at or after block c — exactly the
                 // trial the sequential rejection loop would have accepted, found in one step however many it rejects
-                if (env.mTot < 0.f) env = upar_envelope(k.cell.a, fabsf(k.x_in));
+                if (env.mTot < 0.f) env = upar_envelope(line_a(p, k), fabsf(k.x_in));
                 float uu;
-                const bool ok = upar_try<true>(env, k.cell.a, my_u, my_sC, my_cC, uu);
+                const bool ok = upar_try<true>(env, line_a(p, k), my_u, my_sC, my_cC, uu);
                 const unsigned acc = __ballot_sync(0xffffffffu, ok) & ~((1u << c) - 1u);
                 const uint32_t nrej = (uint32_t)((acc ? __ffs(acc) - 1 : 32) - c);   // rejections before the first acceptance
                 uint32_t ntr;                                 // blocks this step consumes
@@ -230,9 +257,10 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
                 FinDraws d;
                 d.tau_next = a1.z; d.r_mu = u1.y; d.mu_dip = a1.w;
                 d.sphi = a2.x; d.cphi = a2.y; d.nl_p1 = a2.z;
-                d.spsi = b3.x; d.cpsi = b3.y; d.u_dust = u2.y; d.u_mix = u2.z;
+                d.spsi = b3.x; d.cpsi = b3.y; d.u_dust = u2.y; d.u_mix = u2.z; d.u_alb = u2.w;
                 const int ev = finish_scatter<HUBBLE, PEEL, true>(p, sh.voigt, k, d, pr, pc, lane == 0);
-                if (ev != EV_SCATTERED) { if (lane == 0) tally_packet(p, sh, ev, k); break; }
+                if (ev == EV_DUST_SCATTERED) ++ds;
+                else if (ev != EV_SCATTERED) { if (lane == 0) tally_packet(p, sh, ev, k); break; }
                 st = LS_MARCH;
             }
         }
@@ -240,6 +268,7 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
     if (lane == 0) {
         atomicAdd(&sh.counters[CT_PEEL_RAYS], (unsigned long long)pr);
         atomicAdd(&sh.counters[CT_PEEL_CELLS], (unsigned long long)pc);
+        if (ds) atomicAdd(&sh.counters[CT_DUST_SCATTERINGS], (unsigned long long)ds);
     }
     __syncthreads();
     for (int i = threadIdx.x; i < N_COUNTERS; i += blockDim.x)
@@ -270,7 +299,7 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
     k.stale = true; k.inv_ok = false;
     UparEnvelope env;
     env.mTot = -1.f;
-    uint32_t peel_rays = 0, peel_cells = 0;
+    uint32_t peel_rays = 0, peel_cells = 0, dust_scat = 0;
     bool more = true;                                         // warp-uniform: photon counter not yet exhausted
 
     for (;;) {
@@ -322,8 +351,14 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
         // ---- a4-a7: one cell step for every marching lane ----
         if (state == LS_MARCH) {
             const int ev = GL ? march_step_gridless(p, sh.voigt, k) : march_step<HUBBLE, EARLY>(p, sh.voigt, k);
-            if (ev == EV_HIT) { env.mTot = -1.f; state = LS_TRIAL; }   // envelope not built yet
-            else if (ev != EV_CROSSED) { tally_packet(p, sh, ev, k); state = LS_IDLE; }
+            if (ev == EV_HIT) {
+                env.mTot = -1.f;                                  // envelope not built yet
+                state = LS_TRIAL;
+                if (p.doublet_on) {                               // which interaction: one more counter block
+                    select_line(p, k, k.rng.next4(k0, k1).x);
+                    if (k.line < 0) state = LS_FINISH;            // dust: no atom velocity to draw
+                }
+            } else if (ev != EV_CROSSED) { tally_packet(p, sh, ev, k); state = LS_IDLE; }
         }
 
         // ---- a8: ONE rejection trial of u_par for every lane that needs one.  No inner loop: a
@@ -331,10 +366,10 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
         // march, instead of the whole warp waiting for its slowest lane (the paper's "largest source of thread
         // divergence"; E[max of 32 iterations]/E[iterations] = 2.1-4.2) ----
         if (state == LS_TRIAL) {
-            if (env.mTot < 0.f) env = upar_envelope(k.cell.a, fabsf(k.x_in));
+            if (env.mTot < 0.f) env = upar_envelope(line_a(p, k), fabsf(k.x_in));
             ++k.rej_iters;
             float u;
-            const bool ok = upar_try<false>(env, k.cell.a, k.rng.next4(k0, k1), 0.f, 0.f, u);
+            const bool ok = upar_try<false>(env, line_a(p, k), k.rng.next4(k0, k1), 0.f, 0.f, u);
             // fail-safe: acceptance is >= ~0.2 everywhere; 2^20 rejections cannot happen unless x is NaN
             if (ok || ++k.trials >= (1u << 20)) { k.upar = k.x_in < 0.f ? -u : u; state = LS_FINISH; }
         }
@@ -352,6 +387,7 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
                 const FinDraws d = fin_draws(s1, s2);
                 const int ev = finish_scatter<HUBBLE, PEEL, false>(p, sh.voigt, k, d, peel_rays, peel_cells, true);
                 if (ev == EV_SCATTERED) state = LS_MARCH;
+                else if (ev == EV_DUST_SCATTERED) { state = LS_MARCH; ++dust_scat; }
                 else { tally_packet(p, sh, ev, k); state = LS_IDLE; }
             }
         }
@@ -360,6 +396,7 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
     // ---- flush the block's tallies with global atomics ----
     atomicAdd(&sh.counters[CT_PEEL_RAYS], (unsigned long long)peel_rays);
     atomicAdd(&sh.counters[CT_PEEL_CELLS], (unsigned long long)peel_cells);
+    if (dust_scat) atomicAdd(&sh.counters[CT_DUST_SCATTERINGS], (unsigned long long)dust_scat);
     __syncthreads();
     for (int i = threadIdx.x; i < N_COUNTERS; i += blockDim.x)
         if (sh.counters[i]) atomicAdd(p.counters + i, sh.counters[i]);
@@ -393,8 +430,12 @@ static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t st
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, drain_kernel<HUBBLE, PEEL, GL>, DRAIN_THREADS, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
+    const long long slots = blocks * (WALK_THREADS / 32) * COOP_MAX_LANES;      // most the walk kernel can have parked
+    pool_order_kernel<<<(unsigned)((slots + 255) / 256), 256, 0, stream>>>(p);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
     long long dblocks = (long long)n_sm * per_sm;
-    const long long cap = (blocks * (WALK_THREADS / 32) * COOP_MAX_LANES + DRAIN_WARPS - 1) / DRAIN_WARPS;   // one warp per slot
+    const long long cap = (slots + DRAIN_WARPS - 1) / DRAIN_WARPS;               // one warp per slot at most
     if (cap < dblocks) dblocks = cap;
     drain_kernel<HUBBLE, PEEL, GL><<<(unsigned)dblocks, DRAIN_THREADS, 0, stream>>>(p);
     return cudaGetLastError();

@@ -12,7 +12,7 @@
 
 namespace thor {
 
-enum : int { LS_IDLE = 0, LS_MARCH = 1, LS_TRIAL = 2, LS_FINISH = 3, LS_OUT = 4 };
+enum : int { LS_IDLE = 0, LS_MARCH = 1, LS_TRIAL = 2, LS_FINISH = 3, LS_OUT = 4, LS_SELECT = 5 };
 
 // a5 cell gather + derived per-cell quantities (one MUFU.RSQ): SoA fp32 fields through the read-only path.  A packet
 // keeps the Cell of the cell it is in (registers) until it crosses a face: in optically thick cells a packet
@@ -60,6 +60,16 @@ __device__ __forceinline__ Cell load_cell(const WalkParams& p, int64_t i) {
     return c;
 }
 
+// Line opacity per cell length at gas-frame frequency x of line 1: n sigma_0 [H(a, x) + rs H(a ra, x - dv / v_th)]
+// (the cross-sections of a doublet's transitions add); k2 = the second line's share.
+__device__ __forceinline__ float line_opacity(const WalkParams& p, const float2* s_tab, const Cell& c, float x, float& k2) {
+    k2 = 0.f;
+    if (!(c.nsig > 0.f)) return 0.f;
+    const float k1 = c.nsig * voigt_H(s_tab, c.a, x);
+    if (p.doublet_on) k2 = c.nsig * p.db_rs * voigt_H(s_tab, c.a * p.db_ra, fmaf(-p.db_dv, c.inv_vth, x));
+    return k1 + k2;
+}
+
 // a6/a7: optical depth of one segment of length len (cell units) starting at velocity offset V0, or the distance
 // s_hit at which tau_need is reached (linear within the step).  Without Hubble drift: kappa len.
 // With drift Hc (km/s per cell length): sub-steps per reading A12 — n_sub = 1 if min|x| over the segment > 6 else
@@ -67,11 +77,11 @@ __device__ __forceinline__ Cell load_cell(const WalkParams& p, int64_t i) {
 template <bool HUBBLE>
 __device__ __forceinline__ bool integrate_segment(const WalkParams& p, const float2* s_tab, const Cell& c, float V0,
                                                   float vk, float len, float tau_need, float& tau_out, float& s_hit,
-                                                  float& k_tot) {
-    tau_out = 0.f; s_hit = 0.f; k_tot = 0.f;
+                                                  float& k_tot, float& k2) {
+    tau_out = 0.f; s_hit = 0.f; k_tot = 0.f; k2 = 0.f;
     if (c.nsig <= 0.f && c.kd <= 0.f) return false;
     if (!HUBBLE) {
-        const float kl = c.nsig > 0.f ? c.nsig * voigt_H(s_tab, c.a, (V0 - vk) * c.inv_vth) : 0.f;
+        const float kl = line_opacity(p, s_tab, c, (V0 - vk) * c.inv_vth, k2);
         const float kt = kl + c.kd;
         const float dtau = kt * len;
         if (dtau >= tau_need && kt > 0.f) {
@@ -97,7 +107,7 @@ __device__ __forceinline__ bool integrate_segment(const WalkParams& p, const flo
     float tau = 0.f;
     for (int j = 0; j < nsub; ++j) {
         const float Vmid = Hc != 0.f ? fmaf(-Hc, ((float)j + 0.5f) * ds, V0) : V0;   // no 0 * inf when ds = +inf (A24)
-        const float kl = c.nsig > 0.f ? c.nsig * voigt_H(s_tab, c.a, (Vmid - vk) * c.inv_vth) : 0.f;
+        const float kl = line_opacity(p, s_tab, c, (Vmid - vk) * c.inv_vth, k2);
         const float kt = kl + c.kd;
         const float dtau = kt * ds;
         if (tau + dtau >= tau_need && kt > 0.f) {
@@ -113,9 +123,8 @@ __device__ __forceinline__ bool integrate_segment(const WalkParams& p, const flo
 }
 
 // Total opacity per cell length at velocity offset V for direction cosine-weighted bulk velocity vk (no drift).
-__device__ __forceinline__ float cell_opacity(const float2* s_tab, const Cell& c, float V, float vk) {
-    const float kl = c.nsig > 0.f ? c.nsig * voigt_H(s_tab, c.a, (V - vk) * c.inv_vth) : 0.f;
-    return kl + c.kd;
+__device__ __forceinline__ float cell_opacity(const WalkParams& p, const float2* s_tab, const Cell& c, float V, float vk, float& k2) {
+    return line_opacity(p, s_tab, c, (V - vk) * c.inv_vth, k2) + c.kd;
 }
 
 // a12 peel-off: w = P^ exp(-tau_obs), tau_obs integrated from `at` along k_obs to the box face at
@@ -148,7 +157,8 @@ __device__ __forceinline__ void peel_ray_body(const WalkParams& p, const float2*
         // the ray is dropped beyond tau_peel_max (reading A13): asking the segment for no more than what is left to the
         // cap lets it stop at the sub-step that reaches it instead of integrating the whole cell
         ++n_cells;
-        if (integrate_segment<HUBBLE>(p, s_tab, c, V, vk, len, fmaf(p.tau_peel_max - tau, 1.0000002f, 1e-30f), dtau, s_hit, kt)) return;
+        float k2;
+        if (integrate_segment<HUBBLE>(p, s_tab, c, V, vk, len, fmaf(p.tau_peel_max - tau, 1.0000002f, 1e-30f), dtau, s_hit, kt, k2)) return;
         tau += dtau;
         if (HUBBLE) V = fmaf(-p.hubble, len, V);
         if (tau > p.tau_peel_max) return;
@@ -191,7 +201,9 @@ struct Packet {
     BlockRng rng;
     float V;                     // lab-frame velocity offset from line centre, km/s
     float tau_rem;               // optical depth left to the next interaction
-    float hit_kt, x_in, upar;    // at the interaction site: total opacity, gas-frame frequency, accepted u_par
+    float hit_kt, x_in, upar;    // at the interaction site: total opacity, gas-frame frequency (of the chosen line), accepted u_par
+    float hit_k2;                // doublet: the second line's opacity there
+    int line;                    // doublet: the interaction drawn at the site: 0 / 1 = line, -1 = dust
     uint32_t nscat, crossings, rej_iters, trials;
     bool stale;                  // cell must be (re)gathered / derived before use
     bool inv_ok;                 // 1/k of the current direction is in `ray`
@@ -199,7 +211,7 @@ struct Packet {
                                  // is 1e-6 ... 1e-9 of the radius, below fp32 spacing); unused and optimised away on grids
 };
 
-enum : int { EV_CROSSED = 0, EV_HIT = 1, EV_ESCAPED = 2, EV_TERMINATED = 3, EV_CAPPED = 4, EV_ABSORBED = 5, EV_SCATTERED = 6 };
+enum : int { EV_CROSSED = 0, EV_HIT = 1, EV_ESCAPED = 2, EV_TERMINATED = 3, EV_CAPPED = 4, EV_ABSORBED = 5, EV_SCATTERED = 6, EV_DUST_SCATTERED = 7 };
 
 // a2/a3: emission of photon `id`: source ∝ luminosity, isotropic k (reading A22), Gaussian line in the
 // source cell's gas frame (A10), tau_target = -ln u.  dV_out: the line offset, for the peel of the unscattered packet.
@@ -245,7 +257,7 @@ __device__ __forceinline__ int march_step(const WalkParams& p, const float2* s_t
         // Piecewise-constant cell: the interaction lies at s = tau / kappa if that is inside the cell.
         // Deep in an optically thick cell s is far smaller than the distance to the nearest face, which bounds the
         // segment length from below: no DDA step and no reciprocals of k are needed at all.
-        kt = cell_opacity(s_tab, k.cell, k.V, vk);
+        kt = cell_opacity(p, s_tab, k.cell, k.V, vk, k.hit_k2);
         const float s = kt > 0.f ? k.tau_rem / kt : CUDART_INF_F;
         if (kt > 0.f && s <= dda_min_face_distance(k.ray, p.g)) {
             hit = true; s_hit = s;
@@ -259,7 +271,7 @@ __device__ __forceinline__ int march_step(const WalkParams& p, const float2* s_t
     } else {
         if (!k.inv_ok) { ray_set_inv(k.ray); k.inv_ok = true; }
         ex = dda_next_face(k.ray, p.g, len);
-        hit = integrate_segment<true>(p, s_tab, k.cell, k.V, vk, len, k.tau_rem, dtau, s_hit, kt);
+        hit = integrate_segment<true>(p, s_tab, k.cell, k.V, vk, len, k.tau_rem, dtau, s_hit, kt, k.hit_k2);
     }
     if (hit) {
         dda_advance_within(k.ray, p.g, s_hit);
@@ -267,6 +279,7 @@ __device__ __forceinline__ int march_step(const WalkParams& p, const float2* s_t
         k.hit_kt = kt;
         k.x_in = (k.V - vk) * k.cell.inv_vth;
         k.trials = 0u;
+        k.line = 0;
         return EV_HIT;
     }
     // reading A24: infinite segment (ray parallel to every non-frozen axis) without interaction: the packet can neither
@@ -348,12 +361,12 @@ __device__ __forceinline__ int march_step_gridless(const WalkParams& p, const fl
             // homogeneous static sphere: the gas does not depend on the step, so the interaction site s = tau / kappa is
             // known before the boundary is; (|r| + s)^2 <= R^2 is implied by r^2 + s^2 + 2 s R <= R^2: no square root
             gl_props(p, k.gx, k.gy, k.gz, k.cell);
-            const float kt0 = cell_opacity(s_tab, k.cell, k.V, 0.f);
+            const float kt0 = cell_opacity(p, s_tab, k.cell, k.V, 0.f, k.hit_k2);
             if (kt0 > 0.f) {
                 const double s = (double)(k.tau_rem / kt0);
                 if (fma(s, s + 2.0 * R, r2) <= R * R) {
                     k.gx = fma(s, kx, k.gx); k.gy = fma(s, ky, k.gy); k.gz = fma(s, kz, k.gz);
-                    k.hit_kt = kt0; k.x_in = k.V * k.cell.inv_vth; k.trials = 0u;
+                    k.hit_kt = kt0; k.x_in = k.V * k.cell.inv_vth; k.trials = 0u; k.line = 0;
                     return EV_HIT;
                 }
             }
@@ -376,12 +389,12 @@ __device__ __forceinline__ int march_step_gridless(const WalkParams& p, const fl
     if (in_gas) {
         gl_props(p, fma(0.5 * len, kx, k.gx), fma(0.5 * len, ky, k.gy), fma(0.5 * len, kz, k.gz), k.cell);
         vk = dot3(k.cell.vx, k.cell.vy, k.cell.vz, k.ray.kx, k.ray.ky, k.ray.kz);
-        kt = cell_opacity(s_tab, k.cell, k.V, vk);
+        kt = cell_opacity(p, s_tab, k.cell, k.V, vk, k.hit_k2);
     }
     if (kt > 0.f && (inf_step || kt * (float)len >= k.tau_rem)) {
         const double s = (double)(k.tau_rem / kt);
         k.gx = fma(s, kx, k.gx); k.gy = fma(s, ky, k.gy); k.gz = fma(s, kz, k.gz);
-        k.hit_kt = kt; k.x_in = (k.V - vk) * k.cell.inv_vth; k.trials = 0u;
+        k.hit_kt = kt; k.x_in = (k.V - vk) * k.cell.inv_vth; k.trials = 0u; k.line = 0;
         return EV_HIT;
     }
     if (inf_step) return EV_CAPPED;
@@ -408,7 +421,7 @@ struct FinDraws {
     float r_mu, mu_dip;          // s1.y, and dipole_mu(s1.y) if computed ahead
     float sphi, cphi;            // azimuth of k'
     float nl_p1, spsi, cpsi;     // u_perp: -ln s1.w, angle 2 pi s2.x
-    float u_dust, u_mix;         // s2.y, s2.z
+    float u_dust, u_mix, u_alb;  // s2.y, s2.z, s2.w
 };
 
 __device__ __forceinline__ FinDraws fin_draws(const float4 s1, const float4 s2) {
@@ -418,9 +431,20 @@ __device__ __forceinline__ FinDraws fin_draws(const float4 s1, const float4 s2) 
     sincos_uniform(s1.z, d.sphi, d.cphi);
     d.nl_p1 = neg_log(s1.w);
     sincos_uniform(s2.x, d.spsi, d.cpsi);
-    d.u_dust = s2.y; d.u_mix = s2.z;
+    d.u_dust = s2.y; d.u_mix = s2.z; d.u_alb = s2.w;
     return d;
 }
+
+// Doublet: the interaction is drawn at the site, before the u_par trials, because they need the line's own x and a
+// (interaction i with probability tau_i / tau): u kappa < kappa_dust -> dust, < kappa_dust + kappa_1 -> line 1,
+// else line 2, whose frequencies are measured from ITS centre.
+__device__ __forceinline__ void select_line(const WalkParams& p, Packet& k, float u) {
+    const float t = u * k.hit_kt;
+    if (p.has_dust && t < k.cell.kd) { k.line = -1; return; }
+    if (t >= k.hit_kt - k.hit_k2) { k.line = 1; k.x_in = fmaf(-p.db_dv, k.cell.inv_vth, k.x_in); }
+    else k.line = 0;
+}
+__device__ __forceinline__ float line_a(const WalkParams& p, const Packet& k) { return k.line > 0 ? k.cell.a * p.db_ra : k.cell.a; }
 
 // a7, a9-a12: the interaction itself (PAPER.md 2.3.1): dust or line, u_perp (Eq. 5, core-skipping
 // PAPER.md:244), phase function, rotation, Eq. 7 with the recoil dropped, peel-off
@@ -428,13 +452,40 @@ __device__ __forceinline__ FinDraws fin_draws(const float4 s1, const float4 s2) 
 template <bool HUBBLE, bool PEEL, bool PRE>
 __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2* s_tab, Packet& k, const FinDraws& d,
                                               uint32_t& peel_rays, uint32_t& peel_cells, bool add) {
-    if (p.has_dust && d.u_dust * k.hit_kt < k.cell.kd) return EV_ABSORBED;
     const float kx = k.ray.kx, ky = k.ray.ky, kz = k.ray.kz;
     const Cell& c = k.cell;
+    if (p.has_dust && (p.doublet_on ? k.line < 0 : d.u_dust * k.hit_kt < c.kd)) {
+        // dust (PAPER.md 2.3.2): scattered with probability albedo (Eq. 8) into the Henyey-Greenstein phase function (Eq. 9),
+        // coherently in the bulk frame of the cell (grains are heavy and move with the gas, reading A33); else destroyed
+        if (!(p.dust_albedo > 0.f) || !(d.u_alb < p.dust_albedo)) return EV_ABSORBED;
+        const float mu = hg_mu(p.dust_g, d.r_mu);
+        float e1[3], e2[3];
+        ortho_basis(kx, ky, kz, e1, e2);
+        const float vk = dot3(c.vx, c.vy, c.vz, kx, ky, kz);
+        if (PEEL) {
+            const float mu_o = dot3(kx, ky, kz, p.kobs[0], p.kobs[1], p.kobs[2]);
+            ++peel_rays;
+            peel_ray<HUBBLE, PRE>(p, s_tab, k.ray, c, k.V - vk + dot3(c.vx, c.vy, c.vz, p.kobs[0], p.kobs[1], p.kobs[2]),
+                                  hg_value(p.dust_g, mu_o), peel_cells, add);
+        }
+        const float st = sqrtf(fmaxf(0.f, fmaf(-mu, mu, 1.f)));
+        float nx = fmaf(st, fmaf(d.cphi, e1[0], d.sphi * e2[0]), mu * kx);
+        float ny = fmaf(st, fmaf(d.cphi, e1[1], d.sphi * e2[1]), mu * ky);
+        float nz = fmaf(st, fmaf(d.cphi, e1[2], d.sphi * e2[2]), mu * kz);
+        const float inv = rsqrtf(dot3(nx, ny, nz, nx, ny, nz));
+        nx *= inv; ny *= inv; nz *= inv;
+        ray_set_k(k.ray, nx, ny, nz);
+        k.inv_ok = false;
+        k.V = k.V - vk + dot3(c.vx, c.vy, c.vz, nx, ny, nz);
+        k.tau_rem = d.tau_next;
+        return EV_DUST_SCATTERED;
+    }
+    const float dv_line = k.line > 0 ? p.db_dv : 0.f;             // frequencies of this event are relative to its line
+    const float a_l = line_a(p, k);
     float x_crit = 0.f;
     if (p.core_skip_mode == 1) x_crit = p.x_crit;
     else if (p.core_skip_mode == 2) {              // local: a tau_0 over half a cell (reading A7)
-        const float atau = c.a * c.nsig * 0.5f;
+        const float atau = a_l * c.nsig * (k.line > 0 ? p.db_rs : 1.f) * 0.5f;
         x_crit = atau >= 1.f ? 0.2f * cbrtf(atau) : 0.f;
     }
     float up1, up2;
@@ -451,7 +502,7 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
         const float e1o = dot3(e1[0], e1[1], e1[2], p.kobs[0], p.kobs[1], p.kobs[2]);
         const float e2o = dot3(e2[0], e2[1], e2[2], p.kobs[0], p.kobs[1], p.kobs[2]);
         const float x_o = fmaf(up2, e2o, fmaf(up1, e1o, fmaf(k.upar, mu_o, xa)));
-        const float V_o = fmaf(x_o, c.vth, dot3(c.vx, c.vy, c.vz, p.kobs[0], p.kobs[1], p.kobs[2]));
+        const float V_o = fmaf(x_o, c.vth, dot3(c.vx, c.vy, c.vz, p.kobs[0], p.kobs[1], p.kobs[2])) + dv_line;
         ++peel_rays;
         // mix: the sampled branch weights the ray (unbiased; reading A27)
         peel_ray<HUBBLE, PRE>(p, s_tab, k.ray, c, V_o, is_dipole ? 0.75f * fmaf(mu_o, mu_o, 1.f) : 1.f, peel_cells, add);
@@ -466,7 +517,7 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
     const float x_out = fmaf(st, fmaf(up1, d.cphi, up2 * d.sphi), fmaf(k.upar, mu, xa));
     ray_set_k(k.ray, nx, ny, nz);
     k.inv_ok = false;
-    k.V = fmaf(x_out, c.vth, dot3(c.vx, c.vy, c.vz, nx, ny, nz));
+    k.V = fmaf(x_out, c.vth, dot3(c.vx, c.vy, c.vz, nx, ny, nz)) + dv_line;
     ++k.nscat;
     if (p.v_max > 0.f && fabsf(k.V) > p.v_max) return EV_TERMINATED;
     if ((p.max_scatter && k.nscat >= p.max_scatter) || !(fabsf(k.V) <= 3.0e38f)) return EV_CAPPED;   // cap, or fail-safe: non-finite V

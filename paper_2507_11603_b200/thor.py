@@ -16,7 +16,7 @@ GRID_HOST, PERIODIC_X, PERIODIC_Y, PERIODIC_Z, GRID_NO_VALIDATE, GRID_PACK = 0x1
 GRID_L2_PERSIST, GRID_L2_FETCH32 = 0x400, 0x800
 TALLY_SPECTRUM, TALLY_NSCAT_HIST, TALLY_COUNTERS, TALLY_CUBE, TALLY_RAW, TALLY_DEVICE_DST = 0, 1, 2, 3, 4, 0x100
 COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "cell_crossings", "rejection_iters",
-                 "peel_rays", "peel_cells"]
+                 "peel_rays", "peel_cells", "dust_scatterings"]
 RAW_DTYPE = np.dtype([("V", "<f4"), ("nscat", "<u4"), ("status", "<i4"), ("kx", "<f4"), ("ky", "<f4"), ("kz", "<f4")])
 
 EXPORTS = ["thor_grid_create", "thor_dataset_create_gridless", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run",
@@ -46,6 +46,8 @@ class Opts(C.Structure):
         ("photon_id_offset", C.c_uint64), ("max_scatter", C.c_uint64),
         ("raw_output", C.c_int32), ("accumulate", C.c_int32),
         ("max_crossings", C.c_uint64), ("walk_variant", C.c_int32), ("drain_mode", C.c_int32),
+        ("dust_albedo", C.c_double), ("dust_g", C.c_double), ("doublet_on", C.c_int32),
+        ("doublet_dv_kms", C.c_double), ("doublet_sigma_ratio", C.c_double), ("doublet_a_ratio", C.c_double),
     ]
 
 

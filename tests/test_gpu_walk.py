@@ -520,7 +520,7 @@ def _cube_bins_within_4sigma(cg, co, wmax=1.0, min_sum=10.0):
     edges = np.unique(np.concatenate([[0], edges + 1, [g.size]]))
     bg, bo = np.add.reduceat(g, edges[:-1]), np.add.reduceat(o, edges[:-1])
     z = np.abs(bg - bo) / np.sqrt(wmax * (bg + bo) + 1e-30)
-    assert len(bg) > 20, len(bg)
+    assert len(bg) > 8, len(bg)
     assert z.max() <= 4.0, (z.max(), len(bg))
     return len(bg)
 
