@@ -44,7 +44,7 @@ BYTES_PER_CROSSING = 20.0                              # n_HI, T, v_x, v_y, v_z 
 TRAFFIC = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))) if os.path.exists(os.path.join(ROOT, "profiles", "traffic.json")) else {}
 
 HEADLINE = "web1536"
-SUBS = ["shell", "sphere", "slab", "gather", "turb512"]
+SUBS = ["shell", "sphere", "slab", "slab_paper", "gather", "turb512"]
 
 
 def make_workload(name, n_photons=None, device="cuda"):
@@ -79,6 +79,10 @@ def make_workload(name, n_photons=None, device="cuda"):
                               n0=tau0 / (W.RECIPE_SIGMA0_T4 / (T / 1e4) ** 0.5 * W.PC_CM)),
                  sources=dict(pos=np.zeros((1, 3), np.float32), lum=np.ones(1, np.float32), sigma=np.zeros(1, np.float32)),
                  opts=dict(phase_core=0, phase_wing=0, spec_mode=0, spec_T_ref=T, spec_bins=400, spec_lo=-60.0, spec_hi=60.0))
+    elif name == "slab_paper":  # configs[2] with the PAPER's phase functions (1/3-2/3 mix in the core, dipole in the wings)
+        w = W.static_slab(n_photons=1_000_000, phase_core=2, phase_wing=1)
+        w["name"] += "_paper_phases"
+        note = dict(phase_assignment="PAPER.md:132 (mix core / dipole wing) instead of BASELINE.json's dipole core / isotropic wing")
     elif name == "gather":   # the cell-gather regime: configs[4]'s recipe at 512^3 made optically thin (mean n_HI 1e-11), so
         # packets stream through ~340 cells each and the walk is bound by the HBM gathers, not by scatterings
         w = W.cosmic_web(n=512, n_src=1 << 16, n_photons=4_000_000, map_pix=2048, mean_n=1e-11)
@@ -244,7 +248,7 @@ def run_reference(args):
 
 def workload_label(name):
     return {"web1536": "cosmic_web_n1536", "web512": "cosmic_web_n512", "turb512": "turbulent_box_n512",
-            "shell": "expanding_shell_n128", "sphere": "static_sphere_n32_tau10000_T10", "slab": "static_slab_nz256_tau1e+07", "neufeld": "neufeld_sphere_gridless_tau1e6",
+            "shell": "expanding_shell_n128", "sphere": "static_sphere_n32_tau10000_T10", "slab": "static_slab_nz256_tau1e+07", "neufeld": "neufeld_sphere_gridless_tau1e6", "slab_paper": "static_slab_nz256_tau1e+07_paper_phases",
             "gather": "cosmic_web_n512_thin_gather"}.get(name, name)
 
 def run_operators(args):
@@ -385,7 +389,9 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
         pack = bool(args.pack)
     n = w["n_photons"]
     opts = dict(w["opts"], raw_output=0)
-    t_gen = time.perf_counter()
+    if args.max_scatter >= 0:
+        opts["max_scatter"] = args.max_scatter
+    id0 = args.photon_id_offset
     gridless = "dataset" in w
     ctx = thor.Context.gridless(**w["dataset"]) if gridless else thor.Context.from_workload(w["grid"], pack=pack, extra_flags=args.grid_flags)   # resident before the timed region
     ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
@@ -396,7 +402,7 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
 
     def step(i):
         # rank r walks photon ids [r n, (r+1) n) of step i's seed; tallies summed over ranks (the one exchange step)
-        ctx.run(n, w["seed"] + i, dict(opts, photon_id_offset=rank * n))
+        ctx.run(n, w["seed"] + (i if not id0 else 0), dict(opts, photon_id_offset=id0 + rank * n))
         ctx.tally_to_device(thor.TALLY_SPECTRUM, spec_dev)
         ctx.tally_to_device(thor.TALLY_COUNTERS, cnt_dev)
         shard.allreduce_tallies([spec_dev, cnt_dev])               # no-op at N = 1
@@ -467,9 +473,10 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
     peak = n_sm * SCHEDULERS_PER_SM * LANES * sm_hz * world
     inst = INST_PER_SCATTERING * c["scatterings"] + INST_PER_CROSSING * crossings
     achieved = inst / (kernel_ms * 1e-3)
-    traffic = TRAFFIC.get(name) if not n_photons else None
+    tr = TRAFFIC.get(name)
+    traffic = tr["bytes_per_launch"] * n / tr["n_photons"] if tr else None      # measured at tr[n_photons] packets, scaled to n
     alu = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "G thread-inst/s", "frac": achieved / peak,
-           "traffic": traffic, "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch (profiles/traffic.json, profiles/r02_*.md)",
+           "traffic": traffic, "traffic_source": (tr["source"] + f"; measured at {tr['n_photons']} packets, scaled linearly to {n}") if tr else None,
            "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_hz / 1e6:.0f} MHz (clocks.max.sm), derived in DESIGN.md 5",
            "kernel": "walk_kernel", "kernel_ms_per_launch": kernel_ms / steps,
            "inst_per_scattering": INST_PER_SCATTERING, "inst_per_crossing": INST_PER_CROSSING,
@@ -502,7 +509,8 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
         cube_bytes = opts.get("peel_nx", 0) * opts.get("peel_ny", 0) * opts.get("peel_nv", 0) * 8 if opts.get("peel_on") else 0
         d2h = (opts["spec_bins"] + 2 + 64 + len(thor.COUNTER_NAMES)) * 8 + cube_bytes
         e_scat, e_secs = 0, 0.0
-        for i in range(-1, steps):                                  # one untimed warm-up pass
+        e_steps = min(steps, 2)
+        for i in range(0 if not regrid else -1, e_steps):           # small grids: one untimed pass warms the re-creation path
             flush.zero_()
             if world > 1:
                 dist.barrier()
@@ -510,7 +518,7 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
             t0 = time.perf_counter()
             cx = thor.Context.from_workload(g, host=True, pack=pack) if regrid else ctx
             cx.sources_set(src["pos"], src["lum"], src["sigma"])
-            cx.run(n, w["seed"] + max(i, 0), dict(opts, photon_id_offset=rank * n))
+            cx.run(n, w["seed"] + (max(i, 0) if not id0 else 0), dict(opts, photon_id_offset=id0 + rank * n))
             cx.spectrum(); cx.nscat_hist()
             if cube_bytes:
                 cx.cube()
@@ -527,7 +535,7 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
             if i >= 0:
                 e_secs += float(tt[0]); e_scat += float(tt[1])
         out["e2e"] = {"value": e_scat / e_secs, "unit": "scatterings/s", "h2d_bytes_per_step": int(h2d),
-                      "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e_secs / steps,
+                      "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e_secs / e_steps, "steps": e_steps,
                       "timing": ("host wall clock around " + ("create(host arrays)+" if regrid else "") +
                                  "sources_set(host arrays)+run+tally_get(host: spectrum, histogram, counters" +
                                  (", cube" if cube_bytes else "") + ")" + ("+destroy" if regrid else "") +
@@ -554,6 +562,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-subs", action="store_true", help="skip the `workloads` sub-dict")
     ap.add_argument("--sub-steps", type=int, default=2)
+    ap.add_argument("--photon-id-offset", type=int, default=0, help="first photon id of rank 0 (with --n-photons 1: one chosen packet alone on the GPU, the lone-lane regime of DESIGN.md 4.6)")
+    ap.add_argument("--max-scatter", type=int, default=-1, help="override the workload's scattering cap")
     ap.add_argument("--grid-flags", type=lambda v: int(v, 0), default=0, help="extra thor_grid_create flags (0x400 L2 persistence window, 0x800 32-byte L2 fetch granularity)")
     ap.add_argument("--pack", type=int, default=-1, help="THOR_GRID_PACK (1/0); default: on for the gather workload")
     args = ap.parse_args()

@@ -105,7 +105,9 @@ thor_status thor_sources_set(thor_ctx *ctx, long long n_src, const float *pos_xy
 /* Run options.  Set struct_size = sizeof(thor_opts); use thor_opts_default() for the defaults. */
 typedef struct thor_opts {
     uint32_t struct_size;
-    int32_t phase_core, phase_wing;   /* THOR_PHASE_*; default isotropic / isotropic */
+    int32_t phase_core, phase_wing;   /* THOR_PHASE_*; default isotropic / isotropic, which is what BASELINE.json's configs
+                                         state; the paper's own assignment is MIX in the core and DIPOLE in
+                                         the wings and has to be asked for */
     int32_t phase_frame;              /* 0: split on atom-frame |x_in - u_par| (default), 1: gas-frame |x_in| (A3) */
     double phase_split_x;             /* 0.2 */
     int32_t core_skip_mode;           /* 0 off, 1 global x_crit, 2 local per cell (reading A7) */
@@ -126,7 +128,8 @@ typedef struct thor_opts {
     uint64_t photon_id_offset;        /* the run covers photon ids [offset, offset + n_photons) */
     uint64_t max_scatter;             /* safety cap per packet (0 = none); capped packets are counted, not tallied */
     int32_t raw_output;               /* keep one thor_raw_record per packet (THOR_TALLY_RAW) */
-    int32_t accumulate;               /* do not zero the tallies before this run */
+    int32_t accumulate;               /* do not zero the tallies before this run; the spectrum axis and the peel geometry must
+                                         be those of the run it adds to (THOR_ERR_ARG otherwise) */
     uint64_t max_crossings;           /* cap on cell crossings per packet (capped packets are counted, not tallied);
                                          0 = the built-in limit 2^32 - 1 (reading A26).  Required (> 0) on a
                                          grid that is periodic on all three axes: no packet can ever leave it */
@@ -262,6 +265,10 @@ const char *thor_last_error(const thor_ctx *ctx);
 /* a1 RNG: out[i*n_draws + d] = draw d of photon (id0 + i) under seed — Philox4x32-10, counter = (d>>2 lo, d>>2 hi,
  * id lo, id hi), key = (seed lo, seed hi), word d&3 (reading A16; cuRAND's curand_init(seed, id, 0) layout). */
 thor_status thor_unit_philox(uint64_t seed, uint64_t id0, long long n_ids, int n_draws, uint32_t *out, void *stream);
+
+/* The same draws through cuRAND's own device API — curand_init(seed, id0 + i, 0) on a curandStatePhilox4_32_10_t, then
+ * curand4() word by word — to pin reading A16's counter / key layout against the library that defines it. */
+thor_status thor_unit_curand_philox(uint64_t seed, uint64_t id0, long long n_ids, int n_draws, uint32_t *out, void *stream);
 
 /* a4 DDA: traces n rays (org, dir: float[n][3], cell units) through an (nx,ny,nz) grid with `periodic_flags`
  * (THOR_PERIODIC_*), at most max_steps cells each.  Per ray: hash_idx = word-wise FNV-1a (offset 0xCBF29CE484222325,

@@ -67,6 +67,16 @@ struct thor_ctx {
 
 static thread_local std::string g_err;
 
+// Every entry point works on the context's device and leaves the caller's current device as it found it.
+struct DevGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DevGuard(int dev) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DevGuard() { if (switched) cudaSetDevice(prev); }
+};
+
 static constexpr size_t SMALL_NEXT = 0, SMALL_COUNTERS = 1, SMALL_HIST = SMALL_COUNTERS + thor::N_COUNTERS,
                         SMALL_SPEC = SMALL_HIST + 64, SMALL_TIMES = SMALL_SPEC + 4096 + 2, SMALL_MAXN = SMALL_TIMES + 2, SMALL_POOL = SMALL_MAXN + 1, SMALL_TOTAL = SMALL_POOL + 2;
 
@@ -105,7 +115,7 @@ extern "C" void thor_opts_default(thor_opts* o) {
 
 extern "C" void thor_grid_destroy(thor_ctx* ctx) {
     if (!ctx) return;
-    cudaSetDevice(ctx->device);
+    DevGuard dev_guard(ctx->device);
     for (float* p : ctx->owned) if (p) cudaFree(p);
     if (ctx->d_packed) cudaFree(ctx->d_packed);
     if (ctx->d_src_pos) cudaFree(ctx->d_src_pos);
@@ -287,7 +297,7 @@ extern "C" thor_status thor_sources_set(thor_ctx* ctx, long long n_src, const fl
     double acc = 0;
     for (long long i = 0; i < n_src; ++i) { acc += lum[i]; cdf[(size_t)i] = acc / tot; }
     cdf[(size_t)n_src - 1] = 1.0;
-    CU(cudaSetDevice(ctx->device));
+    DevGuard dev_guard(ctx->device);
     if (ctx->d_src_pos) { cudaFree(ctx->d_src_pos); ctx->d_src_pos = nullptr; }
     if (ctx->d_src_sigma) { cudaFree(ctx->d_src_sigma); ctx->d_src_sigma = nullptr; }
     if (ctx->d_src_cdf) { cudaFree(ctx->d_src_cdf); ctx->d_src_cdf = nullptr; }
@@ -437,7 +447,7 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     p.dust_albedo = (float)o.dust_albedo; p.dust_g = (float)o.dust_g;
     p.doublet_on = o.doublet_on ? 1 : 0;
     p.db_dv = (float)o.doublet_dv_kms; p.db_rs = (float)o.doublet_sigma_ratio; p.db_ra = (float)o.doublet_a_ratio;
-    CU(cudaSetDevice(ctx->device));
+    DevGuard dev_guard(ctx->device);
     if (o.drain_mode == 0 && !ctx->d_pool)
         CU(cudaMalloc(&ctx->d_pool, (size_t)thor::walk_pool_slots(ctx->n_sm) * thor::walk_pool_words() * sizeof(uint32_t)));
     if (o.drain_mode == 0 && !ctx->d_pool_order)
@@ -445,6 +455,16 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     p.pool = o.drain_mode == 0 ? ctx->d_pool : nullptr;
     p.pool_order = ctx->d_pool_order;
     const bool keep = o.accumulate && ctx->have_run;
+    if (keep) {
+        const thor_opts& l = ctx->last;
+        const bool same = l.spec_bins == o.spec_bins && l.spec_lo == o.spec_lo && l.spec_hi == o.spec_hi && l.spec_mode == o.spec_mode &&
+                          l.spec_T_ref == o.spec_T_ref && l.peel_on == o.peel_on &&
+                          (!o.peel_on || (l.peel_nx == o.peel_nx && l.peel_ny == o.peel_ny && l.peel_nv == o.peel_nv && l.peel_v_lo == o.peel_v_lo &&
+                                          l.peel_v_hi == o.peel_v_hi && l.peel_width_cells == o.peel_width_cells && l.k_obs[0] == o.k_obs[0] &&
+                                          l.k_obs[1] == o.k_obs[1] && l.k_obs[2] == o.k_obs[2]));
+        if (!same) return fail(ctx, THOR_ERR_ARG, "thor_run: accumulate needs the spectrum axis and the peel geometry of the run it adds to");
+    }
+    ctx->have_run = false;                          // from here on the tallies are in flux: valid again only after a completed run
     if (cube_elems != ctx->cube_elems) {
         if (ctx->d_cube) { cudaFree(ctx->d_cube); ctx->d_cube = nullptr; }
         ctx->cube_elems = 0;
@@ -480,7 +500,6 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     p.nscat_hist = ctx->d_small + SMALL_HIST;
     p.spectrum = ctx->d_small + SMALL_SPEC;
     p.cube = ctx->d_cube;
-    ctx->have_run = false;
     CU(cudaEventRecord(ctx->ev0, ctx->stream));
     if (n_photons > 0) CU(thor::launch_walk(p, ctx->n_sm, ctx->stream, &ctx->last_blocks));
     CU(cudaEventRecord(ctx->ev1, ctx->stream));
@@ -545,7 +564,7 @@ extern "C" thor_status thor_raytrace_ex(thor_ctx* ctx, long long n_rays, const f
     if (!std::isfinite(o->hubble_kms_per_cell) || !(o->hubble_eps >= 0) || !(o->max_length_cells >= 0) || !std::isfinite(o->max_length_cells))
         return fail(ctx, THOR_ERR_ARG, "thor_raytrace: bad Hubble term / sub-sampling / length");
     const thor::WalkParams p = grid_params(ctx);
-    CU(cudaSetDevice(ctx->device));
+    DevGuard dev_guard(ctx->device);
     const bool host = (o->flags & THOR_RAYS_HOST) != 0;
     const int n_v = out_tau ? o->n_v : 0;
     Staged st;
@@ -604,7 +623,7 @@ extern "C" thor_status thor_volume_render_ex(thor_ctx* ctx, long long n_rays, co
         tf.r[q] = k[2]; tf.g[q] = k[3]; tf.b[q] = k[4];
     }
     const thor::WalkParams p = grid_params(ctx);
-    CU(cudaSetDevice(ctx->device));
+    DevGuard dev_guard(ctx->device);
     const bool host = (flags & THOR_RAYS_HOST) != 0;
     Staged st;
     const float *d_org = org_xyz, *d_dir = dir_xyz;
@@ -632,7 +651,7 @@ extern "C" thor_status thor_slice(thor_ctx* ctx, long long n_points, const float
     if (field < THOR_FIELD_NHI || field > THOR_FIELD_KDUST) return fail(ctx, THOR_ERR_ARG, "thor_slice: unknown field");
     if (field == THOR_FIELD_KDUST && !ctx->has_dust) return fail(ctx, THOR_ERR_ARG, "thor_slice: the grid has no dust field");
     const thor::WalkParams p = grid_params(ctx);
-    CU(cudaSetDevice(ctx->device));
+    DevGuard dev_guard(ctx->device);
     const bool host = (flags & THOR_RAYS_HOST) != 0;
     Staged st;
     const float* d_pos = pos_xyz;
@@ -692,7 +711,7 @@ extern "C" thor_status thor_tally_get(thor_ctx* ctx, int kind, void* dst, size_t
     if (!dst) return THOR_OK;
     if (dst_bytes < bytes) return fail(ctx, THOR_ERR_ARG, "thor_tally_get: dst_bytes too small");
     if (bytes == 0) return THOR_OK;
-    CU(cudaSetDevice(ctx->device));
+    DevGuard dev_guard(ctx->device);
     if (k == THOR_TALLY_CUBE && !dev_dst) {
         // fixed point -> double on the host
         std::vector<unsigned long long> tmp;

@@ -1,5 +1,6 @@
 // Single steps of the path as stand-alone kernels (thor_unit_* of include/thor.h) + the field validation scan.
 #include <cuda_runtime.h>
+#include <curand_kernel.h>
 #include <string>
 #include "../../include/thor.h"
 #include "philox.cuh"
@@ -52,6 +53,19 @@ __global__ void unit_philox_kernel(uint64_t seed, uint64_t id0, long long n_ids,
     Stream s;
     s.init(seed, id0 + (uint64_t)i);
     for (int d = 0; d < n_draws; ++d) out[i * n_draws + d] = s.next_u32();
+}
+
+// cuRAND's Philox4x32-10 on the same (seed, subsequence = photon id, offset = 0): test-only cross-check of the layout.
+__global__ void unit_curand_kernel(uint64_t seed, uint64_t id0, long long n_ids, int n_draws, uint32_t* out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_ids) return;
+    curandStatePhilox4_32_10_t st;
+    curand_init((unsigned long long)seed, (unsigned long long)(id0 + (uint64_t)i), 0ull, &st);
+    for (int d = 0; d < n_draws; d += 4) {
+        const uint4 r = curand4(&st);
+        const uint32_t w[4] = {r.x, r.y, r.z, r.w};
+        for (int j = 0; j < 4 && d + j < n_draws; ++j) out[i * n_draws + d + j] = w[j];
+    }
 }
 
 __device__ __forceinline__ uint64_t fnv_word(uint64_t h, uint64_t w) { return (h ^ w) * 0x100000001B3ull; }
@@ -135,6 +149,13 @@ extern "C" thor_status thor_unit_philox(uint64_t seed, uint64_t id0, long long n
     if (n_ids <= 0 || n_draws <= 0 || !out) return THOR_ERR_ARG;
     thor::unit_philox_kernel<<<(unsigned)((n_ids + 127) / 128), 128, 0, (cudaStream_t)stream>>>(seed, id0, n_ids, n_draws, out);
     return unit_done((cudaStream_t)stream, "thor_unit_philox");
+}
+
+extern "C" thor_status thor_unit_curand_philox(uint64_t seed, uint64_t id0, long long n_ids, int n_draws, uint32_t* out,
+                                               void* stream) {
+    if (n_ids <= 0 || n_draws <= 0 || !out) return THOR_ERR_ARG;
+    thor::unit_curand_kernel<<<(unsigned)((n_ids + 127) / 128), 128, 0, (cudaStream_t)stream>>>(seed, id0, n_ids, n_draws, out);
+    return unit_done((cudaStream_t)stream, "thor_unit_curand_philox");
 }
 
 extern "C" thor_status thor_unit_dda_trace(int nx, int ny, int nz, unsigned periodic_flags, long long n,

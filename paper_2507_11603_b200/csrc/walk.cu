@@ -17,6 +17,9 @@ __device__ __forceinline__ unsigned long long global_timer_ns() {
 #ifndef THOR_WALK_MIN_CTAS
 #define THOR_WALK_MIN_CTAS 3
 #endif
+#ifndef THOR_PEEL_MIN_CTAS
+#define THOR_PEEL_MIN_CTAS 2
+#endif
 #ifndef THOR_FINISH_MIN_LANES
 #define THOR_FINISH_MIN_LANES 24
 #endif
@@ -321,7 +324,7 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
                     else emit_packet(p, k, p.id_offset + i, k0, k1, dV);
                     if (PEEL) {
                         ++peel_rays;
-                        peel_ray<HUBBLE, false>(p, sh.voigt, k.ray, k.cell,
+                        peel_ray<HUBBLE, true>(p, sh.voigt, k.ray, k.cell,
                                          dot3(k.cell.vx, k.cell.vy, k.cell.vz, p.kobs[0], p.kobs[1], p.kobs[2]) + dV, 1.f,
                                          peel_cells, true);
                     }
@@ -451,8 +454,8 @@ cudaError_t launch_walk(const WalkParams& p, int n_sm, cudaStream_t stream, int*
     const double cells = (double)p.g.nx * p.g.ny * p.g.nz;
     const double grid_bytes = cells * (p.packed ? 32.0 : (p.has_dust ? 24.0 : 20.0));
     const bool beyond_l2 = p.walk_variant ? p.walk_variant == 4 : grid_bytes > 96.0e6;
-    if (peel) return hub ? launch_variant<true, true, 2>(p, n_sm, stream, blocks_out)
-                         : launch_variant<false, true, 2>(p, n_sm, stream, blocks_out);
+    if (peel) return hub ? launch_variant<true, true, THOR_PEEL_MIN_CTAS>(p, n_sm, stream, blocks_out)
+                         : launch_variant<false, true, THOR_PEEL_MIN_CTAS>(p, n_sm, stream, blocks_out);
     if (beyond_l2) return hub ? launch_variant<true, false, 4>(p, n_sm, stream, blocks_out)
                               : launch_variant<false, false, 4>(p, n_sm, stream, blocks_out);
     return hub ? launch_variant<true, false, THOR_WALK_MIN_CTAS>(p, n_sm, stream, blocks_out)

@@ -465,7 +465,7 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
         if (PEEL) {
             const float mu_o = dot3(kx, ky, kz, p.kobs[0], p.kobs[1], p.kobs[2]);
             ++peel_rays;
-            peel_ray<HUBBLE, PRE>(p, s_tab, k.ray, c, k.V - vk + dot3(c.vx, c.vy, c.vz, p.kobs[0], p.kobs[1], p.kobs[2]),
+            peel_ray<HUBBLE, true>(p, s_tab, k.ray, c, k.V - vk + dot3(c.vx, c.vy, c.vz, p.kobs[0], p.kobs[1], p.kobs[2]),
                                   hg_value(p.dust_g, mu_o), peel_cells, add);
         }
         const float st = sqrtf(fmaxf(0.f, fmaf(-mu, mu, 1.f)));
@@ -505,7 +505,7 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
         const float V_o = fmaf(x_o, c.vth, dot3(c.vx, c.vy, c.vz, p.kobs[0], p.kobs[1], p.kobs[2])) + dv_line;
         ++peel_rays;
         // mix: the sampled branch weights the ray (unbiased; reading A27)
-        peel_ray<HUBBLE, PRE>(p, s_tab, k.ray, c, V_o, is_dipole ? 0.75f * fmaf(mu_o, mu_o, 1.f) : 1.f, peel_cells, add);
+        peel_ray<HUBBLE, true>(p, s_tab, k.ray, c, V_o, is_dipole ? 0.75f * fmaf(mu_o, mu_o, 1.f) : 1.f, peel_cells, add);
     }
     const float st = sqrtf(fmaxf(0.f, fmaf(-mu, mu, 1.f)));
     float nx = fmaf(st, fmaf(d.cphi, e1[0], d.sphi * e2[0]), mu * kx);

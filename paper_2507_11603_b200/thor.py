@@ -20,7 +20,7 @@ COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "
 RAW_DTYPE = np.dtype([("V", "<f4"), ("nscat", "<u4"), ("status", "<i4"), ("kx", "<f4"), ("ky", "<f4"), ("kz", "<f4")])
 
 EXPORTS = ["thor_grid_create", "thor_dataset_create_gridless", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run",
-           "thor_last_run_ms", "thor_last_run_feed_ms", "thor_last_run_max_nscat", "thor_raytrace", "thor_raytrace_ex", "thor_volume_render", "thor_volume_render_ex", "thor_slice", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_dda_trace",
+           "thor_last_run_ms", "thor_last_run_feed_ms", "thor_last_run_max_nscat", "thor_raytrace", "thor_raytrace_ex", "thor_volume_render", "thor_volume_render_ex", "thor_slice", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_curand_philox", "thor_unit_dda_trace",
            "thor_unit_voigt", "thor_unit_scatter"]
 
 
@@ -101,6 +101,7 @@ def lib():
         L.thor_last_error.argtypes = [P]
         L.thor_last_error.restype = C.c_char_p
         L.thor_unit_philox.argtypes = [u64, u64, i64, i32, P, P]
+        L.thor_unit_curand_philox.argtypes = [u64, u64, i64, i32, P, P]
         L.thor_unit_dda_trace.argtypes = [i32, i32, i32, u32, i64, P, P, i64, P, P, P, P, P, P]
         L.thor_unit_voigt.argtypes = [i64, P, P, P, P]
         L.thor_unit_scatter.argtypes = [f, f, f, i32, u64, u64, i64, P, P, P, P, P]
@@ -330,6 +331,13 @@ def unit_philox(seed, id0, n_ids, n_draws):
     import torch
     out = torch.empty((n_ids, n_draws), dtype=torch.int32, device="cuda")
     _check(lib().thor_unit_philox(int(seed), int(id0), n_ids, n_draws, C.c_void_p(out.data_ptr()), _stream()))
+    return out.cpu().numpy().view(np.uint32)
+
+
+def unit_curand_philox(seed, id0, n_ids, n_draws):
+    import torch
+    out = torch.empty((n_ids, n_draws), dtype=torch.int32, device="cuda")
+    _check(lib().thor_unit_curand_philox(int(seed), int(id0), n_ids, n_draws, C.c_void_p(out.data_ptr()), _stream()))
     return out.cpu().numpy().view(np.uint32)
 
 

@@ -217,3 +217,12 @@ def test_gathers_beyond_2_31_on_a_borrowed_grid(thor):
         ctx.close()
         del buf, f
         torch.cuda.empty_cache()
+
+
+def test_philox_layout_is_curands(thor):
+    """S§8(c) P13 / reading A16: the walk's Philox stream for (seed, photon id) is, word for word, what cuRAND's own device
+    API gives for curand_init(seed, subsequence = id, offset = 0) + curand4() — across 32-bit boundaries of seed and id."""
+    for seed, id0 in ((1, 0), (0xDEADBEEFCAFEF00D, (1 << 32) - 3), ((1 << 64) - 1, (1 << 40) + 17)):
+        a = thor.unit_philox(seed, id0, 50, 23)
+        b = thor.unit_curand_philox(seed, id0, 50, 23)
+        assert np.array_equal(a, b), (seed, id0)

@@ -639,3 +639,23 @@ def test_long_core_chains_at_1e4K(thor, oracle):
     _conserved(g, n)
     assert g["counters"]["escaped"] == n and g["raw"]["nscat"].mean() > 1e5
     _statistical_parity(g, o, n, n)
+
+
+def test_accumulate_needs_the_same_tally_layout(thor):
+    """accumulate = 1 adds to the tallies of the previous run: a different spectrum axis or peel geometry is refused instead
+    of silently summed or reallocated, and after a refused run the previous tallies are still served."""
+    w = W.static_sphere(n=8, tau0=10.0, T=10.0, n_photons=500)
+    ctx = thor.Context.from_workload(w["grid"])
+    try:
+        ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
+        ctx.run(500, 1, dict(w["opts"]))
+        first = ctx.spectrum().copy()
+        for bad in (dict(spec_bins=w["opts"]["spec_bins"] // 2), dict(spec_hi=w["opts"]["spec_hi"] * 2),
+                    dict(peel_on=1, peel_nx=4, peel_ny=4, peel_nv=4, peel_width_cells=8.0)):
+            with pytest.raises(thor.ThorError) as e:
+                ctx.run(500, 1, dict(w["opts"], accumulate=1, photon_id_offset=500, **bad))
+            assert e.value.status == 1 and "accumulate" in str(e.value)
+        ctx.run(500, 1, dict(w["opts"], accumulate=1, photon_id_offset=500))
+        assert int(ctx.spectrum().sum()) == 2 * int(first.sum()) == 1000
+    finally:
+        ctx.close()
