@@ -443,6 +443,7 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
         cube_elems = (size_t)o.peel_nx * o.peel_ny * o.peel_nv;
     }
     p.id_offset = o.photon_id_offset; p.n_photons = n_photons; p.seed = seed; p.max_scatter = o.max_scatter;
+    p.max_scatter32 = o.max_scatter > 0xffffffffull ? 0xffffffffu : (unsigned)o.max_scatter;
     p.walk_variant = o.walk_variant;
     p.dust_albedo = (float)o.dust_albedo; p.dust_g = (float)o.dust_g;
     p.doublet_on = o.doublet_on ? 1 : 0;

@@ -77,6 +77,7 @@ struct WalkParams {
     float peel_inv_width;                // 1 / peel_width_cells
     float tau_peel_max;
     unsigned long long id_offset, n_photons, seed, max_scatter;
+    unsigned int max_scatter32;          // max_scatter clamped to 32 bits (the per-packet counter's width); 0 = none
     unsigned int max_crossings;          // per-packet cap on cell crossings (reading A26); 2^32 - 1 = the built-in limit
     // work distribution + tallies (device)
     unsigned long long* next_photon;     // a14: global atomic photon counter

@@ -520,7 +520,7 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
     k.V = fmaf(x_out, c.vth, dot3(c.vx, c.vy, c.vz, nx, ny, nz)) + dv_line;
     ++k.nscat;
     if (p.v_max > 0.f && fabsf(k.V) > p.v_max) return EV_TERMINATED;
-    if ((p.max_scatter && k.nscat >= p.max_scatter) || !(fabsf(k.V) <= 3.0e38f)) return EV_CAPPED;   // cap, or fail-safe: non-finite V
+    if ((p.max_scatter32 && k.nscat >= p.max_scatter32) || !(fabsf(k.V) <= 3.0e38f)) return EV_CAPPED;   // cap, or fail-safe: non-finite V
     k.tau_rem = d.tau_next;
     return EV_SCATTERED;
 }
