@@ -169,6 +169,90 @@ __global__ void pool_order_kernel(const __grid_constant__ WalkParams p) {
     p.pool_order[rank] = (unsigned int)i;
 }
 
+// ---- deferred peel rays --------------------------------------------------------------------------
+// Most peel rays end in the packet's own cell (optically thick: tau > tau_peel_max) and the few that go on cross tens to
+// thousands of cells.  Marched in place they hold the warp at ONE active lane: 43 % of the walk kernel's issued
+// instructions on config 5 (profiles/r02_lanes.md).  So the walk kernel marches only the first cell in place and puts a
+// ray that goes on into a per-warp queue in shared memory (10 words: cell, offset, tau, V, weight, pixel); when 32 have
+// gathered the warp serves them, one ray per lane and one cell per turn, topping idle lanes up from the queue and putting
+// the unfinished rays back once fewer than PEEL_MIN_ACTIVE are left.  The cube is fixed point, so the order of its
+// additions changes nothing: tallies stay bit-identical to the in-place march.
+constexpr int PEELQ_CAP = 64;                           // entries per warp (at most PEEL_MIN_ACTIVE - 1 + 32 are ever queued)
+constexpr int PEELQ_WORDS = 10;
+constexpr int PEELQ_SERVE = 32;                         // serve when this many are queued
+#ifndef THOR_PEEL_MIN_ACTIVE
+#define THOR_PEEL_MIN_ACTIVE 16
+#endif
+constexpr int PEEL_MIN_ACTIVE = THOR_PEEL_MIN_ACTIVE;
+
+// Queue layout: word w of entry e at q[w * PEELQ_CAP + e] (consecutive lanes, consecutive banks).
+__device__ __forceinline__ void peelq_put(uint32_t* q, int e, const PeelPend& d) {
+    q[0 * PEELQ_CAP + e] = (uint32_t)d.cx; q[1 * PEELQ_CAP + e] = (uint32_t)d.cy; q[2 * PEELQ_CAP + e] = (uint32_t)d.cz;
+    q[3 * PEELQ_CAP + e] = __float_as_uint(d.fx); q[4 * PEELQ_CAP + e] = __float_as_uint(d.fy); q[5 * PEELQ_CAP + e] = __float_as_uint(d.fz);
+    q[6 * PEELQ_CAP + e] = __float_as_uint(d.tau); q[7 * PEELQ_CAP + e] = __float_as_uint(d.V);
+    q[8 * PEELQ_CAP + e] = __float_as_uint(d.phat); q[9 * PEELQ_CAP + e] = (uint32_t)d.pix;
+}
+__device__ __forceinline__ void peelq_get(const uint32_t* q, int e, PeelPend& d) {
+    d.cx = (int)q[0 * PEELQ_CAP + e]; d.cy = (int)q[1 * PEELQ_CAP + e]; d.cz = (int)q[2 * PEELQ_CAP + e];
+    d.fx = __uint_as_float(q[3 * PEELQ_CAP + e]); d.fy = __uint_as_float(q[4 * PEELQ_CAP + e]); d.fz = __uint_as_float(q[5 * PEELQ_CAP + e]);
+    d.tau = __uint_as_float(q[6 * PEELQ_CAP + e]); d.V = __uint_as_float(q[7 * PEELQ_CAP + e]);
+    d.phat = __uint_as_float(q[8 * PEELQ_CAP + e]); d.pix = (int)q[9 * PEELQ_CAP + e];
+}
+
+// The lanes whose `pend` is live append it to the warp's queue (whole warp calls; cnt is warp-uniform).
+__device__ __forceinline__ void peelq_push(uint32_t* q, int& cnt, PeelPend& pend, unsigned lane) {
+    const unsigned m = __ballot_sync(0xffffffffu, pend.live);
+    if (!m) return;
+    if (pend.live) peelq_put(q, cnt + __popc(m & ((1u << lane) - 1u)), pend);
+    pend.live = false;
+    cnt += __popc(m);
+    __syncwarp();
+}
+
+// Serve the queue (whole warp calls).  flush: to the last ray (before the warp leaves the kernel).
+template <bool HUBBLE>
+__device__ __noinline__ void peelq_serve(const WalkParams& p, const float2* s_tab, uint32_t* q, int& cnt, uint32_t& n_cells,
+                                        bool flush, unsigned lane) {
+    PeelPend d;
+    d.live = false;
+    Ray r;
+    peel_ray_direction(p, r);
+    for (;;) {
+        const unsigned idle = __ballot_sync(0xffffffffu, !d.live);
+        if (idle && cnt > 0) {                                // top idle lanes up from the back of the queue
+            const int take = min(__popc(idle), cnt);
+            const int rank = __popc(idle & ((1u << lane) - 1u));
+            if (!d.live && rank < take) {
+                peelq_get(q, cnt - 1 - rank, d);
+                r.cx = d.cx; r.cy = d.cy; r.cz = d.cz; r.fx = d.fx; r.fy = d.fy; r.fz = d.fz;
+                if (d.pix == PEEL_PIX_UNSET) d.pix = peel_pixel(p, r);      // a ray queued whole (drain kernel) starts here
+                d.live = d.pix >= 0;
+            }
+            cnt -= take;
+            __syncwarp();
+        }
+        const unsigned act = __ballot_sync(0xffffffffu, d.live);
+        if (!act) return;
+        if (!flush && __popc(act) < PEEL_MIN_ACTIVE) {        // too few left (the queue is empty): back they go
+            if (d.live) {
+                d.cx = r.cx; d.cy = r.cy; d.cz = r.cz; d.fx = r.fx; d.fy = r.fy; d.fz = r.fz;
+                peelq_put(q, cnt + __popc(act & ((1u << lane) - 1u)), d);
+            }
+            cnt += __popc(act);
+            __syncwarp();
+            return;
+        }
+        if (d.live) {
+            const Cell c = load_cell(p, dda_linear(r, p.g));
+            const int st = peel_cell<HUBBLE>(p, s_tab, r, c, d.tau, d.V, n_cells);
+            if (st != PEEL_NEXT) {
+                if (st == PEEL_LEFT) peel_deposit(p, d.pix, d.V, d.tau, d.phat, true);
+                d.live = false;
+            }
+        }
+    }
+}
+
 // The drain kernel: launched behind walk_kernel on the same stream.  Each warp pops one parked packet at a time from the
 // global pool and walks it to its end, all 32 lanes on that one packet (see above).  4 warps per CTA — one per SM
 // sub-partition — and a register budget of its own (the walk kernel is held to 80 registers by its occupancy).
@@ -176,6 +260,7 @@ template <bool HUBBLE, bool PEEL, bool GL>
 __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_constant__ WalkParams p) {
     __shared__ BlockTallies sh;
     __shared__ float4 s_win[DRAIN_WARPS][32 * WIN_STRIDE / 4];
+    __shared__ uint32_t sh_peelq[PEEL ? DRAIN_WARPS * PEELQ_CAP * PEELQ_WORDS : 1];
     voigt_table_load(sh.voigt);
     for (int i = threadIdx.x; i < N_COUNTERS; i += blockDim.x) sh.counters[i] = 0ull;
     for (int i = threadIdx.x; i < 64; i += blockDim.x) sh.nscat_hist[i] = 0u;
@@ -187,6 +272,13 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
     float4* win = s_win[threadIdx.x >> 5];
     const unsigned long long n_pool = *p.pool_count;
     uint32_t pr = 0, pc = 0, ds = 0;
+    // Peel rays are queued whole and served 32 at a time, one per lane: a ray is ~230 of the ~900 dependent
+    // instructions of a scattering but nothing in the packet's walk waits for it — the one place where this warp's lanes do
+    // different work.
+    uint32_t* const peelq = sh_peelq + (PEEL ? (threadIdx.x >> 5) * PEELQ_CAP * PEELQ_WORDS : 0);
+    int peelq_cnt = 0;
+    PeelPend pend;
+    pend.live = false;
     const int need0 = p.doublet_on ? 4 : 3;                   // blocks one scattering takes at least: [select,] trial, 2 x finish
     Packet k;
     for (;;) {
@@ -261,12 +353,24 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
                 d.tau_next = a1.z; d.r_mu = u1.y; d.mu_dip = a1.w;
                 d.sphi = a2.x; d.cphi = a2.y; d.nl_p1 = a2.z;
                 d.spsi = b3.x; d.cpsi = b3.y; d.u_dust = u2.y; d.u_mix = u2.z; d.u_alb = u2.w;
-                const int ev = finish_scatter<HUBBLE, PEEL, true>(p, sh.voigt, k, d, pr, pc, lane == 0);
+                uint32_t none = 0;
+                const int ev = finish_scatter<HUBBLE, PEEL, true, PEEL_QUEUED>(p, sh.voigt, k, d, pr, none, lane == 0, &pend);
+                if (PEEL && pend.live) {                      // warp-uniform: every lane holds the same ray
+                    if (lane == 0) peelq_put(peelq, peelq_cnt, pend);
+                    pend.live = false;
+                    ++peelq_cnt;
+                    __syncwarp();
+                    if (peelq_cnt >= PEELQ_SERVE) peelq_serve<HUBBLE>(p, sh.voigt, peelq, peelq_cnt, pc, false, lane);
+                }
                 if (ev == EV_DUST_SCATTERED) ++ds;
                 else if (ev != EV_SCATTERED) { if (lane == 0) tally_packet(p, sh, ev, k); break; }
                 st = LS_MARCH;
             }
         }
+    }
+    if (PEEL) {
+        if (peelq_cnt > 0) peelq_serve<HUBBLE>(p, sh.voigt, peelq, peelq_cnt, pc, true, lane);
+        pc = __reduce_add_sync(0xffffffffu, pc);               // cells are counted by the lane that marched them
     }
     if (lane == 0) {
         atomicAdd(&sh.counters[CT_PEEL_RAYS], (unsigned long long)pr);
@@ -286,6 +390,7 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
 template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL>
 __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __grid_constant__ WalkParams p) {
     __shared__ BlockTallies sh;
+    __shared__ uint32_t sh_peelq[PEEL ? (WALK_THREADS / 32) * PEELQ_CAP * PEELQ_WORDS : 1];
     if (threadIdx.x == 0) atomicMin(p.t_start, global_timer_ns());
     voigt_table_load(sh.voigt);
     for (int i = threadIdx.x; i < N_COUNTERS; i += blockDim.x) sh.counters[i] = 0ull;
@@ -294,6 +399,10 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
     for (int i = threadIdx.x; i < p.spec_bins + 2; i += blockDim.x) sh.spectrum[i] = 0u;
     __syncthreads();
 
+    uint32_t* const peelq = sh_peelq + (PEEL ? (threadIdx.x >> 5) * PEELQ_CAP * PEELQ_WORDS : 0);   // this warp's queue
+    int peelq_cnt = 0;                                        // warp-uniform
+    PeelPend pend;
+    pend.live = false;
     constexpr bool EARLY = MIN_CTAS >= 4;                     // the variant launched for grids beyond L2
     const unsigned lane = threadIdx.x & 31u;
     const uint32_t k0 = (uint32_t)p.seed, k1 = (uint32_t)(p.seed >> 32);   // Philox key = seed (reading A16)
@@ -324,12 +433,16 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
                     else emit_packet(p, k, p.id_offset + i, k0, k1, dV);
                     if (PEEL) {
                         ++peel_rays;
-                        peel_ray<HUBBLE, true>(p, sh.voigt, k.ray, k.cell,
+                        peel_ray<HUBBLE, PEEL_FIRST>(p, sh.voigt, k.ray, k.cell,
                                          dot3(k.cell.vx, k.cell.vy, k.cell.vz, p.kobs[0], p.kobs[1], p.kobs[2]) + dV, 1.f,
-                                         peel_cells, true);
+                                         peel_cells, true, &pend);
                     }
                     state = LS_MARCH;
                 }
+            }
+            if (PEEL) {
+                peelq_push(peelq, peelq_cnt, pend, lane);
+                if (peelq_cnt >= PEELQ_SERVE) peelq_serve<HUBBLE>(p, sh.voigt, peelq, peelq_cnt, peel_cells, false, lane);
             }
             if (__any_sync(0xffffffffu, state == LS_OUT)) {
                 // the queue is empty: from here on the launch only drains the packets in flight
@@ -388,13 +501,18 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
             if (state == LS_FINISH) {
                 const float4 s1 = k.rng.next4(k0, k1), s2 = k.rng.next4(k0, k1);
                 const FinDraws d = fin_draws(s1, s2);
-                const int ev = finish_scatter<HUBBLE, PEEL, false>(p, sh.voigt, k, d, peel_rays, peel_cells, true);
+                const int ev = finish_scatter<HUBBLE, PEEL, false, PEEL_FIRST>(p, sh.voigt, k, d, peel_rays, peel_cells, true, &pend);
                 if (ev == EV_SCATTERED) state = LS_MARCH;
                 else if (ev == EV_DUST_SCATTERED) { state = LS_MARCH; ++dust_scat; }
                 else { tally_packet(p, sh, ev, k); state = LS_IDLE; }
             }
+            if (PEEL) {
+                peelq_push(peelq, peelq_cnt, pend, lane);
+                if (peelq_cnt >= PEELQ_SERVE) peelq_serve<HUBBLE>(p, sh.voigt, peelq, peelq_cnt, peel_cells, false, lane);
+            }
         }
     }
+    if (PEEL && peelq_cnt > 0) peelq_serve<HUBBLE>(p, sh.voigt, peelq, peelq_cnt, peel_cells, true, lane);
 
     // ---- flush the block's tallies with global atomics ----
     atomicAdd(&sh.counters[CT_PEEL_RAYS], (unsigned long long)peel_rays);

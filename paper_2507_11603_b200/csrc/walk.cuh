@@ -131,55 +131,106 @@ __device__ __forceinline__ float cell_opacity(const WalkParams& p, const float2*
 // velocity offset V_o by the same march (a4-a6), dropped beyond tau_peel_max (reading A13); added to
 // (pixel of the starting point projected perpendicular to k_obs, spectral bin of dv = -V at the box face).  `add` is
 // false on the lanes that only shadow a packet in the cooperative drain (one lane tallies).
-template <bool HUBBLE>
-__device__ __forceinline__ void peel_ray_body(const WalkParams& p, const float2* s_tab, const Ray& at, const Cell& own, float V_o,
-                                              float phat, uint32_t& n_cells, bool add) {
+// The ray is written as three steps shared by the two ways it is run: whole (peel_ray_body: the drain kernel and the
+// emission of a lone packet) and deferred (walk kernel: the first cell in place, the rest queued).
+
+// Pixel of the ray's starting point; -1 if it projects outside the image.
+__device__ __forceinline__ int peel_pixel(const WalkParams& p, const Ray& at) {
     const float px0 = (float)at.cx + at.fx - 0.5f * (float)p.g.nx;
     const float py0 = (float)at.cy + at.fy - 0.5f * (float)p.g.ny;
     const float pz0 = (float)at.cz + at.fz - 0.5f * (float)p.g.nz;
     const float px = fmaf(dot3(px0, py0, pz0, p.img1[0], p.img1[1], p.img1[2]), p.peel_inv_width, 0.5f) * (float)p.peel_nx;
     const float py = fmaf(dot3(px0, py0, pz0, p.img2[0], p.img2[1], p.img2[2]), p.peel_inv_width, 0.5f) * (float)p.peel_ny;
-    if (!(px >= 0.f && px < (float)p.peel_nx && py >= 0.f && py < (float)p.peel_ny)) return;
-    Ray r = at;
-    r.kx = p.kobs[0]; r.ky = p.kobs[1]; r.kz = p.kobs[2];     // 1 / k_obs: IEEE quotients made once on the host
-    r.ix = p.kobs_inv[0]; r.iy = p.kobs_inv[1]; r.iz = p.kobs_inv[2];
-    float tau = 0.f, V = V_o;
-    bool first = true;
-    for (;;) {
-        float len;
-        const int ex = dda_next_face(r, p.g, len);
-        if (!(len < CUDART_INF_F)) return;                    // reading A24: never reaches a box face -> dropped
-        // the ray starts in the packet's own cell, whose derived properties the packet already holds (most rays end there)
-        const Cell c = first ? own : load_cell(p, dda_linear(r, p.g));
-        first = false;
-        const float vk = dot3(c.vx, c.vy, c.vz, r.kx, r.ky, r.kz);
-        float dtau, s_hit, kt;
-        // the ray is dropped beyond tau_peel_max (reading A13): asking the segment for no more than what is left to the
-        // cap lets it stop at the sub-step that reaches it instead of integrating the whole cell
-        ++n_cells;
-        float k2;
-        if (integrate_segment<HUBBLE>(p, s_tab, c, V, vk, len, fmaf(p.tau_peel_max - tau, 1.0000002f, 1e-30f), dtau, s_hit, kt, k2)) return;
-        tau += dtau;
-        if (HUBBLE) V = fmaf(-p.hubble, len, V);
-        if (tau > p.tau_peel_max) return;
-        // peel rays leave through the first box face they meet, periodic or not
-        const float ke = ex == 0 ? r.kx : ex == 1 ? r.ky : r.kz;
-        const int cn = (ex == 0 ? r.cx : ex == 1 ? r.cy : r.cz) + (ke > 0.f ? 1 : -1);
-        const int nn = ex == 0 ? p.g.nx : ex == 1 ? p.g.ny : p.g.nz;
-        if (cn < 0 || cn >= nn) break;
-        dda_cross(r, p.g, ex, len);
-    }
+    if (!(px >= 0.f && px < (float)p.peel_nx && py >= 0.f && py < (float)p.peel_ny)) return -1;
+    return (int)py * p.peel_nx + (int)px;
+}
+
+enum : int { PEEL_DROPPED = 0, PEEL_LEFT = 1, PEEL_NEXT = 2 };
+
+// One cell of the ray (r along k_obs, c = the gas of r's cell): PEEL_DROPPED beyond tau_peel_max (or a ray that never
+// meets a face, reading A24), PEEL_LEFT at the box face (tau, V final), PEEL_NEXT after stepping into the next cell.
+template <bool HUBBLE>
+__device__ __forceinline__ int peel_cell(const WalkParams& p, const float2* s_tab, Ray& r, const Cell& c, float& tau, float& V,
+                                         uint32_t& n_cells) {
+    float len;
+    const int ex = dda_next_face(r, p.g, len);
+    if (!(len < CUDART_INF_F)) return PEEL_DROPPED;
+    const float vk = dot3(c.vx, c.vy, c.vz, r.kx, r.ky, r.kz);
+    float dtau, s_hit, kt;
+    // the ray is dropped beyond tau_peel_max (reading A13): asking the segment for no more than what is left to the
+    // cap lets it stop at the sub-step that reaches it instead of integrating the whole cell
+    ++n_cells;
+    float k2;
+    if (integrate_segment<HUBBLE>(p, s_tab, c, V, vk, len, fmaf(p.tau_peel_max - tau, 1.0000002f, 1e-30f), dtau, s_hit, kt, k2)) return PEEL_DROPPED;
+    tau += dtau;
+    if (HUBBLE) V = fmaf(-p.hubble, len, V);
+    if (tau > p.tau_peel_max) return PEEL_DROPPED;
+    // peel rays leave through the first box face they meet, periodic or not
+    const float ke = ex == 0 ? r.kx : ex == 1 ? r.ky : r.kz;
+    const int cn = (ex == 0 ? r.cx : ex == 1 ? r.cy : r.cz) + (ke > 0.f ? 1 : -1);
+    const int nn = ex == 0 ? p.g.nx : ex == 1 ? p.g.ny : p.g.nz;
+    if (cn < 0 || cn >= nn) return PEEL_LEFT;
+    dda_cross(r, p.g, ex, len);
+    return PEEL_NEXT;
+}
+
+__device__ __forceinline__ void peel_deposit(const WalkParams& p, int pix, float V, float tau, float phat, bool add) {
     const int iv = (int)floorf((-V - p.peel_v_lo) * p.peel_inv_dv);
     if (iv < 0 || iv >= p.peel_nv) return;
     const float w = phat * __expf(-tau);
     const unsigned long long q = (unsigned long long)__float2ull_rn(w * (float)CUBE_FIXED_SCALE);
-    if (q && add) atomicAdd(p.cube + ((size_t)(int)py * p.peel_nx + (int)px) * p.peel_nv + iv, q);
+    if (q && add) atomicAdd(p.cube + (size_t)pix * p.peel_nv + iv, q);
+}
+
+__device__ __forceinline__ void peel_ray_direction(const WalkParams& p, Ray& r) {
+    r.kx = p.kobs[0]; r.ky = p.kobs[1]; r.kz = p.kobs[2];     // 1 / k_obs: IEEE quotients made once on the host
+    r.ix = p.kobs_inv[0]; r.iy = p.kobs_inv[1]; r.iz = p.kobs_inv[2];
+}
+
+template <bool HUBBLE>
+__device__ __forceinline__ void peel_ray_body(const WalkParams& p, const float2* s_tab, const Ray& at, const Cell& own, float V_o,
+                                              float phat, uint32_t& n_cells, bool add) {
+    const int pix = peel_pixel(p, at);
+    if (pix < 0) return;
+    Ray r = at;
+    peel_ray_direction(p, r);
+    float tau = 0.f, V = V_o;
+    // the ray starts in the packet's own cell, whose derived properties the packet already holds (most rays end there)
+    int st = peel_cell<HUBBLE>(p, s_tab, r, own, tau, V, n_cells);
+    while (st == PEEL_NEXT) {
+        const Cell c = load_cell(p, dda_linear(r, p.g));
+        st = peel_cell<HUBBLE>(p, s_tab, r, c, tau, V, n_cells);
+    }
+    if (st == PEEL_LEFT) peel_deposit(p, pix, V, tau, phat, add);
+}
+
+// A peel ray that left its first cell, waiting in the walk kernel's per-warp queue for enough company.
+struct PeelPend {
+    int cx, cy, cz;
+    float fx, fy, fz;
+    float tau, V, phat;
+    int pix;
+    bool live;
+};
+
+// Deferred form: the first cell only; a ray that goes on is handed back in `pend` (live = true).
+template <bool HUBBLE>
+__device__ __forceinline__ void peel_ray_first(const WalkParams& p, const float2* s_tab, const Ray& at, const Cell& own, float V_o,
+                                               float phat, uint32_t& n_cells, bool add, PeelPend& pend) {
+    const int pix = peel_pixel(p, at);
+    if (pix < 0) return;
+    Ray r = at;
+    peel_ray_direction(p, r);
+    float tau = 0.f, V = V_o;
+    const int st = peel_cell<HUBBLE>(p, s_tab, r, own, tau, V, n_cells);
+    if (st == PEEL_LEFT) peel_deposit(p, pix, V, tau, phat, add);
+    else if (st == PEEL_NEXT) {
+        pend.cx = r.cx; pend.cy = r.cy; pend.cz = r.cz; pend.fx = r.fx; pend.fy = r.fy; pend.fz = r.fz;
+        pend.tau = tau; pend.V = V; pend.phat = phat; pend.pix = pix; pend.live = true;
+    }
 }
 
 // INLINE: the drain kernel has registers to spare and walks one packet per warp, where a call's spills are pure latency.
-template <bool HUBBLE, bool INLINE>
-__device__ __forceinline__ void peel_ray(const WalkParams& p, const float2* s_tab, const Ray& at, const Cell& own, float V_o,
-                                         float phat, uint32_t& n_cells, bool add);
 
 template <bool HUBBLE>
 __device__ __noinline__ void peel_ray_call(const WalkParams& p, const float2* s_tab, const Ray& at, const Cell& own, float V_o,
@@ -187,10 +238,20 @@ __device__ __noinline__ void peel_ray_call(const WalkParams& p, const float2* s_
     peel_ray_body<HUBBLE>(p, s_tab, at, own, V_o, phat, n_cells, add);
 }
 
-template <bool HUBBLE, bool INLINE>
+// How a caller runs the ray: PEEL_CALL / PEEL_INLINE = whole and in place (out of line / inlined), PEEL_FIRST = the first
+// cell in place and the rest handed back in `pend` (walk kernel), PEEL_QUEUED = nothing in place, the whole ray handed back
+// (drain kernel: the ray is off the packet's serial chain, and 32 of them are marched side by side).
+enum : int { PEEL_CALL = 0, PEEL_INLINE = 1, PEEL_FIRST = 2, PEEL_QUEUED = 3 };
+constexpr int PEEL_PIX_UNSET = -2;                     // a queued ray whose pixel is still to be found
+
+template <bool HUBBLE, int MODE>
 __device__ __forceinline__ void peel_ray(const WalkParams& p, const float2* s_tab, const Ray& at, const Cell& own, float V_o,
-                                         float phat, uint32_t& n_cells, bool add) {
-    if (INLINE) peel_ray_body<HUBBLE>(p, s_tab, at, own, V_o, phat, n_cells, add);
+                                         float phat, uint32_t& n_cells, bool add, PeelPend* pend) {
+    if (MODE == PEEL_QUEUED) {
+        pend->cx = at.cx; pend->cy = at.cy; pend->cz = at.cz; pend->fx = at.fx; pend->fy = at.fy; pend->fz = at.fz;
+        pend->tau = 0.f; pend->V = V_o; pend->phat = phat; pend->pix = PEEL_PIX_UNSET; pend->live = true;
+    } else if (MODE == PEEL_FIRST) peel_ray_first<HUBBLE>(p, s_tab, at, own, V_o, phat, n_cells, add, *pend);
+    else if (MODE == PEEL_INLINE) peel_ray_body<HUBBLE>(p, s_tab, at, own, V_o, phat, n_cells, add);
     else peel_ray_call<HUBBLE>(p, s_tab, at, own, V_o, phat, n_cells, add);
 }
 
@@ -449,9 +510,9 @@ __device__ __forceinline__ float line_a(const WalkParams& p, const Packet& k) { 
 // a7, a9-a12: the interaction itself (PAPER.md 2.3.1): dust or line, u_perp (Eq. 5, core-skipping
 // PAPER.md:244), phase function, rotation, Eq. 7 with the recoil dropped, peel-off
 // before k' is adopted, new tau_target.  Returns EV_ABSORBED / EV_TERMINATED / EV_CAPPED / EV_SCATTERED.
-template <bool HUBBLE, bool PEEL, bool PRE>
+template <bool HUBBLE, bool PEEL, bool PRE, int PMODE = PEEL_INLINE>
 __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2* s_tab, Packet& k, const FinDraws& d,
-                                              uint32_t& peel_rays, uint32_t& peel_cells, bool add) {
+                                              uint32_t& peel_rays, uint32_t& peel_cells, bool add, PeelPend* pend = nullptr) {
     const float kx = k.ray.kx, ky = k.ray.ky, kz = k.ray.kz;
     const Cell& c = k.cell;
     if (p.has_dust && (p.doublet_on ? k.line < 0 : d.u_dust * k.hit_kt < c.kd)) {
@@ -465,8 +526,8 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
         if (PEEL) {
             const float mu_o = dot3(kx, ky, kz, p.kobs[0], p.kobs[1], p.kobs[2]);
             ++peel_rays;
-            peel_ray<HUBBLE, true>(p, s_tab, k.ray, c, k.V - vk + dot3(c.vx, c.vy, c.vz, p.kobs[0], p.kobs[1], p.kobs[2]),
-                                  hg_value(p.dust_g, mu_o), peel_cells, add);
+            peel_ray<HUBBLE, PMODE>(p, s_tab, k.ray, c, k.V - vk + dot3(c.vx, c.vy, c.vz, p.kobs[0], p.kobs[1], p.kobs[2]),
+                                  hg_value(p.dust_g, mu_o), peel_cells, add, pend);
         }
         const float st = sqrtf(fmaxf(0.f, fmaf(-mu, mu, 1.f)));
         float nx = fmaf(st, fmaf(d.cphi, e1[0], d.sphi * e2[0]), mu * kx);
@@ -505,7 +566,7 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
         const float V_o = fmaf(x_o, c.vth, dot3(c.vx, c.vy, c.vz, p.kobs[0], p.kobs[1], p.kobs[2])) + dv_line;
         ++peel_rays;
         // mix: the sampled branch weights the ray (unbiased; reading A27)
-        peel_ray<HUBBLE, true>(p, s_tab, k.ray, c, V_o, is_dipole ? 0.75f * fmaf(mu_o, mu_o, 1.f) : 1.f, peel_cells, add);
+        peel_ray<HUBBLE, PMODE>(p, s_tab, k.ray, c, V_o, is_dipole ? 0.75f * fmaf(mu_o, mu_o, 1.f) : 1.f, peel_cells, add, pend);
     }
     const float st = sqrtf(fmaxf(0.f, fmaf(-mu, mu, 1.f)));
     float nx = fmaf(st, fmaf(d.cphi, e1[0], d.sphi * e2[0]), mu * kx);

@@ -608,6 +608,31 @@ def test_drain_kernel_is_bit_identical(thor):
             assert np.array_equal(a["cube"], b["cube"]), w["tag"]
 
 
+def test_deferred_peel_rays_are_bit_identical(thor):
+    """The walk kernel marches a peel ray's first cell in place and queues the rest per warp; the drain kernel
+    marches every ray in place, start to end.  A packet launched alone is parked at once and walked by the drain kernel, so
+    the cube of ONE launch of N packets must equal, bit for bit (fixed point), the cube accumulated over N one-packet
+    launches — in media thin enough that most rays cross many cells, with and without Hubble drift."""
+    n = 300
+    cases = [dict(W.turbulent_box(n=32, n_src=64, n_photons=n, peel_pix=16, peel_bins=20, cell_pc=2e-4), tag="turb"),
+             dict(W.cosmic_web(n=32, n_src=64, n_photons=n, mean_n=3e-9, map_pix=16, v_max=40.0), tag="web")]
+    for w in cases:
+        opts = dict(w["opts"], max_scatter=2000)
+        whole = thor.run_workload(dict(w, opts=opts), drain_mode=1)          # walk kernel only: every ray deferred
+        assert whole["counters"]["peel_cells"] > 3 * whole["counters"]["peel_rays"], w["tag"]   # rays do go on
+        ctx = thor.Context.from_workload(w["grid"])
+        try:
+            ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
+            for i in range(n):
+                ctx.run(1, w["seed"], dict(opts, photon_id_offset=i, accumulate=1 if i else 0))
+            cube, c = ctx.cube(), ctx.counters()
+        finally:
+            ctx.close()
+        assert np.array_equal(cube, whole["cube"]), w["tag"]
+        assert c["peel_cells"] == whole["counters"]["peel_cells"] and c["peel_rays"] == whole["counters"]["peel_rays"]
+        assert c["scatterings"] == whole["counters"]["scatterings"]
+
+
 def test_mean_scattering_count_within_one_percent(thor, oracle):
     """BASELINE.json's bar as stated: mean scattering count within 1 % — on a rung where the standard error lets it bind
     (reading A23): tau0 = 1e2, 4e5 packets per side, 3 SE = 0.6 %.  Plain |dmean| <= 1 %, no SE allowance."""
