@@ -161,6 +161,33 @@ void thor_opts_default(thor_opts *o);
  * allocated; THOR_ERR_CUDA. */
 thor_status thor_run(thor_ctx *ctx, unsigned long long n_photons, unsigned long long seed, const thor_opts *opts);
 
+/* thor_run for callers that cannot allocate device memory at run time (code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): the same walk (same kernels, same packets: tallies equal thor_run's bit for bit),
+ * but this call makes NO cudaMalloc / cudaFree and no allocating library call.  thor_run allocates its parked-packet pool,
+ * its cube and its raw records on first use; here the kernels' scratch — photon counter, timers, pool counters, the pool
+ * of parked packets and its ordering — lives in ONE file-scope `static __device__` array of
+ * THOR_NOALLOC_SCRATCH_BYTES (4.0 MB) that every GPU which loads the library holds until exit, and the tallies go straight
+ * into buffers the caller owns:
+ *   spectrum_out   DEVICE uint64[opts->spec_bins + 2]   (layout of THOR_TALLY_SPECTRUM; may be NULL if spec_bins == 0)
+ *   counters_out   DEVICE uint64[THOR_N_COUNTERS]
+ *   nscat_hist_out DEVICE uint64[64]                    (layout of THOR_TALLY_NSCAT_HIST)
+ * all three overwritten (cleared, then filled).  ctx is a grid context with its sources set (that set-up allocates; do
+ * it beforehand).  Asynchronous: the clears and kernels are enqueued on the context's stream and the call returns; the
+ * outputs are valid once that stream has drained.  The context's own tallies, thor_tally_get and thor_last_run_* are not
+ * touched.
+ * Limits: the pool is sized for GPUs of up to THOR_NOALLOC_MAX_SM multiprocessors — a larger GPU is refused with
+ * THOR_ERR_ARG and a message saying so; peel-off (its cube would have to be allocated), raw_output, accumulate and
+ * gridless datasets are refused with THOR_ERR_UNSUPPORTED.  Other errors as thor_run.
+ * Every call on a GPU shares the one array, which keeps the last call's contents (each call clears the words that must
+ * start at zero).  Calls on the same context are ordered by its stream; calls that OVERLAP on the GPU — two contexts on
+ * different streams of one device — race on the scratch and give wrong tallies: serialise them.  The first call on a
+ * device looks the array's device address up (cudaGetSymbolAddress: no allocation): make it outside a capture. */
+#define THOR_NOALLOC_MAX_SM 160
+#define THOR_NOALLOC_SCRATCH_BYTES (256 + 160 * 128 * 4 + 160 * 128 * 192)
+thor_status thor_run_noalloc(thor_ctx *ctx, unsigned long long n_photons, unsigned long long seed, const thor_opts *opts,
+                             unsigned long long *spectrum_out, unsigned long long *counters_out,
+                             unsigned long long *nscat_hist_out);
+
 /* Duration of the walk kernel of the last thor_run in milliseconds, from CUDA events on the context's stream. */
 thor_status thor_last_run_ms(const thor_ctx *ctx, float *ms);
 

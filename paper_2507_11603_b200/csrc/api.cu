@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -530,6 +531,111 @@ static thor::WalkParams grid_params(const thor_ctx* ctx) {
     p.cell_cm = (float)ctx->cell_cm;
     p.gl_geom = -1;
     return p;
+}
+
+// ---- thor_run_noalloc: the walk for callers that cannot allocate at run time (include/thor.h) -------------------------------
+// The kernels' scratch in one file-scope device array: [0, 256) six 64-bit words (photon counter, t_start, t_dry, max_nscat,
+// pool_count, pool_next), then the pool ordering (one uint32 per slot), then the parked packets (48 words per slot).
+// Every GPU that loads the library holds these 4.0 MB until exit; every call shares them.
+static constexpr long long NOALLOC_SLOTS = (long long)THOR_NOALLOC_MAX_SM * 128;       // walk_pool_slots(THOR_NOALLOC_MAX_SM)
+static constexpr int NOALLOC_PK_WORDS = 48;
+static constexpr size_t NOALLOC_ORDER_OFF = 256, NOALLOC_POOL_OFF = NOALLOC_ORDER_OFF + (size_t)NOALLOC_SLOTS * 4,
+                        NOALLOC_BYTES = NOALLOC_POOL_OFF + (size_t)NOALLOC_SLOTS * NOALLOC_PK_WORDS * 4;
+static_assert(NOALLOC_BYTES == THOR_NOALLOC_SCRATCH_BYTES, "thor.h states the size of the scratch array");
+static_assert(NOALLOC_POOL_OFF % 256 == 0, "the pool starts on a 256-byte boundary");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_BYTES];
+
+// In host code `g_noalloc_scratch` is only a handle: its device address is looked up once per device, with that device
+// current (the caller holds a DevGuard), and cached.
+static cudaError_t noalloc_scratch_address(int device, unsigned char** out) {
+    static std::mutex mu;
+    static unsigned char* addr[64] = {};
+    if (device < 0 || device >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[device]) {
+        void* sym = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&sym, g_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        addr[device] = static_cast<unsigned char*>(sym);
+    }
+    *out = addr[device];
+    return cudaSuccess;
+}
+
+extern "C" thor_status thor_run_noalloc(thor_ctx* ctx, unsigned long long n_photons, unsigned long long seed, const thor_opts* opts,
+                                        unsigned long long* spectrum_out, unsigned long long* counters_out,
+                                        unsigned long long* nscat_hist_out) {
+    if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_run_noalloc: ctx is NULL");
+    if (ctx->gridless) return fail(ctx, THOR_ERR_UNSUPPORTED, "thor_run_noalloc: gridless datasets are not supported (use thor_run)");
+    if (ctx->n_src <= 0) return fail(ctx, THOR_ERR_STATE, "thor_run_noalloc: call thor_sources_set first");
+    thor_opts o;
+    thor_opts_default(&o);
+    if (opts) {
+        if (opts->struct_size == 0 || opts->struct_size > sizeof o) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: opts->struct_size is not set (use thor_opts_default)");
+        std::memcpy(&o, opts, opts->struct_size);
+        o.struct_size = (uint32_t)sizeof o;
+    }
+    if (o.peel_on || o.raw_output || o.accumulate)
+        return fail(ctx, THOR_ERR_UNSUPPORTED, "thor_run_noalloc: peel-off, raw_output and accumulate need memory this entry point may not allocate (use thor_run)");
+    if (!counters_out || !nscat_hist_out || (o.spec_bins > 0 && !spectrum_out)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: an output buffer is NULL");
+    if (!phase_ok(o.phase_core) || !phase_ok(o.phase_wing)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: unknown phase function");
+    if (o.core_skip_mode < 0 || o.core_skip_mode > 2 || !(o.x_crit >= 0)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: bad core-skip options");
+    if (o.spec_bins < 0 || o.spec_bins > 4096) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: spec_bins must be in [0, 4096]");
+    if (o.spec_bins > 0 && !(o.spec_hi > o.spec_lo)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: spec_hi must exceed spec_lo");
+    if (o.spec_mode != 0 && o.spec_mode != 1) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: spec_mode must be 0 or 1");
+    if (o.spec_mode == 0 && !(o.spec_T_ref > 0)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: spec_T_ref must be > 0");
+    if ((o.walk_variant != 0 && o.walk_variant != 3 && o.walk_variant != 4) || (o.drain_mode != 0 && o.drain_mode != 1)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: bad walk_variant / drain_mode");
+    if (!(o.dust_albedo >= 0 && o.dust_albedo <= 1) || !(o.dust_g >= -1 && o.dust_g <= 1)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: dust_albedo must be in [0, 1] and dust_g in [-1, 1]");
+    if (o.doublet_on && (!std::isfinite(o.doublet_dv_kms) || !(o.doublet_sigma_ratio >= 0) || !(o.doublet_a_ratio > 0) || !std::isfinite(o.doublet_sigma_ratio) || !std::isfinite(o.doublet_a_ratio)))
+        return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: bad doublet options");
+    if (!(o.hubble_eps > 0) || !(o.v_max_kms >= 0) || !std::isfinite(o.hubble_kms_per_cell)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: bad Hubble / v_max options");
+    if (ctx->g.periodic == 7u && ctx->g.frozen != 7u && o.max_crossings == 0)
+        return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: the grid is periodic on all three axes (no packet can leave it): set opts.max_crossings");
+    // the one size this entry point cannot grow with: the pool holds walk_pool_slots(n_sm) parked packets
+    const long long slots = thor::walk_pool_slots(ctx->n_sm);
+    if (ctx->n_sm > THOR_NOALLOC_MAX_SM || slots > NOALLOC_SLOTS || thor::walk_pool_words() > NOALLOC_PK_WORDS)
+        return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: this GPU has " + std::to_string(ctx->n_sm) + " multiprocessors and needs " + std::to_string(slots) +
+                                       " pool slots; the static scratch holds " + std::to_string(NOALLOC_SLOTS) + " (THOR_NOALLOC_MAX_SM = " +
+                                       std::to_string(THOR_NOALLOC_MAX_SM) + "): use thor_run");
+    const thor::LyaConstants K = thor::lya_constants();
+    thor::WalkParams p = grid_params(ctx);
+    p.max_crossings = (o.max_crossings && o.max_crossings < 0xffffffffull) ? (unsigned)o.max_crossings : 0xffffffffu;
+    p.n_src = ctx->n_src; p.src_pos = ctx->d_src_pos; p.src_sigma = ctx->d_src_sigma; p.src_cdf = ctx->d_src_cdf;
+    p.phase_core = o.phase_core; p.phase_wing = o.phase_wing; p.phase_frame = o.phase_frame;
+    p.phase_split_x = (float)o.phase_split_x;
+    p.core_skip_mode = o.core_skip_mode; p.x_crit = (float)o.x_crit;
+    p.spec_mode = o.spec_mode; p.spec_bins = o.spec_bins;
+    p.spec_inv_vth_ref = (float)(1.0 / (K.c_vth * std::sqrt(o.spec_T_ref)));
+    p.spec_lo = (float)o.spec_lo;
+    p.spec_inv_width = o.spec_bins > 0 ? (float)(o.spec_bins / (o.spec_hi - o.spec_lo)) : 0.f;
+    p.hubble = (float)o.hubble_kms_per_cell; p.hubble_eps = (float)o.hubble_eps; p.v_max = (float)o.v_max_kms;
+    p.peel_on = 0;
+    p.id_offset = o.photon_id_offset; p.n_photons = n_photons; p.seed = seed; p.max_scatter = o.max_scatter;
+    p.max_scatter32 = o.max_scatter > 0xffffffffull ? 0xffffffffu : (unsigned)o.max_scatter;
+    p.walk_variant = o.walk_variant;
+    p.dust_albedo = (float)o.dust_albedo; p.dust_g = (float)o.dust_g;
+    p.doublet_on = o.doublet_on ? 1 : 0;
+    p.db_dv = (float)o.doublet_dv_kms; p.db_rs = (float)o.doublet_sigma_ratio; p.db_ra = (float)o.doublet_a_ratio;
+    DevGuard dev_guard(ctx->device);
+    unsigned char* scratch = nullptr;
+    CU(noalloc_scratch_address(ctx->device, &scratch));
+    unsigned long long* small = reinterpret_cast<unsigned long long*>(scratch);
+    // what must start at zero: the photon counter, max_nscat, the pool counters (words 0, 3, 4, 5); the timers start at ~0.
+    // The pool and its ordering need no clearing: the kernels read only the slots this launch has written.
+    CU(cudaMemsetAsync(small, 0, 6 * sizeof(unsigned long long), ctx->stream));
+    CU(cudaMemsetAsync(small + 1, 0xFF, 2 * sizeof(unsigned long long), ctx->stream));
+    CU(cudaMemsetAsync(counters_out, 0, thor::N_COUNTERS * sizeof(unsigned long long), ctx->stream));
+    CU(cudaMemsetAsync(nscat_hist_out, 0, 64 * sizeof(unsigned long long), ctx->stream));
+    if (o.spec_bins > 0) CU(cudaMemsetAsync(spectrum_out, 0, (size_t)(o.spec_bins + 2) * sizeof(unsigned long long), ctx->stream));
+    p.next_photon = small + 0; p.t_start = small + 1; p.t_dry = small + 2; p.max_nscat = small + 3;
+    p.pool_count = small + 4; p.pool_next = small + 5;
+    p.pool_order = reinterpret_cast<unsigned int*>(scratch + NOALLOC_ORDER_OFF);
+    p.pool = o.drain_mode == 0 ? reinterpret_cast<uint32_t*>(scratch + NOALLOC_POOL_OFF) : nullptr;
+    p.counters = counters_out; p.nscat_hist = nscat_hist_out; p.spectrum = spectrum_out;
+    p.cube = nullptr; p.raw = nullptr;
+    int blocks = 0;
+    if (n_photons > 0) CU(thor::launch_walk(p, ctx->n_sm, ctx->stream, &blocks));
+    return THOR_OK;
 }
 
 // HOST <-> DEVICE staging of the ray operators' buffers (THOR_RAYS_HOST): device twins owned for the length of one call.

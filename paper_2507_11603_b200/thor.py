@@ -19,7 +19,7 @@ COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "
                  "peel_rays", "peel_cells", "dust_scatterings"]
 RAW_DTYPE = np.dtype([("V", "<f4"), ("nscat", "<u4"), ("status", "<i4"), ("kx", "<f4"), ("ky", "<f4"), ("kz", "<f4")])
 
-EXPORTS = ["thor_grid_create", "thor_dataset_create_gridless", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run",
+EXPORTS = ["thor_grid_create", "thor_dataset_create_gridless", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run", "thor_run_noalloc",
            "thor_last_run_ms", "thor_last_run_feed_ms", "thor_last_run_max_nscat", "thor_raytrace", "thor_raytrace_ex", "thor_volume_render", "thor_volume_render_ex", "thor_slice", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_curand_philox", "thor_unit_dda_trace",
            "thor_unit_voigt", "thor_unit_scatter"]
 
@@ -89,6 +89,7 @@ def lib():
         L.thor_opts_default.argtypes = [C.POINTER(Opts)]
         L.thor_opts_default.restype = None
         L.thor_run.argtypes = [P, C.c_ulonglong, C.c_ulonglong, C.POINTER(Opts)]
+        L.thor_run_noalloc.argtypes = [P, C.c_ulonglong, C.c_ulonglong, C.POINTER(Opts), P, P, P]
         L.thor_last_run_ms.argtypes = [P, C.POINTER(f)]
         L.thor_last_run_feed_ms.argtypes = [P, C.POINTER(f)]
         L.thor_last_run_max_nscat.argtypes = [P, C.POINTER(C.c_ulonglong)]
@@ -225,6 +226,16 @@ class Context:
         self._opts = opts
         self._n = int(n_photons)
         _check(lib().thor_run(self._ctx, int(n_photons), int(seed), C.byref(opts)), self._ctx)
+
+    def run_noalloc(self, n_photons, seed, opts, spectrum_out, counters_out, nscat_hist_out):
+        """thor_run_noalloc: the same walk without any device allocation; the tallies go into the caller's torch CUDA int64
+        tensors (spectrum_out: spec_bins + 2, counters_out: len(COUNTER_NAMES), nscat_hist_out: 64).  Asynchronous on the
+        context's stream; the context's own tallies are not touched."""
+        if isinstance(opts, dict):
+            opts = make_opts(**opts)
+        ptr = lambda t: None if t is None else C.c_void_p(t.data_ptr())
+        _check(lib().thor_run_noalloc(self._ctx, int(n_photons), int(seed), C.byref(opts), ptr(spectrum_out), ptr(counters_out),
+                                      ptr(nscat_hist_out)), self._ctx)
 
     def last_run_ms(self):
         ms = C.c_float()
