@@ -79,25 +79,28 @@ __device__ __forceinline__ void dda_advance_within(Ray& r, const GridDims& g, fl
 }
 
 // Cross the face found by dda_next_face.  Returns false if the ray left the grid through a non-periodic face.
+// Written with selects only: the exit axis differs from lane to lane, and per-axis branches would run each axis with a third
+// of the warp (measured on the thin `gather` workload: 20 % of the kernel's issued instructions at 6-13 of 32 lanes).
 __device__ __forceinline__ bool dda_cross(Ray& r, const GridDims& g, int ex, float len) {
-    if (ex != 0 && !(g.frozen & 1u)) r.fx = dda_move(r.fx, len, r.kx);
-    if (ex != 1 && !(g.frozen & 2u)) r.fy = dda_move(r.fy, len, r.ky);
-    if (ex != 2 && !(g.frozen & 4u)) r.fz = dda_move(r.fz, len, r.kz);
+    const float mx = (g.frozen & 1u) ? r.fx : dda_move(r.fx, len, r.kx);      // warp-uniform conditions
+    const float my = (g.frozen & 2u) ? r.fy : dda_move(r.fy, len, r.ky);
+    const float mz = (g.frozen & 4u) ? r.fz : dda_move(r.fz, len, r.kz);
     const float ke = ex == 0 ? r.kx : ex == 1 ? r.ky : r.kz;
     const int n = ex == 0 ? g.nx : ex == 1 ? g.ny : g.nz;
     const int s = ke > 0.0f ? 1 : -1;
     const float fe = s > 0 ? 0.0f : 1.0f;
     int c = (ex == 0 ? r.cx : ex == 1 ? r.cy : r.cz) + s;
-    bool inside = true;
-    if (c < 0 || c >= n) {
-        if (g.periodic & (1u << ex)) c = c < 0 ? n - 1 : 0;
-        else inside = false;
-    }
-    if (inside) {
-        if (ex == 0) { r.cx = c; r.fx = fe; }
-        else if (ex == 1) { r.cy = c; r.fy = fe; }
-        else { r.cz = c; r.fz = fe; }
-    }
+    const bool out = c < 0 || c >= n;
+    const bool wrap = (g.periodic & (1u << ex)) != 0u;
+    c = (out && wrap) ? (c < 0 ? n - 1 : 0) : c;
+    const bool inside = !out || wrap;
+    // the exit axis lands on the face of the new cell (only if there is one); the other axes move by len unless frozen
+    r.fx = ex == 0 ? (inside ? fe : r.fx) : mx;
+    r.fy = ex == 1 ? (inside ? fe : r.fy) : my;
+    r.fz = ex == 2 ? (inside ? fe : r.fz) : mz;
+    r.cx = (inside && ex == 0) ? c : r.cx;
+    r.cy = (inside && ex == 1) ? c : r.cy;
+    r.cz = (inside && ex == 2) ? c : r.cz;
     return inside;
 }
 

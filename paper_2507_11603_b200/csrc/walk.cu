@@ -27,7 +27,7 @@ constexpr int WALK_THREADS = THOR_WALK_THREADS;
 constexpr int MAX_SPEC_BINS = 4096;
 constexpr int FINISH_MIN_LANES = THOR_FINISH_MIN_LANES;
 #ifndef THOR_REFILL_MIN_LANES
-#define THOR_REFILL_MIN_LANES 8
+#define THOR_REFILL_MIN_LANES 1
 #endif
 constexpr int REFILL_MIN_LANES = THOR_REFILL_MIN_LANES;
 #ifndef THOR_COOP_MAX_LANES
@@ -416,10 +416,12 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
 
     for (;;) {
         // ---- a14 + a2/a3: refill idle lanes from the global photon counter, emit ----
-        // Refills are batched: emission is a chain of dependent loads (binary search of the source CDF, source cell
-        // gather) that stalls the whole warp, so it waits until REFILL_MIN_LANES lanes are idle (or nothing else runs).
+        // A lane is refilled as soon as it is idle (REFILL_MIN_LANES = 1).  Emission is a chain of dependent loads (binary
+        // search of the source CDF, source cell gather) run by the few lanes that need it, but waiting for 4 / 8 / 16 idle
+        // lanes before paying for it was measured slower on every workload (feed phase +7 / +16 / +36 % on config 3, +100 % on
+        // config 4 at 512^3: the idle lanes cost more than the emission's poor lane count).
         const unsigned idle = __ballot_sync(0xffffffffu, state == LS_IDLE);
-        if (more && idle && (__popc(idle) >= REFILL_MIN_LANES || idle == __ballot_sync(0xffffffffu, state == LS_IDLE || state == LS_OUT))) {
+        if (more && idle && (__popc(idle) >= REFILL_MIN_LANES || __ballot_sync(0xffffffffu, state == LS_IDLE || state == LS_OUT) == 0xffffffffu)) {
             unsigned long long base = 0;
             if (lane == 0) base = atomicAdd(p.next_photon, (unsigned long long)__popc(idle));
             base = __shfl_sync(0xffffffffu, base, 0);
