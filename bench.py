@@ -8,7 +8,10 @@ configuration, configs[4]: the 1536^3 cosmic web (72.5 GB of SoA fp32 fields gen
 library), with Hubble drift, termination at 5 Å and a 2048^2 surface-brightness map by peel-off; each step walks a STATED
 subsample of the config's 1e8 packets (config.n_photons_per_step_per_gpu of config.n_photons_subsample_of).  value =
 scatterings/s over the timed steps (whole job, all ranks), with packets/s and cell crossings/s beside it; inputs are
-resident in HBM when the timed region starts.  `e2e` is the same metric through the C-ABI with HOST buffers for what a
+resident in HBM when the timed region starts.  Steps are independent batches: up to --in-flight of them (default 3) run at
+once, each in a context, stream and host thread of its own on the shared resident grid, so that the tail of one step (a few
+long packets) overlaps the feed phase of the next; ms_per_step = timed region / steps, serial_ms_per_step = the
+warm-up steps, which run one at a time.  `e2e` is the same metric through the C-ABI with HOST buffers for what a
 step takes in and gives back (the source list in, the tallies out; the 72.5 GB grid is the resident dataset).  `roofline` is the
 issue-slot ("alu") roofline of the walk kernel (DESIGN.md §5), `roofline_hbm` the cell-gather bandwidth beside it;
 `workloads` holds the other configurations measured in the same run (configs[1], [2], [3] at 512^3, the scaled configs[0],
@@ -393,48 +396,103 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
         opts["max_scatter"] = args.max_scatter
     id0 = args.photon_id_offset
     gridless = "dataset" in w
-    ctx = thor.Context.gridless(**w["dataset"]) if gridless else thor.Context.from_workload(w["grid"], pack=pack, extra_flags=args.grid_flags)   # resident before the timed region
-    ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
-    spec_dev = torch.zeros(opts["spec_bins"] + 2, dtype=torch.int64, device="cuda")
-    cnt_dev = torch.zeros(len(thor.COUNTER_NAMES), dtype=torch.int64, device="cuda")
-    feed_ms, max_nscat = [], []
+    # Steps in flight: consecutive steps are independent batches, so up to C of them run at once, each in a context of its own
+    # on a stream of its own (one host thread each; thor_run is synchronous), all borrowing the same resident grid.  A step is
+    # tail-bound (its last seconds walk a few long packets): with several in flight the tail of one step overlaps
+    # the feed phase of the next, as in a production run of many batches.  --in-flight 1 runs them one after the other.
+    C = max(1, min(args.in_flight, steps))
+    if not gridless:                                               # small host-made grids: uploaded once, shared by every context
+        gsh = dict(w["grid"])
+        for key in ("nHI", "T", "vx", "vy", "vz", "kdust"):
+            if gsh.get(key) is not None and not isinstance(gsh[key], torch.Tensor):
+                gsh[key] = torch.from_numpy(np.ascontiguousarray(gsh[key], np.float32)).cuda()
+    streams = [torch.cuda.current_stream()] + [torch.cuda.Stream() for _ in range(C - 1)]
+    ctxs = []
+    for j in range(C):
+        with torch.cuda.stream(streams[j]):                        # the context keeps the stream it is created on
+            cx = thor.Context.gridless(**w["dataset"]) if gridless else thor.Context.from_workload(gsh, pack=pack, extra_flags=args.grid_flags)
+            cx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])   # resident before the timed region
+        ctxs.append(cx)
+    ctx = ctxs[0]
+    flush = [torch.empty(256 << 20, dtype=torch.uint8, device="cuda") for _ in range(C)]   # > 126 MB L2
+    n_spec, n_cnt = opts["spec_bins"] + 2, len(thor.COUNTER_NAMES)
+    spec_dev = [torch.zeros(n_spec, dtype=torch.int64, device="cuda") for _ in range(C)]
+    cnt_dev = [torch.zeros(n_cnt, dtype=torch.int64, device="cuda") for _ in range(C)]
+    spec_sum = [torch.zeros(n_spec, dtype=torch.int64, device="cuda") for _ in range(C)]
+    cnt_sum = [torch.zeros(n_cnt, dtype=torch.int64, device="cuda") for _ in range(C)]
 
-    def step(i):
-        # rank r walks photon ids [r n, (r+1) n) of step i's seed; tallies summed over ranks (the one exchange step)
-        ctx.run(n, w["seed"] + (i if not id0 else 0), dict(opts, photon_id_offset=id0 + rank * n))
-        ctx.tally_to_device(thor.TALLY_SPECTRUM, spec_dev)
-        ctx.tally_to_device(thor.TALLY_COUNTERS, cnt_dev)
-        shard.allreduce_tallies([spec_dev, cnt_dev])               # no-op at N = 1
-        feed_ms.append(ctx.last_run_feed_ms())
-        max_nscat.append(ctx.last_run_max_nscat())
-        return ctx.last_run_ms()
+    def step(j, i):
+        # rank r walks photon ids [r n, (r+1) n) of step i's seed
+        cx = ctxs[j]
+        cx.run(n, w["seed"] + (i if not id0 else 0), dict(opts, photon_id_offset=id0 + rank * n))
+        cx.tally_to_device(thor.TALLY_SPECTRUM, spec_dev[j])
+        cx.tally_to_device(thor.TALLY_COUNTERS, cnt_dev[j])
+        return cx.last_run_ms(), cx.last_run_feed_ms(), cx.last_run_max_nscat()
 
-    for i in range(warmup):
-        step(-1 - i)
+    serial_ms = []
+    for i in range(warmup):                                        # warm-up: one step at a time, on every context in turn
+        j = i % C
+        with torch.cuda.stream(streams[j]):
+            t0 = time.perf_counter()
+            step(j, -1 - i)
+            streams[j].synchronize()
+            serial_ms.append(1e3 * (time.perf_counter() - t0))
+    for j in range(min(warmup, C), C):                             # contexts the warm-up did not reach: a short run each
+        with torch.cuda.stream(streams[j]):
+            ctxs[j].run(min(n, 1024), w["seed"], dict(opts, photon_id_offset=id0 + rank * n))
     sampler = ClockSampler(local) if sample_clocks else None
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
     if sampler:
         sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-    kern_ms, totals = [], np.zeros(len(thor.COUNTER_NAMES), np.int64)
-    for i in range(steps):
-        flush.zero_()                                              # flush L2 between timed iterations (untimed)
-        ev[i][0].record()
-        kern_ms.append(step(i))
-        ev[i][1].record()
-        totals += cnt_dev.cpu().numpy()                            # already summed over ranks
+    kern_ms, feed_ms, max_nscat = [0.0] * steps, [0.0] * steps, [0] * steps
+    nxt, lock, errors = [0], threading.Lock(), []
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def worker(j):
+        try:
+            torch.cuda.set_device(local)
+            with torch.cuda.stream(streams[j]):
+                while True:
+                    with lock:
+                        i = nxt[0]
+                        nxt[0] += 1
+                    if i >= steps:
+                        return
+                    flush[j].zero_()                               # L2 flush before every timed step (on this step's stream)
+                    kern_ms[i], feed_ms[i], max_nscat[i] = step(j, i)
+                    spec_sum[j] += spec_dev[j]
+                    cnt_sum[j] += cnt_dev[j]
+        except Exception as e:                                     # surfaced after the join
+            errors.append(e)
+
+    ev0.record()
+    if C == 1:
+        worker(0)
+    else:
+        th = [threading.Thread(target=worker, args=(j,)) for j in range(C)]
+        [t.start() for t in th]
+        [t.join() for t in th]
+    for st in streams:
+        st.synchronize()
+    ev1.record()
     torch.cuda.synchronize()
+    if errors:
+        raise errors[0]
+    spec_tot, cnt_tot = sum(spec_sum[1:], spec_sum[0]), sum(cnt_sum[1:], cnt_sum[0])
+    shard.allreduce_tallies([spec_tot, cnt_tot])                   # the one exchange step; no-op at N = 1
     if world > 1:
         dist.barrier()
     clocks = sampler.stop() if sampler else None
-    step_ms = sum(a.elapsed_time(b) for a, b in ev)
+    totals = cnt_tot.cpu().numpy()
+    step_ms = ev0.elapsed_time(ev1)                                # the whole timed region, device clock
     t = torch.tensor([step_ms, sum(kern_ms)], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     step_ms, kernel_ms = float(t[0]), float(t[1])
+    if C > 1:
+        kernel_ms = step_ms                                        # launches overlap: the region is their span
     c = dict(zip(thor.COUNTER_NAMES, (int(v) for v in totals)))
     packets = c["escaped"] + c["absorbed"] + c["terminated"] + c["capped"]
     assert packets == n * world * steps, (packets, n, world, steps)
@@ -445,21 +503,26 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
         "metric": "lya_scatterings_per_sec", "value": c["scatterings"] / secs, "unit": "scatterings/s",
         "packets_per_sec": packets / secs, "cell_crossings_per_sec": crossings / secs,
         "steps": steps, "warmup": warmup, "ms_per_step": step_ms / steps,
+        "serial_ms_per_step": float(np.mean(serial_ms)) if serial_ms else None,
         "config": {"workload": workload_label(name), "grid": [g["nx"], g["ny"], g["nz"]], "n_photons_per_step_per_gpu": n,
                    "layout": "gridless (analytic sphere, fp64 geometry)" if gridless else "packed 32 B/cell (THOR_GRID_PACK)" if pack else "SoA fp32, borrowed",
                    "parallelism": f"photon-id shards x{world}, grid replicated",
-                   "l2": "flushed between timed iterations (256 MB memset)",
+                   "steps_in_flight": C,
+                   "steps_in_flight_note": (f"{C} independent steps at a time, each in its own context / stream / host thread on the shared resident grid; "
+                                            "ms_per_step = timed region / steps; serial_ms_per_step = the warm-up steps, run one at a time") if C > 1 else "steps run one after the other",
+                   "l2": "flushed before every timed step (256 MB memset on the step's stream)",
                    "scatterings_per_packet": c["scatterings"] / packets,
                    "crossings_per_packet": crossings / packets,
                    "rejection_iters_per_scattering": c["rejection_iters"] / max(1, c["scatterings"]),
                    "phase_functions": f"core {opts.get('phase_core', 0)} / wing {opts.get('phase_wing', 0)} (0 isotropic, 1 dipole, 2 mix)"},
         # how the kernel time splits: until the photon counter runs dry the walk is fed (throughput phase); after that
         # the launch only drains the packets in flight, and lasts as long as its longest single packet
-        "phases": {"feed_ms_per_step": float(np.mean(feed_ms[-steps:])),
-                   "drain_ms_per_step": kernel_ms / steps - float(np.mean(feed_ms[-steps:])),
-                   "longest_packet_scatterings": [int(v) for v in max_nscat[-steps:]],
+        "phases": {"feed_ms_per_step": float(np.mean(feed_ms)),
+                   "drain_ms_per_step": float(np.mean(kern_ms)) - float(np.mean(feed_ms)),
+                   "launch_ms_per_step": float(np.mean(kern_ms)),
+                   "longest_packet_scatterings": [int(v) for v in max_nscat],
                    "drain_ns_per_scattering_of_longest_packet": float(np.mean([1e6 * (k - f) / max(1, m) for k, f, m in
-                                                                               zip(kern_ms, feed_ms[-steps:], max_nscat[-steps:])])),
+                                                                               zip(kern_ms, feed_ms, max_nscat)])),
                    "source": "device %globaltimer at kernel entry and when the photon counter is first found exhausted (thor_last_run_feed_ms)"},
         "counters": c,
     }
@@ -478,7 +541,8 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
     alu = {"bound": "alu", "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "G thread-inst/s", "frac": achieved / peak,
            "traffic": traffic, "traffic_source": (tr["source"] + f"; measured at {tr['n_photons']} packets, scaled linearly to {n}") if tr else None,
            "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_hz / 1e6:.0f} MHz (clocks.max.sm), derived in DESIGN.md 5",
-           "kernel": "walk_kernel", "kernel_ms_per_launch": kernel_ms / steps,
+           "kernel": "walk_kernel + drain_kernel (one thor_run)", "kernel_ms_per_launch": kernel_ms / steps,
+           "kernel_ms_note": "CUDA events around the timed region / steps (launches of different steps overlap)" if C > 1 else "thor_last_run_ms: CUDA events around the launch on the context's stream",
            "inst_per_scattering": INST_PER_SCATTERING, "inst_per_crossing": INST_PER_CROSSING,
            "constants_source": "SURVEY.md 8(d) a-priori budgets"}
     peaks = {}
@@ -508,41 +572,73 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
             h2d += sum(g[k].nbytes for k in ("nHI", "T", "vx", "vy", "vz", "kdust") if g.get(k) is not None)
         cube_bytes = opts.get("peel_nx", 0) * opts.get("peel_ny", 0) * opts.get("peel_nv", 0) * 8 if opts.get("peel_on") else 0
         d2h = (opts["spec_bins"] + 2 + 64 + len(thor.COUNTER_NAMES)) * 8 + cube_bytes
-        e_scat, e_secs = 0, 0.0
-        e_steps = min(steps, 2)
-        for i in range(0 if not regrid else -1, e_steps):           # small grids: one untimed pass warms the re-creation path
-            flush.zero_()
-            if world > 1:
-                dist.barrier()
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            cx = thor.Context.from_workload(g, host=True, pack=pack) if regrid else ctx
-            cx.sources_set(src["pos"], src["lum"], src["sigma"])
-            cx.run(n, w["seed"] + (max(i, 0) if not id0 else 0), dict(opts, photon_id_offset=id0 + rank * n))
-            cx.spectrum(); cx.nscat_hist()
-            if cube_bytes:
-                cx.cube()
-            cc = cx.counters()
-            if regrid:
-                cx.close()
-            torch.cuda.synchronize()
-            dt = time.perf_counter() - t0
-            tt = torch.tensor([dt, float(cc["scatterings"])], dtype=torch.float64, device="cuda")
-            if world > 1:
-                mx = tt.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-                dist.all_reduce(tt)
-                tt[0] = mx[0]
-            if i >= 0:
-                e_secs += float(tt[0]); e_scat += float(tt[1])
-        out["e2e"] = {"value": e_scat / e_secs, "unit": "scatterings/s", "h2d_bytes_per_step": int(h2d),
-                      "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e_secs / e_steps, "steps": e_steps,
-                      "timing": ("host wall clock around " + ("create(host arrays)+" if regrid else "") +
+        e_steps = steps
+        e_scat = [0.0] * e_steps
+
+        def e2e_step(j, i):
+            with torch.cuda.stream(streams[j]):
+                flush[j].zero_()
+                cx = thor.Context.from_workload(g, host=True, pack=pack) if regrid else ctxs[j]
+                cx.sources_set(src["pos"], src["lum"], src["sigma"])
+                cx.run(n, w["seed"] + (max(i, 0) if not id0 else 0), dict(opts, photon_id_offset=id0 + rank * n))
+                cx.spectrum(); cx.nscat_hist()
+                if cube_bytes:
+                    cx.cube()
+                cc = cx.counters()
+                if regrid:
+                    cx.close()
+                return float(cc["scatterings"])
+
+        if regrid:
+            e2e_step(0, -1)                                         # small grids: one untimed pass warms the re-creation path
+        nxt[0] = 0
+        del errors[:]
+
+        def e2e_worker(j):
+            try:
+                torch.cuda.set_device(local)
+                while True:
+                    with lock:
+                        i = nxt[0]
+                        nxt[0] += 1
+                    if i >= e_steps:
+                        return
+                    e_scat[i] = e2e_step(j, i)
+            except Exception as e:
+                errors.append(e)
+
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        if C == 1:
+            e2e_worker(0)
+        else:
+            th = [threading.Thread(target=e2e_worker, args=(j,)) for j in range(C)]
+            [t.start() for t in th]
+            [t.join() for t in th]
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if errors:
+            raise errors[0]
+        tt = torch.tensor([dt, float(sum(e_scat))], dtype=torch.float64, device="cuda")
+        if world > 1:
+            mx = tt.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+            dist.all_reduce(tt)
+            tt[0] = mx[0]
+        e_secs, e_tot = float(tt[0]), float(tt[1])
+        out["e2e"] = {"value": e_tot / e_secs, "unit": "scatterings/s", "h2d_bytes_per_step": int(h2d),
+                      "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e_secs / e_steps, "steps": e_steps, "steps_in_flight": C,
+                      "timing": ("host wall clock around " + str(e_steps) + " steps of " + ("create(host arrays)+" if regrid else "") +
                                  "sources_set(host arrays)+run+tally_get(host: spectrum, histogram, counters" +
                                  (", cube" if cube_bytes else "") + ")" + ("+destroy" if regrid else "") +
-                                 ", device synchronised on both sides, max over ranks" +
-                                 ("" if regrid else "; the grid is the resident dataset (72.5 GB) and is not re-copied"))}
-    ctx.close()
-    del ctx, flush, w, g
+                                 f", {C} in flight, device synchronised on both sides, max over ranks" +
+                                 ("" if regrid else "; the grid is the resident dataset and is not re-copied"))}
+    for cx in ctxs:
+        cx.close()
+    del ctxs, ctx, flush, w, g
+    if not gridless:
+        del gsh
     torch.cuda.empty_cache()
     return out
 
@@ -565,6 +661,7 @@ def main():
     ap.add_argument("--photon-id-offset", type=int, default=0, help="first photon id of rank 0 (with --n-photons 1: one chosen packet alone on the GPU, the lone-lane regime of DESIGN.md 4.6)")
     ap.add_argument("--max-scatter", type=int, default=-1, help="override the workload's scattering cap")
     ap.add_argument("--grid-flags", type=lambda v: int(v, 0), default=0, help="extra thor_grid_create flags (0x400 L2 persistence window, 0x800 32-byte L2 fetch granularity)")
+    ap.add_argument("--in-flight", type=int, default=3, help="independent steps run at once, each in its own context and stream (1 = one after the other)")
     ap.add_argument("--pack", type=int, default=-1, help="THOR_GRID_PACK (1/0); default: on for the gather workload")
     args = ap.parse_args()
     if args.workload in ("project", "render"):
@@ -594,9 +691,9 @@ def main():
                         sample_clocks=True, want_e2e=not args.no_e2e)
     out = {"metric": head["metric"], "value": head["value"], "unit": head["unit"], "packets_per_sec": head["packets_per_sec"],
            "cell_crossings_per_sec": head["cell_crossings_per_sec"], "n_gpus": world, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+           "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "serial_ms_per_step": head["serial_ms_per_step"], "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": head["config"], "clocks": head.get("clocks"),
-           "gpu_launches": args.steps, "phases": head["phases"], "counters": head["counters"],
+           "gpu_launches": 3 * args.steps, "phases": head["phases"], "counters": head["counters"],
            "roofline": head["roofline"]}
     for k in ("roofline_hbm", "roofline_alu", "e2e"):
         if k in head:
@@ -608,9 +705,9 @@ def main():
         for name in SUBS:
             r = measure_walk(args, name, args.sub_steps, 3, rank, local, world)
             out["workloads"][name] = {k: r[k] for k in ("value", "unit", "packets_per_sec", "cell_crossings_per_sec", "steps",
-                                                         "warmup", "ms_per_step", "config", "phases", "roofline")}
+                                                         "warmup", "ms_per_step", "serial_ms_per_step", "config", "phases", "roofline")}
             out["workloads"][name]["roofline_other"] = r.get("roofline_hbm") or r.get("roofline_alu")
-            out["gpu_launches"] += args.sub_steps
+            out["gpu_launches"] += 3 * args.sub_steps
     # ---- cpu_baseline: the oracle on a bounded sample, rank 0 at N = 1 only
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.workload, args.cpu_budget, max(1, args.ref_chunk))

@@ -416,6 +416,7 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     p.spec_lo = (float)o.spec_lo;
     p.spec_inv_width = o.spec_bins > 0 ? (float)(o.spec_bins / (o.spec_hi - o.spec_lo)) : 0.f;
     p.hubble = (float)o.hubble_kms_per_cell; p.hubble_eps = (float)o.hubble_eps; p.v_max = (float)o.v_max_kms;
+    p.v_max_or_inf = p.v_max > 0.f ? p.v_max : INFINITY;
     p.peel_on = o.peel_on ? 1 : 0;
     size_t cube_elems = 0;
     if (p.peel_on) {
@@ -444,7 +445,7 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
         cube_elems = (size_t)o.peel_nx * o.peel_ny * o.peel_nv;
     }
     p.id_offset = o.photon_id_offset; p.n_photons = n_photons; p.seed = seed; p.max_scatter = o.max_scatter;
-    p.max_scatter32 = o.max_scatter > 0xffffffffull ? 0xffffffffu : (unsigned)o.max_scatter;
+    p.max_scatter_or_max = (o.max_scatter == 0 || o.max_scatter > 0xffffffffull) ? 0xffffffffu : (unsigned)o.max_scatter;
     p.walk_variant = o.walk_variant;
     p.dust_albedo = (float)o.dust_albedo; p.dust_g = (float)o.dust_g;
     p.doublet_on = o.doublet_on ? 1 : 0;
@@ -609,9 +610,10 @@ extern "C" thor_status thor_run_noalloc(thor_ctx* ctx, unsigned long long n_phot
     p.spec_lo = (float)o.spec_lo;
     p.spec_inv_width = o.spec_bins > 0 ? (float)(o.spec_bins / (o.spec_hi - o.spec_lo)) : 0.f;
     p.hubble = (float)o.hubble_kms_per_cell; p.hubble_eps = (float)o.hubble_eps; p.v_max = (float)o.v_max_kms;
+    p.v_max_or_inf = p.v_max > 0.f ? p.v_max : INFINITY;
     p.peel_on = 0;
     p.id_offset = o.photon_id_offset; p.n_photons = n_photons; p.seed = seed; p.max_scatter = o.max_scatter;
-    p.max_scatter32 = o.max_scatter > 0xffffffffull ? 0xffffffffu : (unsigned)o.max_scatter;
+    p.max_scatter_or_max = (o.max_scatter == 0 || o.max_scatter > 0xffffffffull) ? 0xffffffffu : (unsigned)o.max_scatter;
     p.walk_variant = o.walk_variant;
     p.dust_albedo = (float)o.dust_albedo; p.dust_g = (float)o.dust_g;
     p.doublet_on = o.doublet_on ? 1 : 0;

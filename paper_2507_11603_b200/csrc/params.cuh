@@ -70,6 +70,7 @@ struct WalkParams {
     float spec_inv_vth_ref;              // 1 / v_th(spec_T_ref)
     float spec_lo, spec_inv_width;       // bin = floor((val - lo) * inv_width), inv_width = bins / (hi - lo)
     float hubble, hubble_eps, v_max;
+    float v_max_or_inf;                  // v_max, or +inf when there is none: one compare on a lone packet's serial chain
     int peel_on;
     float kobs[3], kobs_inv[3], img1[3], img2[3];   // kobs_inv = 1 / kobs (IEEE single-precision quotients; +-inf for 0)
     int peel_nx, peel_ny, peel_nv;
@@ -77,7 +78,7 @@ struct WalkParams {
     float peel_inv_width;                // 1 / peel_width_cells
     float tau_peel_max;
     unsigned long long id_offset, n_photons, seed, max_scatter;
-    unsigned int max_scatter32;          // max_scatter clamped to 32 bits (the per-packet counter's width); 0 = none
+    unsigned int max_scatter_or_max;     // max_scatter clamped to 32 bits (the per-packet counter's width); 2^32 - 1 = none
     unsigned int max_crossings;          // per-packet cap on cell crossings (reading A26); 2^32 - 1 = the built-in limit
     // work distribution + tallies (device)
     unsigned long long* next_photon;     // a14: global atomic photon counter

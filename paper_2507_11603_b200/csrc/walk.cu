@@ -256,7 +256,7 @@ __device__ __noinline__ void peelq_serve(const WalkParams& p, const float2* s_ta
 // The drain kernel: launched behind walk_kernel on the same stream.  Each warp pops one parked packet at a time from the
 // global pool and walks it to its end, all 32 lanes on that one packet (see above).  4 warps per CTA — one per SM
 // sub-partition — and a register budget of its own (the walk kernel is held to 80 registers by its occupancy).
-template <bool HUBBLE, bool PEEL, bool GL>
+template <bool HUBBLE, bool PEEL, bool GL, bool DB>
 __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_constant__ WalkParams p) {
     __shared__ BlockTallies sh;
     __shared__ float4 s_win[DRAIN_WARPS][32 * WIN_STRIDE / 4];
@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
     int peelq_cnt = 0;
     PeelPend pend;
     pend.live = false;
-    const int need0 = p.doublet_on ? 4 : 3;                   // blocks one scattering takes at least: [select,] trial, 2 x finish
+    const int need0 = (DB && p.doublet_on) ? 4 : 3;                   // blocks one scattering takes at least: [select,] trial, 2 x finish
     Packet k;
     for (;;) {
         unsigned long long slot = 0;
@@ -295,10 +295,10 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
         env.mTot = -1.f;
         for (;;) {
             if (st == LS_MARCH) {
-                const int ev = GL ? march_step_gridless(p, sh.voigt, k) : march_step<HUBBLE, false>(p, sh.voigt, k);
+                const int ev = GL ? march_step_gridless(p, sh.voigt, k) : march_step<HUBBLE, false, DB>(p, sh.voigt, k);
                 if (ev == EV_CROSSED) continue;
                 if (ev != EV_HIT) { if (lane == 0) tally_packet(p, sh, ev, k); break; }
-                st = p.doublet_on ? LS_SELECT : LS_TRIAL;
+                st = (DB && p.doublet_on) ? LS_SELECT : LS_TRIAL;
                 env.mTot = -1.f;
             }
             if (c + need0 > 32) {                                 // fewer than a trial + a FINISH left: a new window
@@ -307,7 +307,7 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
                 __syncwarp();
                 c = 0;
             }
-            if (st == LS_SELECT) {                            // doublet: which interaction, from one more block
+            if (DB && st == LS_SELECT) {                      // doublet: which interaction, from one more block
                 const float4 u = win[5 * c];
                 ++c;
                 k.rng.b_lo += 1u; k.rng.b_hi += (k.rng.b_lo == 0u);
@@ -317,9 +317,9 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
             if (st == LS_TRIAL) {
                 // every lane tries its OWN block; the packet takes the first acceptance at or after block c — exactly the
                 // trial the sequential rejection loop would have accepted, found in one step however many it rejects
-                if (env.mTot < 0.f) env = upar_envelope(line_a(p, k), fabsf(k.x_in));
+                if (env.mTot < 0.f) env = upar_envelope(line_a<DB>(p, k), fabsf(k.x_in));
                 float uu;
-                const bool ok = upar_try<true>(env, line_a(p, k), my_u, my_sC, my_cC, uu);
+                const bool ok = upar_try<true>(env, line_a<DB>(p, k), my_u, my_sC, my_cC, uu);
                 const unsigned acc = __ballot_sync(0xffffffffu, ok) & ~((1u << c) - 1u);
                 const uint32_t nrej = (uint32_t)((acc ? __ffs(acc) - 1 : 32) - c);   // rejections before the first acceptance
                 uint32_t ntr;                                 // blocks this step consumes
@@ -354,7 +354,7 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
                 d.sphi = a2.x; d.cphi = a2.y; d.nl_p1 = a2.z;
                 d.spsi = b3.x; d.cpsi = b3.y; d.u_dust = u2.y; d.u_mix = u2.z; d.u_alb = u2.w;
                 uint32_t none = 0;
-                const int ev = finish_scatter<HUBBLE, PEEL, true, PEEL_QUEUED>(p, sh.voigt, k, d, pr, none, lane == 0, &pend);
+                const int ev = finish_scatter<HUBBLE, PEEL, true, PEEL_QUEUED, DB>(p, sh.voigt, k, d, pr, none, lane == 0, &pend);
                 if (PEEL && pend.live) {                      // warp-uniform: every lane holds the same ray
                     if (lane == 0) peelq_put(peelq, peelq_cnt, pend);
                     pend.live = false;
@@ -550,7 +550,9 @@ static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t st
     walk_kernel<HUBBLE, PEEL, MIN_CTAS, GL><<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess || !p.pool) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, drain_kernel<HUBBLE, PEEL, GL>, DRAIN_THREADS, 0);
+    // the drain kernel is specialised on the doublet as well: its tests sit on the serial chain of a lone packet
+    const auto drain = p.doublet_on ? drain_kernel<HUBBLE, PEEL, GL, true> : drain_kernel<HUBBLE, PEEL, GL, false>;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, drain, DRAIN_THREADS, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     const long long slots = blocks * (WALK_THREADS / 32) * COOP_MAX_LANES;      // most the walk kernel can have parked
@@ -560,7 +562,7 @@ static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t st
     long long dblocks = (long long)n_sm * per_sm;
     const long long cap = (slots + DRAIN_WARPS - 1) / DRAIN_WARPS;               // one warp per slot at most
     if (cap < dblocks) dblocks = cap;
-    drain_kernel<HUBBLE, PEEL, GL><<<(unsigned)dblocks, DRAIN_THREADS, 0, stream>>>(p);
+    drain<<<(unsigned)dblocks, DRAIN_THREADS, 0, stream>>>(p);
     return cudaGetLastError();
 }
 

@@ -62,11 +62,14 @@ __device__ __forceinline__ Cell load_cell(const WalkParams& p, int64_t i) {
 
 // Line opacity per cell length at gas-frame frequency x of line 1: n sigma_0 [H(a, x) + rs H(a ra, x - dv / v_th)]
 // (the cross-sections of a doublet's transitions add); k2 = the second line's share.
+// DB = false: instantiated for runs without a doublet (drain kernel): the tests of that run constant — a uniform-register
+// load, compare and branch of ~45 cycles each on the serial chain of a lone packet — are compiled out.
+template <bool DB = true>
 __device__ __forceinline__ float line_opacity(const WalkParams& p, const float2* s_tab, const Cell& c, float x, float& k2) {
     k2 = 0.f;
     if (!(c.nsig > 0.f)) return 0.f;
     const float k1 = c.nsig * voigt_H(s_tab, c.a, x);
-    if (p.doublet_on) k2 = c.nsig * p.db_rs * voigt_H(s_tab, c.a * p.db_ra, fmaf(-p.db_dv, c.inv_vth, x));
+    if (DB && p.doublet_on) k2 = c.nsig * p.db_rs * voigt_H(s_tab, c.a * p.db_ra, fmaf(-p.db_dv, c.inv_vth, x));
     return k1 + k2;
 }
 
@@ -74,14 +77,14 @@ __device__ __forceinline__ float line_opacity(const WalkParams& p, const float2*
 // s_hit at which tau_need is reached (linear within the step).  Without Hubble drift: kappa len.
 // With drift Hc (km/s per cell length): sub-steps per reading A12 — n_sub = 1 if min|x| over the segment > 6 else
 // ceil(|dV| / (eps v_th)), midpoint rule.  Returns true on interaction; k_tot is the opacity there.
-template <bool HUBBLE>
+template <bool HUBBLE, bool DB = true>
 __device__ __forceinline__ bool integrate_segment(const WalkParams& p, const float2* s_tab, const Cell& c, float V0,
                                                   float vk, float len, float tau_need, float& tau_out, float& s_hit,
                                                   float& k_tot, float& k2) {
     tau_out = 0.f; s_hit = 0.f; k_tot = 0.f; k2 = 0.f;
     if (c.nsig <= 0.f && c.kd <= 0.f) return false;
     if (!HUBBLE) {
-        const float kl = line_opacity(p, s_tab, c, (V0 - vk) * c.inv_vth, k2);
+        const float kl = line_opacity<DB>(p, s_tab, c, (V0 - vk) * c.inv_vth, k2);
         const float kt = kl + c.kd;
         const float dtau = kt * len;
         if (dtau >= tau_need && kt > 0.f) {
@@ -107,7 +110,7 @@ __device__ __forceinline__ bool integrate_segment(const WalkParams& p, const flo
     float tau = 0.f;
     for (int j = 0; j < nsub; ++j) {
         const float Vmid = Hc != 0.f ? fmaf(-Hc, ((float)j + 0.5f) * ds, V0) : V0;   // no 0 * inf when ds = +inf (A24)
-        const float kl = line_opacity(p, s_tab, c, (Vmid - vk) * c.inv_vth, k2);
+        const float kl = line_opacity<DB>(p, s_tab, c, (Vmid - vk) * c.inv_vth, k2);
         const float kt = kl + c.kd;
         const float dtau = kt * ds;
         if (tau + dtau >= tau_need && kt > 0.f) {
@@ -123,8 +126,9 @@ __device__ __forceinline__ bool integrate_segment(const WalkParams& p, const flo
 }
 
 // Total opacity per cell length at velocity offset V for direction cosine-weighted bulk velocity vk (no drift).
+template <bool DB = true>
 __device__ __forceinline__ float cell_opacity(const WalkParams& p, const float2* s_tab, const Cell& c, float V, float vk, float& k2) {
-    return line_opacity(p, s_tab, c, (V - vk) * c.inv_vth, k2) + c.kd;
+    return line_opacity<DB>(p, s_tab, c, (V - vk) * c.inv_vth, k2) + c.kd;
 }
 
 // a12 peel-off: w = P^ exp(-tau_obs), tau_obs integrated from `at` along k_obs to the box face at
@@ -303,7 +307,7 @@ __device__ __forceinline__ void emit_packet(const WalkParams& p, Packet& k, unsi
 // a4-a7: one cell step.  EV_HIT: the packet sits at its interaction site (hit_kt, x_in set); EV_CROSSED: it entered the
 // next cell; else it ended (escaped / terminated / capped).  EARLY: the variant for grids beyond L2 issues the gather
 // of the next cell at the face crossing and derives it at first use.
-template <bool HUBBLE, bool EARLY>
+template <bool HUBBLE, bool EARLY, bool DB = true>
 __device__ __forceinline__ int march_step(const WalkParams& p, const float2* s_tab, Packet& k) {
     if (k.stale) {
         if (EARLY) derive_cell(p, k.cell);
@@ -318,7 +322,7 @@ __device__ __forceinline__ int march_step(const WalkParams& p, const float2* s_t
         // Piecewise-constant cell: the interaction lies at s = tau / kappa if that is inside the cell.
         // Deep in an optically thick cell s is far smaller than the distance to the nearest face, which bounds the
         // segment length from below: no DDA step and no reciprocals of k are needed at all.
-        kt = cell_opacity(p, s_tab, k.cell, k.V, vk, k.hit_k2);
+        kt = cell_opacity<DB>(p, s_tab, k.cell, k.V, vk, k.hit_k2);
         const float s = kt > 0.f ? k.tau_rem / kt : CUDART_INF_F;
         if (kt > 0.f && s <= dda_min_face_distance(k.ray, p.g)) {
             hit = true; s_hit = s;
@@ -332,7 +336,7 @@ __device__ __forceinline__ int march_step(const WalkParams& p, const float2* s_t
     } else {
         if (!k.inv_ok) { ray_set_inv(k.ray); k.inv_ok = true; }
         ex = dda_next_face(k.ray, p.g, len);
-        hit = integrate_segment<true>(p, s_tab, k.cell, k.V, vk, len, k.tau_rem, dtau, s_hit, kt, k.hit_k2);
+        hit = integrate_segment<true, DB>(p, s_tab, k.cell, k.V, vk, len, k.tau_rem, dtau, s_hit, kt, k.hit_k2);
     }
     if (hit) {
         dda_advance_within(k.ray, p.g, s_hit);
@@ -505,17 +509,19 @@ __device__ __forceinline__ void select_line(const WalkParams& p, Packet& k, floa
     if (t >= k.hit_kt - k.hit_k2) { k.line = 1; k.x_in = fmaf(-p.db_dv, k.cell.inv_vth, k.x_in); }
     else k.line = 0;
 }
-__device__ __forceinline__ float line_a(const WalkParams& p, const Packet& k) { return k.line > 0 ? k.cell.a * p.db_ra : k.cell.a; }
+template <bool DB = true>
+__device__ __forceinline__ float line_a(const WalkParams& p, const Packet& k) { return (DB && k.line > 0) ? k.cell.a * p.db_ra : k.cell.a; }
 
 // a7, a9-a12: the interaction itself (PAPER.md 2.3.1): dust or line, u_perp (Eq. 5, core-skipping
 // PAPER.md:244), phase function, rotation, Eq. 7 with the recoil dropped, peel-off
 // before k' is adopted, new tau_target.  Returns EV_ABSORBED / EV_TERMINATED / EV_CAPPED / EV_SCATTERED.
-template <bool HUBBLE, bool PEEL, bool PRE, int PMODE = PEEL_INLINE>
+template <bool HUBBLE, bool PEEL, bool PRE, int PMODE = PEEL_INLINE, bool DB = true>
 __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2* s_tab, Packet& k, const FinDraws& d,
                                               uint32_t& peel_rays, uint32_t& peel_cells, bool add, PeelPend* pend = nullptr) {
     const float kx = k.ray.kx, ky = k.ray.ky, kz = k.ray.kz;
     const Cell& c = k.cell;
-    if (p.has_dust && (p.doublet_on ? k.line < 0 : d.u_dust * k.hit_kt < c.kd)) {
+    // (a run without dust has kd = 0 in every cell, and u kappa < 0 is never true: the has_dust flag need not be read)
+    if ((DB && p.doublet_on) ? (p.has_dust && k.line < 0) : (d.u_dust * k.hit_kt < c.kd)) {
         // dust (PAPER.md 2.3.2): scattered with probability albedo (Eq. 8) into the Henyey-Greenstein phase function (Eq. 9),
         // coherently in the bulk frame of the cell (grains are heavy and move with the gas, reading A33); else destroyed
         if (!(p.dust_albedo > 0.f) || !(d.u_alb < p.dust_albedo)) return EV_ABSORBED;
@@ -541,12 +547,12 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
         k.tau_rem = d.tau_next;
         return EV_DUST_SCATTERED;
     }
-    const float dv_line = k.line > 0 ? p.db_dv : 0.f;             // frequencies of this event are relative to its line
-    const float a_l = line_a(p, k);
+    const float dv_line = (DB && k.line > 0) ? p.db_dv : 0.f;             // frequencies of this event are relative to its line
+    const float a_l = line_a<DB>(p, k);
     float x_crit = 0.f;
     if (p.core_skip_mode == 1) x_crit = p.x_crit;
     else if (p.core_skip_mode == 2) {              // local: a tau_0 over half a cell (reading A7)
-        const float atau = a_l * c.nsig * (k.line > 0 ? p.db_rs : 1.f) * 0.5f;
+        const float atau = a_l * c.nsig * ((DB && k.line > 0) ? p.db_rs : 1.f) * 0.5f;
         x_crit = atau >= 1.f ? 0.2f * cbrtf(atau) : 0.f;
     }
     float up1, up2;
@@ -580,8 +586,8 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
     k.inv_ok = false;
     k.V = fmaf(x_out, c.vth, dot3(c.vx, c.vy, c.vz, nx, ny, nz)) + dv_line;
     ++k.nscat;
-    if (p.v_max > 0.f && fabsf(k.V) > p.v_max) return EV_TERMINATED;
-    if ((p.max_scatter32 && k.nscat >= p.max_scatter32) || !(fabsf(k.V) <= 3.0e38f)) return EV_CAPPED;   // cap, or fail-safe: non-finite V
+    if (fabsf(k.V) > p.v_max_or_inf) return EV_TERMINATED;     // +inf when there is no v_max
+    if (k.nscat >= p.max_scatter_or_max || !(fabsf(k.V) <= 3.0e38f)) return EV_CAPPED;   // cap (2^32 - 1 when there is none), or fail-safe: non-finite V
     k.tau_rem = d.tau_next;
     return EV_SCATTERED;
 }

@@ -633,6 +633,54 @@ def test_deferred_peel_rays_are_bit_identical(thor):
         assert c["scatterings"] == whole["counters"]["scatterings"]
 
 
+def test_concurrent_contexts_on_a_shared_grid(thor):
+    """Contexts are independent: several of them, each on a stream of its own and driven from a host thread of its own, may
+    borrow the same device fields and run at once (bench.py overlaps consecutive steps this way).  Every run must give,
+    bit for bit, what the same run gives alone."""
+    import threading
+    import torch
+    w = W.expanding_shell(n=32, n_photons=20_000)
+    opts = dict(w["opts"], max_scatter=20_000, raw_output=1)
+    g = dict(w["grid"])
+    for key in ("nHI", "T", "vx", "vy", "vz", "kdust"):
+        if g.get(key) is not None:
+            g[key] = torch.from_numpy(np.ascontiguousarray(g[key], np.float32)).cuda()
+
+    def make(stream):
+        with torch.cuda.stream(stream):
+            ctx = thor.Context.from_workload(g)
+            ctx.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
+        return ctx
+
+    seeds = [3, 4, 5, 6]
+    alone = []
+    ctx = make(torch.cuda.current_stream())
+    for s in seeds:
+        ctx.run(w["n_photons"], s, opts)
+        alone.append((ctx.raw().tobytes(), ctx.spectrum().copy(), ctx.counters()))
+    ctx.close()
+    streams = [torch.cuda.Stream() for _ in seeds]
+    ctxs = [make(st) for st in streams]
+    got, errs = [None] * len(seeds), []
+
+    def worker(j):
+        try:
+            with torch.cuda.stream(streams[j]):
+                for rep in range(2):                                  # twice: the launches of different contexts interleave
+                    ctxs[j].run(w["n_photons"], seeds[j], opts)
+                got[j] = (ctxs[j].raw().tobytes(), ctxs[j].spectrum().copy(), ctxs[j].counters())
+        except Exception as e:
+            errs.append(e)
+
+    th = [threading.Thread(target=worker, args=(j,)) for j in range(len(seeds))]
+    [t.start() for t in th]
+    [t.join() for t in th]
+    assert not errs, errs
+    for a, b in zip(alone, got):
+        assert a[0] == b[0] and np.array_equal(a[1], b[1]) and a[2] == b[2]
+    [c.close() for c in ctxs]
+
+
 def test_mean_scattering_count_within_one_percent(thor, oracle):
     """BASELINE.json's bar as stated: mean scattering count within 1 % — on a rung where the standard error lets it bind
     (reading A23): tau0 = 1e2, 4e5 packets per side, 3 SE = 0.6 %.  Plain |dmean| <= 1 %, no SE allowance."""
