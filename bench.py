@@ -657,7 +657,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-subs", action="store_true", help="skip the `workloads` sub-dict")
-    ap.add_argument("--sub-steps", type=int, default=2)
+    ap.add_argument("--sub-steps", type=int, default=3)
     ap.add_argument("--photon-id-offset", type=int, default=0, help="first photon id of rank 0 (with --n-photons 1: one chosen packet alone on the GPU, the lone-lane regime of DESIGN.md 4.6)")
     ap.add_argument("--max-scatter", type=int, default=-1, help="override the workload's scattering cap")
     ap.add_argument("--grid-flags", type=lambda v: int(v, 0), default=0, help="extra thor_grid_create flags (0x400 L2 persistence window, 0x800 32-byte L2 fetch granularity)")
