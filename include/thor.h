@@ -18,7 +18,9 @@
 extern "C" {
 #endif
 
-typedef struct thor_ctx thor_ctx; /* opaque; one per grid; not thread-safe */
+typedef struct thor_ctx thor_ctx; /* opaque; one per grid.  One context must not be used from two host threads at once;
+                                     different contexts are independent — they may run at once, from different threads or
+                                     through thor_run_async, and may borrow the same device fields */
 
 typedef enum {
     THOR_OK = 0,
@@ -160,6 +162,16 @@ void thor_opts_default(thor_opts *o);
  * is 0 — nothing could end a packet in empty gas there, and thor_run never hangs; THOR_ERR_OOM if tallies cannot be
  * allocated; THOR_ERR_CUDA. */
 thor_status thor_run(thor_ctx *ctx, unsigned long long n_photons, unsigned long long seed, const thor_opts *opts);
+
+/* thor_run in two halves, so that ONE host thread can keep several contexts busy (consecutive batches overlap: the tail of
+ * one run — a few long packets, DESIGN.md 5 — with the feed phase of the next; contexts may borrow the same device fields).
+ * thor_run_async validates, allocates what the run needs and enqueues the kernels on the context's stream, then returns;
+ * thor_wait blocks until that run has finished and publishes its tallies and timings (no-op if nothing is pending).
+ * thor_run == thor_run_async + thor_wait.  While a run is pending, every other call on the SAME context that uses the
+ * run's state (thor_run*, thor_sources_set, thor_tally_get, thor_grid_destroy) completes it first; thor_last_run_* return
+ * THOR_ERR_STATE.  Arguments, results and errors as thor_run; a kernel fault surfaces in thor_wait. */
+thor_status thor_run_async(thor_ctx *ctx, unsigned long long n_photons, unsigned long long seed, const thor_opts *opts);
+thor_status thor_wait(thor_ctx *ctx);
 
 /* thor_run for callers that cannot allocate device memory at run time (code under CUDA graph capture, serving loops,
  * harnesses that forbid cudaMalloc): the same walk (same kernels, same packets: tallies equal thor_run's bit for bit),

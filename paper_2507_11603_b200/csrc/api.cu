@@ -57,6 +57,8 @@ struct thor_ctx {
     unsigned int* d_pool_order = nullptr;
     // last run
     bool have_run = false;
+    bool pending = false;                       // thor_run_async launched, thor_wait not yet called
+    unsigned long long pending_n = 0;
     thor_opts last{};
     unsigned long long last_n = 0;
     float last_ms = 0.f, last_feed_ms = 0.f;
@@ -98,6 +100,8 @@ static thor_status cuda_fail(thor_ctx* c, cudaError_t e, const char* what) {
         if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);   \
     } while (0)
 
+static thor_status run_finish(thor_ctx* ctx);          // completes a pending thor_run_async (defined beside it)
+
 extern "C" const char* thor_last_error(const thor_ctx* ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }
 
 extern "C" void thor_opts_default(thor_opts* o) {
@@ -116,6 +120,7 @@ extern "C" void thor_opts_default(thor_opts* o) {
 
 extern "C" void thor_grid_destroy(thor_ctx* ctx) {
     if (!ctx) return;
+    run_finish(ctx);                                       // a pending run still reads what is freed below
     DevGuard dev_guard(ctx->device);
     for (float* p : ctx->owned) if (p) cudaFree(p);
     if (ctx->d_packed) cudaFree(ctx->d_packed);
@@ -276,6 +281,7 @@ extern "C" thor_status thor_dataset_create_gridless(thor_ctx** out, const thor_g
 extern "C" thor_status thor_sources_set(thor_ctx* ctx, long long n_src, const float* pos_xyz, const float* lum,
                                         const float* sigma_kms) {
     if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_sources_set: ctx is NULL");
+    { const thor_status st = run_finish(ctx); if (st != THOR_OK) return st; }   // a pending run still reads the old list
     if (n_src <= 0 || !pos_xyz || !lum || !sigma_kms) return fail(ctx, THOR_ERR_ARG, "thor_sources_set: empty or NULL source list");
     const int n[3] = {ctx->g.nx, ctx->g.ny, ctx->g.nz};
     std::vector<double> cdf((size_t)n_src);
@@ -346,9 +352,37 @@ extern "C" thor_status thor_sources_set(thor_ctx* ctx, long long n_src, const fl
 
 static bool phase_ok(int p) { return p == THOR_PHASE_ISOTROPIC || p == THOR_PHASE_DIPOLE || p == THOR_PHASE_MIX; }
 
-extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, unsigned long long seed,
-                                const thor_opts* opts) {
+// Second half of a run: waits for the launch, reads its timers, publishes the tallies.  No-op when nothing is pending.
+static thor_status run_finish(thor_ctx* ctx) {
+    if (!ctx->pending) return THOR_OK;
+    DevGuard dev_guard(ctx->device);
+    ctx->pending = false;
+    CU(cudaStreamSynchronize(ctx->stream));
+    CU(cudaEventElapsedTime(&ctx->last_ms, ctx->ev0, ctx->ev1));
+    ctx->last_feed_ms = 0.f;
+    if (ctx->pending_n > 0) {
+        unsigned long long t[3] = {0, 0, 0};                    // t_start, t_dry, max_nscat are adjacent
+        CU(cudaMemcpyAsync(t, ctx->d_small + SMALL_TIMES, sizeof t, cudaMemcpyDeviceToHost, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+        if (t[1] != ~0ull && t[1] >= t[0]) ctx->last_feed_ms = (float)((double)(t[1] - t[0]) * 1e-6);
+        ctx->last_max_nscat = t[2];
+    }
+    ctx->last_n = ctx->pending_n; ctx->have_run = true;
+    return THOR_OK;
+}
+
+extern "C" thor_status thor_wait(thor_ctx* ctx) {
+    if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_wait: ctx is NULL");
+    return run_finish(ctx);
+}
+
+extern "C" thor_status thor_run_async(thor_ctx* ctx, unsigned long long n_photons, unsigned long long seed,
+                                      const thor_opts* opts) {
     if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_run: ctx is NULL");
+    {
+        const thor_status st = run_finish(ctx);                // a run still pending on this context is completed first
+        if (st != THOR_OK) return st;
+    }
     if (ctx->n_src <= 0) return fail(ctx, THOR_ERR_STATE, "thor_run: call thor_sources_set first");
     thor_opts o;
     thor_opts_default(&o);
@@ -506,18 +540,14 @@ extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, uns
     CU(cudaEventRecord(ctx->ev0, ctx->stream));
     if (n_photons > 0) CU(thor::launch_walk(p, ctx->n_sm, ctx->stream, &ctx->last_blocks));
     CU(cudaEventRecord(ctx->ev1, ctx->stream));
-    CU(cudaStreamSynchronize(ctx->stream));
-    CU(cudaEventElapsedTime(&ctx->last_ms, ctx->ev0, ctx->ev1));
-    ctx->last_feed_ms = 0.f;
-    if (n_photons > 0) {
-        unsigned long long t[3] = {0, 0, 0};                    // t_start, t_dry, max_nscat are adjacent
-        CU(cudaMemcpyAsync(t, ctx->d_small + SMALL_TIMES, sizeof t, cudaMemcpyDeviceToHost, ctx->stream));
-        CU(cudaStreamSynchronize(ctx->stream));
-        if (t[1] != ~0ull && t[1] >= t[0]) ctx->last_feed_ms = (float)((double)(t[1] - t[0]) * 1e-6);
-        ctx->last_max_nscat = t[2];
-    }
-    ctx->last = o; ctx->last_n = n_photons; ctx->have_run = true;
+    ctx->last = o; ctx->pending_n = n_photons; ctx->pending = true;   // have_run stays false until thor_wait
     return THOR_OK;
+}
+
+extern "C" thor_status thor_run(thor_ctx* ctx, unsigned long long n_photons, unsigned long long seed,
+                                const thor_opts* opts) {
+    const thor_status st = thor_run_async(ctx, n_photons, seed, opts);
+    return st != THOR_OK ? st : run_finish(ctx);
 }
 
 // grid part of the kernel parameter block, shared by the ray operators
@@ -567,6 +597,7 @@ extern "C" thor_status thor_run_noalloc(thor_ctx* ctx, unsigned long long n_phot
                                         unsigned long long* spectrum_out, unsigned long long* counters_out,
                                         unsigned long long* nscat_hist_out) {
     if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_run_noalloc: ctx is NULL");
+    { const thor_status st = run_finish(ctx); if (st != THOR_OK) return st; }
     if (ctx->gridless) return fail(ctx, THOR_ERR_UNSUPPORTED, "thor_run_noalloc: gridless datasets are not supported (use thor_run)");
     if (ctx->n_src <= 0) return fail(ctx, THOR_ERR_STATE, "thor_run_noalloc: call thor_sources_set first");
     thor_opts o;
@@ -777,6 +808,7 @@ extern "C" thor_status thor_slice(thor_ctx* ctx, long long n_points, const float
 
 extern "C" thor_status thor_last_run_ms(const thor_ctx* ctx, float* ms) {
     if (!ctx || !ms) return fail(nullptr, THOR_ERR_ARG, "thor_last_run_ms: NULL argument");
+    if (ctx->pending) return fail(const_cast<thor_ctx*>(ctx), THOR_ERR_STATE, "thor_last_run_ms: a run is pending (thor_wait first)");
     if (!ctx->have_run) return fail(const_cast<thor_ctx*>(ctx), THOR_ERR_STATE, "thor_last_run_ms: no run yet");
     *ms = ctx->last_ms;
     return THOR_OK;
@@ -784,6 +816,7 @@ extern "C" thor_status thor_last_run_ms(const thor_ctx* ctx, float* ms) {
 
 extern "C" thor_status thor_last_run_max_nscat(const thor_ctx* ctx, unsigned long long* n) {
     if (!ctx || !n) return fail(nullptr, THOR_ERR_ARG, "thor_last_run_max_nscat: NULL argument");
+    if (ctx->pending) return fail(const_cast<thor_ctx*>(ctx), THOR_ERR_STATE, "thor_last_run_max_nscat: a run is pending (thor_wait first)");
     if (!ctx->have_run) return fail(const_cast<thor_ctx*>(ctx), THOR_ERR_STATE, "thor_last_run_max_nscat: no run yet");
     *n = ctx->last_max_nscat;
     return THOR_OK;
@@ -791,6 +824,7 @@ extern "C" thor_status thor_last_run_max_nscat(const thor_ctx* ctx, unsigned lon
 
 extern "C" thor_status thor_last_run_feed_ms(const thor_ctx* ctx, float* ms) {
     if (!ctx || !ms) return fail(nullptr, THOR_ERR_ARG, "thor_last_run_feed_ms: NULL argument");
+    if (ctx->pending) return fail(const_cast<thor_ctx*>(ctx), THOR_ERR_STATE, "thor_last_run_feed_ms: a run is pending (thor_wait first)");
     if (!ctx->have_run) return fail(const_cast<thor_ctx*>(ctx), THOR_ERR_STATE, "thor_last_run_feed_ms: no run yet");
     *ms = ctx->last_feed_ms;
     return THOR_OK;
@@ -798,6 +832,7 @@ extern "C" thor_status thor_last_run_feed_ms(const thor_ctx* ctx, float* ms) {
 
 extern "C" thor_status thor_tally_get(thor_ctx* ctx, int kind, void* dst, size_t dst_bytes, size_t* needed) {
     if (!ctx) return fail(nullptr, THOR_ERR_ARG, "thor_tally_get: ctx is NULL");
+    { const thor_status st = run_finish(ctx); if (st != THOR_OK) return st; }
     if (!ctx->have_run) return fail(ctx, THOR_ERR_STATE, "thor_tally_get: no completed run");
     const bool dev_dst = (kind & THOR_TALLY_DEVICE_DST) != 0;
     const int k = kind & ~THOR_TALLY_DEVICE_DST;

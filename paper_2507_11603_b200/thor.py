@@ -19,7 +19,7 @@ COUNTER_NAMES = ["escaped", "absorbed", "terminated", "capped", "scatterings", "
                  "peel_rays", "peel_cells", "dust_scatterings"]
 RAW_DTYPE = np.dtype([("V", "<f4"), ("nscat", "<u4"), ("status", "<i4"), ("kx", "<f4"), ("ky", "<f4"), ("kz", "<f4")])
 
-EXPORTS = ["thor_grid_create", "thor_dataset_create_gridless", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run", "thor_run_noalloc",
+EXPORTS = ["thor_grid_create", "thor_dataset_create_gridless", "thor_grid_destroy", "thor_sources_set", "thor_opts_default", "thor_run", "thor_run_async", "thor_wait", "thor_run_noalloc",
            "thor_last_run_ms", "thor_last_run_feed_ms", "thor_last_run_max_nscat", "thor_raytrace", "thor_raytrace_ex", "thor_volume_render", "thor_volume_render_ex", "thor_slice", "thor_tally_get", "thor_last_error", "thor_unit_philox", "thor_unit_curand_philox", "thor_unit_dda_trace",
            "thor_unit_voigt", "thor_unit_scatter"]
 
@@ -89,6 +89,8 @@ def lib():
         L.thor_opts_default.argtypes = [C.POINTER(Opts)]
         L.thor_opts_default.restype = None
         L.thor_run.argtypes = [P, C.c_ulonglong, C.c_ulonglong, C.POINTER(Opts)]
+        L.thor_run_async.argtypes = [P, C.c_ulonglong, C.c_ulonglong, C.POINTER(Opts)]
+        L.thor_wait.argtypes = [P]
         L.thor_run_noalloc.argtypes = [P, C.c_ulonglong, C.c_ulonglong, C.POINTER(Opts), P, P, P]
         L.thor_last_run_ms.argtypes = [P, C.POINTER(f)]
         L.thor_last_run_feed_ms.argtypes = [P, C.POINTER(f)]
@@ -226,6 +228,19 @@ class Context:
         self._opts = opts
         self._n = int(n_photons)
         _check(lib().thor_run(self._ctx, int(n_photons), int(seed), C.byref(opts)), self._ctx)
+
+    def run_async(self, n_photons, seed, opts=None, **kw):
+        """thor_run_async: enqueue the run and return; wait() (or any tally getter) completes it."""
+        if opts is None:
+            opts = make_opts(**kw)
+        elif isinstance(opts, dict):
+            opts = make_opts(**{**opts, **kw})
+        self._opts = opts
+        self._n = int(n_photons)
+        _check(lib().thor_run_async(self._ctx, int(n_photons), int(seed), C.byref(opts)), self._ctx)
+
+    def wait(self):
+        _check(lib().thor_wait(self._ctx), self._ctx)
 
     def run_noalloc(self, n_photons, seed, opts, spectrum_out, counters_out, nscat_hist_out):
         """thor_run_noalloc: the same walk without any device allocation; the tallies go into the caller's torch CUDA int64

@@ -681,6 +681,39 @@ def test_concurrent_contexts_on_a_shared_grid(thor):
     [c.close() for c in ctxs]
 
 
+def test_run_async_overlaps_contexts_from_one_thread(thor):
+    """thor_run_async + thor_wait: one host thread keeps three contexts (three streams, one shared grid) busy; every run gives
+    the bits of a synchronous thor_run, thor_last_run_* refuse to answer while the run is pending, a tally getter completes it."""
+    import torch
+    w = W.expanding_shell(n=32, n_photons=20_000)
+    opts = dict(w["opts"], max_scatter=20_000, raw_output=1)
+    g = dict(w["grid"])
+    for key in ("nHI", "T", "vx", "vy", "vz", "kdust"):
+        if g.get(key) is not None:
+            g[key] = torch.from_numpy(np.ascontiguousarray(g[key], np.float32)).cuda()
+    seeds = [11, 12, 13]
+    ctxs = []
+    for _ in seeds:
+        with torch.cuda.stream(torch.cuda.Stream()):
+            c = thor.Context.from_workload(g)
+            c.sources_set(w["sources"]["pos"], w["sources"]["lum"], w["sources"]["sigma"])
+        ctxs.append(c)
+    for c, s in zip(ctxs, seeds):
+        c.run_async(w["n_photons"], s, opts)
+    with pytest.raises(thor.ThorError) as e:
+        ctxs[-1].last_run_ms()
+    assert e.value.status == 2                                         # THOR_ERR_STATE: pending
+    ctxs[0].wait()
+    ctxs[0].wait()                                                     # nothing pending: no-op
+    got = [(c.raw().tobytes(), c.spectrum().copy(), c.counters()) for c in ctxs]   # getters complete the pending runs
+    assert ctxs[-1].last_run_ms() > 0.0
+    for c, s, gt in zip(ctxs, seeds, got):
+        c.run(w["n_photons"], s, opts)
+        assert gt[0] == c.raw().tobytes() and np.array_equal(gt[1], c.spectrum()) and gt[2] == c.counters()
+    ctxs[1].run_async(w["n_photons"], 14, opts)
+    [c.close() for c in ctxs]                                          # destroying a context with a pending run waits for it
+
+
 def test_mean_scattering_count_within_one_percent(thor, oracle):
     """BASELINE.json's bar as stated: mean scattering count within 1 % — on a rung where the standard error lets it bind
     (reading A23): tau0 = 1e2, 4e5 packets per side, 3 SE = 0.6 %.  Plain |dmean| <= 1 %, no SE allowance."""
