@@ -293,10 +293,11 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
         float my_sC = 0.f, my_cC = 0.f;
         UparEnvelope env;
         env.mTot = -1.f;
+        float xc = -1.f;                                      // x_crit of the packet's present cell, once known (finish_scatter)
         for (;;) {
             if (st == LS_MARCH) {
                 const int ev = GL ? march_step_gridless(p, sh.voigt, k) : march_step<HUBBLE, false, DB>(p, sh.voigt, k);
-                if (ev == EV_CROSSED) continue;
+                if (ev == EV_CROSSED) { xc = -1.f; continue; }
                 if (ev != EV_HIT) { if (lane == 0) tally_packet(p, sh, ev, k); break; }
                 st = (DB && p.doublet_on) ? LS_SELECT : LS_TRIAL;
                 env.mTot = -1.f;
@@ -354,7 +355,7 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
                 d.sphi = a2.x; d.cphi = a2.y; d.nl_p1 = a2.z;
                 d.spsi = b3.x; d.cpsi = b3.y; d.u_dust = u2.y; d.u_mix = u2.z; d.u_alb = u2.w;
                 uint32_t none = 0;
-                const int ev = finish_scatter<HUBBLE, PEEL, true, PEEL_QUEUED, DB>(p, sh.voigt, k, d, pr, none, lane == 0, &pend);
+                const int ev = finish_scatter<HUBBLE, PEEL, true, PEEL_QUEUED, DB>(p, sh.voigt, k, d, pr, none, lane == 0, &pend, &xc);
                 if (PEEL && pend.live) {                      // warp-uniform: every lane holds the same ray
                     if (lane == 0) peelq_put(peelq, peelq_cnt, pend);
                     pend.live = false;

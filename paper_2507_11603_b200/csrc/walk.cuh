@@ -517,7 +517,8 @@ __device__ __forceinline__ float line_a(const WalkParams& p, const Packet& k) { 
 // before k' is adopted, new tau_target.  Returns EV_ABSORBED / EV_TERMINATED / EV_CAPPED / EV_SCATTERED.
 template <bool HUBBLE, bool PEEL, bool PRE, int PMODE = PEEL_INLINE, bool DB = true>
 __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2* s_tab, Packet& k, const FinDraws& d,
-                                              uint32_t& peel_rays, uint32_t& peel_cells, bool add, PeelPend* pend = nullptr) {
+                                              uint32_t& peel_rays, uint32_t& peel_cells, bool add, PeelPend* pend = nullptr,
+                                              float* xc_cache = nullptr) {
     const float kx = k.ray.kx, ky = k.ray.ky, kz = k.ray.kz;
     const Cell& c = k.cell;
     // (a run without dust has kd = 0 in every cell, and u kappa < 0 is never true: the has_dust flag need not be read)
@@ -542,18 +543,25 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
         const float inv = rsqrtf(dot3(nx, ny, nz, nx, ny, nz));
         nx *= inv; ny *= inv; nz *= inv;
         ray_set_k(k.ray, nx, ny, nz);
-        k.inv_ok = false;
+        if (HUBBLE) { ray_set_inv(k.ray); k.inv_ok = true; } else k.inv_ok = false;
         k.V = k.V - vk + dot3(c.vx, c.vy, c.vz, nx, ny, nz);
         k.tau_rem = d.tau_next;
         return EV_DUST_SCATTERED;
     }
     const float dv_line = (DB && k.line > 0) ? p.db_dv : 0.f;             // frequencies of this event are relative to its line
     const float a_l = line_a<DB>(p, k);
+    // x_crit depends on the run and, in local mode, on the cell (and the line of a doublet): the cooperative drain, whose
+    // packet scatters ~1e5 times per cell, keeps it between scatterings (xc_cache < 0 = not yet known for this cell; the mode
+    // tests and the cube root are ~200 cycles of a lone packet's serial chain)
     float x_crit = 0.f;
-    if (p.core_skip_mode == 1) x_crit = p.x_crit;
-    else if (p.core_skip_mode == 2) {              // local: a tau_0 over half a cell (reading A7)
-        const float atau = a_l * c.nsig * ((DB && k.line > 0) ? p.db_rs : 1.f) * 0.5f;
-        x_crit = atau >= 1.f ? 0.2f * cbrtf(atau) : 0.f;
+    if (!DB && xc_cache && *xc_cache >= 0.f) x_crit = *xc_cache;
+    else {
+        if (p.core_skip_mode == 1) x_crit = p.x_crit;
+        else if (p.core_skip_mode == 2) {              // local: a tau_0 over half a cell (reading A7)
+            const float atau = a_l * c.nsig * ((DB && k.line > 0) ? p.db_rs : 1.f) * 0.5f;
+            x_crit = atau >= 1.f ? 0.2f * cbrtf(atau) : 0.f;
+        }
+        if (!DB && xc_cache) *xc_cache = x_crit;
     }
     float up1, up2;
     uperp_from(k.x_in, x_crit, d.nl_p1, d.spsi, d.cpsi, up1, up2);
@@ -582,8 +590,11 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
     nx *= inv; ny *= inv; nz *= inv;
     // a11, Eq. 7, recoil dropped: x_out = x_in + u.(k_out - k_in)
     const float x_out = fmaf(st, fmaf(up1, d.cphi, up2 * d.sphi), fmaf(k.upar, mu, xa));
+    // With Hubble drift every march needs the DDA step, hence 1/k: made here, where the three reciprocals (~270 cycles of
+    // MUFU + rounding fix-up) overlap the rest of the event instead of heading the next march; a static walk makes them
+    // only when a segment actually reaches a face
     ray_set_k(k.ray, nx, ny, nz);
-    k.inv_ok = false;
+    if (HUBBLE) { ray_set_inv(k.ray); k.inv_ok = true; } else k.inv_ok = false;
     k.V = fmaf(x_out, c.vth, dot3(c.vx, c.vy, c.vz, nx, ny, nz)) + dv_line;
     ++k.nscat;
     if (fabsf(k.V) > p.v_max_or_inf) return EV_TERMINATED;     // +inf when there is no v_max
