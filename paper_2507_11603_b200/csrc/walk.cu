@@ -388,7 +388,7 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
         if (sh.spectrum[i]) atomicAdd(p.spectrum + i, (unsigned long long)sh.spectrum[i]);
 }
 
-template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL>
+template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL, bool DB>
 __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __grid_constant__ WalkParams p) {
     __shared__ BlockTallies sh;
     __shared__ uint32_t sh_peelq[PEEL ? (WALK_THREADS / 32) * PEELQ_CAP * PEELQ_WORDS : 1];
@@ -469,11 +469,11 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
 
         // ---- a4-a7: one cell step for every marching lane ----
         if (state == LS_MARCH) {
-            const int ev = GL ? march_step_gridless(p, sh.voigt, k) : march_step<HUBBLE, EARLY>(p, sh.voigt, k);
+            const int ev = GL ? march_step_gridless(p, sh.voigt, k) : march_step<HUBBLE, EARLY, DB>(p, sh.voigt, k);
             if (ev == EV_HIT) {
                 env.mTot = -1.f;                                  // envelope not built yet
                 state = LS_TRIAL;
-                if (p.doublet_on) {                               // which interaction: one more counter block
+                if (DB && p.doublet_on) {                         // which interaction: one more counter block
                     select_line(p, k, k.rng.next4(k0, k1).x);
                     if (k.line < 0) state = LS_FINISH;            // dust: no atom velocity to draw
                 }
@@ -485,10 +485,10 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
         // march, instead of the whole warp waiting for its slowest lane (the paper's "largest source of thread
         // divergence"; E[max of 32 iterations]/E[iterations] = 2.1-4.2) ----
         if (state == LS_TRIAL) {
-            if (env.mTot < 0.f) env = upar_envelope(line_a(p, k), fabsf(k.x_in));
+            if (env.mTot < 0.f) env = upar_envelope(line_a<DB>(p, k), fabsf(k.x_in));
             ++k.rej_iters;
             float u;
-            const bool ok = upar_try<false>(env, line_a(p, k), k.rng.next4(k0, k1), 0.f, 0.f, u);
+            const bool ok = upar_try<false>(env, line_a<DB>(p, k), k.rng.next4(k0, k1), 0.f, 0.f, u);
             // fail-safe: acceptance is >= ~0.2 everywhere; 2^20 rejections cannot happen unless x is NaN
             if (ok || ++k.trials >= (1u << 20)) { k.upar = k.x_in < 0.f ? -u : u; state = LS_FINISH; }
         }
@@ -504,7 +504,7 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
             if (state == LS_FINISH) {
                 const float4 s1 = k.rng.next4(k0, k1), s2 = k.rng.next4(k0, k1);
                 const FinDraws d = fin_draws(s1, s2);
-                const int ev = finish_scatter<HUBBLE, PEEL, false, PEEL_FIRST>(p, sh.voigt, k, d, peel_rays, peel_cells, true, &pend);
+                const int ev = finish_scatter<HUBBLE, PEEL, false, PEEL_FIRST, DB>(p, sh.voigt, k, d, peel_rays, peel_cells, true, &pend);
                 if (ev == EV_SCATTERED) state = LS_MARCH;
                 else if (ev == EV_DUST_SCATTERED) { state = LS_MARCH; ++dust_scat; }
                 else { tally_packet(p, sh, ev, k); state = LS_IDLE; }
@@ -541,17 +541,19 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
 template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL = false>
 static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {
     int per_sm = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, walk_kernel<HUBBLE, PEEL, MIN_CTAS, GL>, WALK_THREADS, 0);
+    // both kernels are also compiled without the doublet (DB = false) for the runs that have none: its tests are uniform
+    // branches on a run constant, a few per scattering
+    const auto walk = p.doublet_on ? walk_kernel<HUBBLE, PEEL, MIN_CTAS, GL, true> : walk_kernel<HUBBLE, PEEL, MIN_CTAS, GL, false>;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, walk, WALK_THREADS, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     long long blocks = (long long)n_sm * per_sm;
     const long long need = (long long)((p.n_photons + 31) / 32);   // few packets: spread the warps over the SMs
     if (need < blocks) blocks = need < 1 ? 1 : need;
     if (blocks_out) *blocks_out = (int)blocks;
-    walk_kernel<HUBBLE, PEEL, MIN_CTAS, GL><<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(p);
+    walk<<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess || !p.pool) return e;
-    // the drain kernel is specialised on the doublet as well: its tests sit on the serial chain of a lone packet
     const auto drain = p.doublet_on ? drain_kernel<HUBBLE, PEEL, GL, true> : drain_kernel<HUBBLE, PEEL, GL, false>;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, drain, DRAIN_THREADS, 0);
     if (e != cudaSuccess) return e;
