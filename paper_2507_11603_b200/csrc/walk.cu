@@ -256,7 +256,7 @@ __device__ __noinline__ void peelq_serve(const WalkParams& p, const float2* s_ta
 // The drain kernel: launched behind walk_kernel on the same stream.  Each warp pops one parked packet at a time from the
 // global pool and walks it to its end, all 32 lanes on that one packet (see above).  4 warps per CTA — one per SM
 // sub-partition — and a register budget of its own (the walk kernel is held to 80 registers by its occupancy).
-template <bool HUBBLE, bool PEEL, bool GL, bool DB>
+template <bool HUBBLE, bool PEEL, bool GL, bool DB, int FIN>
 __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_constant__ WalkParams p) {
     __shared__ BlockTallies sh;
     __shared__ float4 s_win[DRAIN_WARPS][32 * WIN_STRIDE / 4];
@@ -355,7 +355,7 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
                 d.sphi = a2.x; d.cphi = a2.y; d.nl_p1 = a2.z;
                 d.spsi = b3.x; d.cpsi = b3.y; d.u_dust = u2.y; d.u_mix = u2.z; d.u_alb = u2.w;
                 uint32_t none = 0;
-                const int ev = finish_scatter<HUBBLE, PEEL, true, PEEL_QUEUED, DB>(p, sh.voigt, k, d, pr, none, lane == 0, &pend, &xc);
+                const int ev = finish_scatter<HUBBLE, PEEL, true, PEEL_QUEUED, DB, FIN>(p, sh.voigt, k, d, pr, none, lane == 0, &pend, &xc);
                 if (PEEL && pend.live) {                      // warp-uniform: every lane holds the same ray
                     if (lane == 0) peelq_put(peelq, peelq_cnt, pend);
                     pend.live = false;
@@ -388,7 +388,7 @@ __global__ void __launch_bounds__(DRAIN_THREADS, 4) drain_kernel(const __grid_co
         if (sh.spectrum[i]) atomicAdd(p.spectrum + i, (unsigned long long)sh.spectrum[i]);
 }
 
-template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL, bool DB>
+template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL, bool DB, int FIN>
 __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __grid_constant__ WalkParams p) {
     __shared__ BlockTallies sh;
     __shared__ uint32_t sh_peelq[PEEL ? (WALK_THREADS / 32) * PEELQ_CAP * PEELQ_WORDS : 1];
@@ -504,7 +504,7 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
             if (state == LS_FINISH) {
                 const float4 s1 = k.rng.next4(k0, k1), s2 = k.rng.next4(k0, k1);
                 const FinDraws d = fin_draws(s1, s2);
-                const int ev = finish_scatter<HUBBLE, PEEL, false, PEEL_FIRST, DB>(p, sh.voigt, k, d, peel_rays, peel_cells, true, &pend);
+                const int ev = finish_scatter<HUBBLE, PEEL, false, PEEL_FIRST, DB, FIN>(p, sh.voigt, k, d, peel_rays, peel_cells, true, &pend);
                 if (ev == EV_SCATTERED) state = LS_MARCH;
                 else if (ev == EV_DUST_SCATTERED) { state = LS_MARCH; ++dust_scat; }
                 else { tally_packet(p, sh, ev, k); state = LS_IDLE; }
@@ -538,12 +538,10 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
 // issue-bound, 4 CTAs (64 registers, 32 warps) when it does not and the walk needs more gathers in flight
 // (+18 % on the 512^3 gather workload, -6 % on the cache-resident sphere); 2 CTAs with peel-off (<= 128 registers).
 // The drain kernel follows on the same stream: a persistent grid of 4-warp CTAs whose warps pop parked packets.
-template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL = false>
-static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {
+template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL, bool DB, int FIN>
+static cudaError_t launch_pair(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {
     int per_sm = 0;
-    // both kernels are also compiled without the doublet (DB = false) for the runs that have none: its tests are uniform
-    // branches on a run constant, a few per scattering
-    const auto walk = p.doublet_on ? walk_kernel<HUBBLE, PEEL, MIN_CTAS, GL, true> : walk_kernel<HUBBLE, PEEL, MIN_CTAS, GL, false>;
+    const auto walk = walk_kernel<HUBBLE, PEEL, MIN_CTAS, GL, DB, FIN>;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, walk, WALK_THREADS, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
@@ -554,7 +552,7 @@ static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t st
     walk<<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(p);
     e = cudaGetLastError();
     if (e != cudaSuccess || !p.pool) return e;
-    const auto drain = p.doublet_on ? drain_kernel<HUBBLE, PEEL, GL, true> : drain_kernel<HUBBLE, PEEL, GL, false>;
+    const auto drain = drain_kernel<HUBBLE, PEEL, GL, DB, FIN>;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, drain, DRAIN_THREADS, 0);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
@@ -567,6 +565,18 @@ static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t st
     if (cap < dblocks) dblocks = cap;
     drain<<<(unsigned)dblocks, DRAIN_THREADS, 0, stream>>>(p);
     return cudaGetLastError();
+}
+
+// Both kernels are also compiled for the run constants whose tests would otherwise be uniform branches in every scattering:
+// without the doublet (DB = false) for the runs that have none, and for the common case of isotropic scattering in core and
+// wing with each core-skipping mode (FIN = 1 / 2 / 3; finish_scatter).  Everything else takes the generic kernels.
+template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL = false>
+static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {
+    if (p.doublet_on) return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, true, 0>(p, n_sm, stream, blocks_out);
+    if (p.phase_core != 0 || p.phase_wing != 0) return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, false, 0>(p, n_sm, stream, blocks_out);
+    if (p.core_skip_mode == 1) return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, false, 1>(p, n_sm, stream, blocks_out);
+    if (p.core_skip_mode == 2) return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, false, 2>(p, n_sm, stream, blocks_out);
+    return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, false, 3>(p, n_sm, stream, blocks_out);
 }
 
 // Slots the pool must hold for a launch of `blocks` walk CTAs.

@@ -515,7 +515,10 @@ __device__ __forceinline__ float line_a(const WalkParams& p, const Packet& k) { 
 // a7, a9-a12: the interaction itself (PAPER.md 2.3.1): dust or line, u_perp (Eq. 5, core-skipping
 // PAPER.md:244), phase function, rotation, Eq. 7 with the recoil dropped, peel-off
 // before k' is adopted, new tau_target.  Returns EV_ABSORBED / EV_TERMINATED / EV_CAPPED / EV_SCATTERED.
-template <bool HUBBLE, bool PEEL, bool PRE, int PMODE = PEEL_INLINE, bool DB = true>
+// FIN: the event compiled for the run's core-skipping mode and phase functions (run constants whose tests are uniform branches,
+// a handful per scattering): 0 = generic (read from the options), 1 / 2 / 3 = isotropic scattering in core and wing with
+// core-skipping mode 1 / 2 / 0.
+template <bool HUBBLE, bool PEEL, bool PRE, int PMODE = PEEL_INLINE, bool DB = true, int FIN = 0>
 __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2* s_tab, Packet& k, const FinDraws& d,
                                               uint32_t& peel_rays, uint32_t& peel_cells, bool add, PeelPend* pend = nullptr,
                                               float* xc_cache = nullptr) {
@@ -553,11 +556,14 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
     // x_crit depends on the run and, in local mode, on the cell (and the line of a doublet): the cooperative drain, whose
     // packet scatters ~1e5 times per cell, keeps it between scatterings (xc_cache < 0 = not yet known for this cell; the mode
     // tests and the cube root are ~200 cycles of a lone packet's serial chain)
+    constexpr int CS = FIN == 1 ? 1 : FIN == 2 ? 2 : FIN == 3 ? 0 : -1;
+    constexpr bool ISO = FIN != 0;
+    const int cs_mode = CS >= 0 ? CS : p.core_skip_mode;
     float x_crit = 0.f;
     if (!DB && xc_cache && *xc_cache >= 0.f) x_crit = *xc_cache;
     else {
-        if (p.core_skip_mode == 1) x_crit = p.x_crit;
-        else if (p.core_skip_mode == 2) {              // local: a tau_0 over half a cell (reading A7)
+        if (cs_mode == 1) x_crit = p.x_crit;
+        else if (cs_mode == 2) {              // local: a tau_0 over half a cell (reading A7)
             const float atau = a_l * c.nsig * ((DB && k.line > 0) ? p.db_rs : 1.f) * 0.5f;
             x_crit = atau >= 1.f ? 0.2f * cbrtf(atau) : 0.f;
         }
@@ -566,7 +572,7 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
     float up1, up2;
     uperp_from(k.x_in, x_crit, d.nl_p1, d.spsi, d.cpsi, up1, up2);
     const float xsel = p.phase_frame == 0 ? fabsf(k.x_in - k.upar) : fabsf(k.x_in);
-    const int phase = xsel > p.phase_split_x ? p.phase_wing : p.phase_core;
+    const int phase = ISO ? 0 : (xsel > p.phase_split_x ? p.phase_wing : p.phase_core);
     bool is_dipole;
     const float mu = sample_mu<PRE>(phase, d.u_mix, d.r_mu, d.mu_dip, is_dipole);
     float e1[3], e2[3];
