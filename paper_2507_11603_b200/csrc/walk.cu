@@ -569,10 +569,12 @@ static cudaError_t launch_pair(const WalkParams& p, int n_sm, cudaStream_t strea
 
 // Both kernels are also compiled for the run constants whose tests would otherwise be uniform branches in every scattering:
 // without the doublet (DB = false) for the runs that have none, and for the common case of isotropic scattering in core and
-// wing with each core-skipping mode (FIN = 1 / 2 / 3; finish_scatter).  Everything else takes the generic kernels.
+// wing with each core-skipping mode (FIN = 1 / 2 / 3; finish_scatter) and for config 3's dipole core / isotropic wing (FIN = 4).  Everything else takes the generic kernels.
 template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL = false>
 static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {
     if (p.doublet_on) return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, true, 0>(p, n_sm, stream, blocks_out);
+    if (p.phase_core == 1 && p.phase_wing == 0 && p.phase_frame == 0 && p.core_skip_mode == 1)
+        return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, false, 4>(p, n_sm, stream, blocks_out);
     if (p.phase_core != 0 || p.phase_wing != 0) return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, false, 0>(p, n_sm, stream, blocks_out);
     if (p.core_skip_mode == 1) return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, false, 1>(p, n_sm, stream, blocks_out);
     if (p.core_skip_mode == 2) return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, false, 2>(p, n_sm, stream, blocks_out);

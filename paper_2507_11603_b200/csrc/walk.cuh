@@ -517,7 +517,8 @@ __device__ __forceinline__ float line_a(const WalkParams& p, const Packet& k) { 
 // before k' is adopted, new tau_target.  Returns EV_ABSORBED / EV_TERMINATED / EV_CAPPED / EV_SCATTERED.
 // FIN: the event compiled for the run's core-skipping mode and phase functions (run constants whose tests are uniform branches,
 // a handful per scattering): 0 = generic (read from the options), 1 / 2 / 3 = isotropic scattering in core and wing with
-// core-skipping mode 1 / 2 / 0.
+// core-skipping mode 1 / 2 / 0, 4 = BASELINE.json config 3's combination: dipole core, isotropic wing, split on the atom-frame
+// frequency, core-skipping mode 1.
 template <bool HUBBLE, bool PEEL, bool PRE, int PMODE = PEEL_INLINE, bool DB = true, int FIN = 0>
 __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2* s_tab, Packet& k, const FinDraws& d,
                                               uint32_t& peel_rays, uint32_t& peel_cells, bool add, PeelPend* pend = nullptr,
@@ -556,8 +557,8 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
     // x_crit depends on the run and, in local mode, on the cell (and the line of a doublet): the cooperative drain, whose
     // packet scatters ~1e5 times per cell, keeps it between scatterings (xc_cache < 0 = not yet known for this cell; the mode
     // tests and the cube root are ~200 cycles of a lone packet's serial chain)
-    constexpr int CS = FIN == 1 ? 1 : FIN == 2 ? 2 : FIN == 3 ? 0 : -1;
-    constexpr bool ISO = FIN != 0;
+    constexpr int CS = (FIN == 1 || FIN == 4) ? 1 : FIN == 2 ? 2 : FIN == 3 ? 0 : -1;
+    constexpr bool ISO = FIN >= 1 && FIN <= 3;
     const int cs_mode = CS >= 0 ? CS : p.core_skip_mode;
     float x_crit = 0.f;
     if (!DB && xc_cache && *xc_cache >= 0.f) x_crit = *xc_cache;
@@ -571,8 +572,8 @@ __device__ __forceinline__ int finish_scatter(const WalkParams& p, const float2*
     }
     float up1, up2;
     uperp_from(k.x_in, x_crit, d.nl_p1, d.spsi, d.cpsi, up1, up2);
-    const float xsel = p.phase_frame == 0 ? fabsf(k.x_in - k.upar) : fabsf(k.x_in);
-    const int phase = ISO ? 0 : (xsel > p.phase_split_x ? p.phase_wing : p.phase_core);
+    const float xsel = (FIN == 4 || p.phase_frame == 0) ? fabsf(k.x_in - k.upar) : fabsf(k.x_in);
+    const int phase = ISO ? 0 : FIN == 4 ? (xsel > p.phase_split_x ? 0 : 1) : (xsel > p.phase_split_x ? p.phase_wing : p.phase_core);
     bool is_dipole;
     const float mu = sample_mu<PRE>(phase, d.u_mix, d.r_mu, d.mu_dip, is_dipole);
     float e1[3], e2[3];
