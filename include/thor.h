@@ -136,7 +136,9 @@ typedef struct thor_opts {
                                          0 = the built-in limit 2^32 - 1 (reading A26).  Required (> 0) on a
                                          grid that is periodic on all three axes: no packet can ever leave it */
     int32_t walk_variant;             /* 0 (default): kernel variant chosen by grid size; 3 / 4: force the cache-resident /
-                                         beyond-L2 variant of the walk kernel.  Results do not depend on it (tests, tuning) */
+                                         beyond-L2 variant of the walk kernel; + 16: the generic kernels instead of the ones compiled
+                                         for the run's doublet / core-skipping / phase-function options.  Results do not
+                                         depend on it (tests, tuning) */
     int32_t drain_mode;               /* 0 (default): once the photon counter is dry, warps left with <= 4 packets hand them
                                          to the cooperative drain kernel; 1: the walk kernel finishes every
                                          packet itself.  Results do not depend on it */

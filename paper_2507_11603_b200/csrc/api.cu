@@ -397,7 +397,7 @@ extern "C" thor_status thor_run_async(thor_ctx* ctx, unsigned long long n_photon
     if (o.spec_bins > 0 && !(o.spec_hi > o.spec_lo)) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_hi must exceed spec_lo");
     if (o.spec_mode != 0 && o.spec_mode != 1) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_mode must be 0 or 1");
     if (o.spec_mode == 0 && !(o.spec_T_ref > 0)) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_T_ref must be > 0");
-    if ((o.walk_variant != 0 && o.walk_variant != 3 && o.walk_variant != 4) || (o.drain_mode != 0 && o.drain_mode != 1)) return fail(ctx, THOR_ERR_ARG, "thor_run: bad walk_variant / drain_mode");
+    if (((o.walk_variant & ~16) != 0 && (o.walk_variant & ~16) != 3 && (o.walk_variant & ~16) != 4) || (o.drain_mode != 0 && o.drain_mode != 1)) return fail(ctx, THOR_ERR_ARG, "thor_run: bad walk_variant / drain_mode");
     if (!(o.dust_albedo >= 0 && o.dust_albedo <= 1) || !(o.dust_g >= -1 && o.dust_g <= 1)) return fail(ctx, THOR_ERR_ARG, "thor_run: dust_albedo must be in [0, 1] and dust_g in [-1, 1]");
     if (o.doublet_on && (!std::isfinite(o.doublet_dv_kms) || !(o.doublet_sigma_ratio >= 0) || !(o.doublet_a_ratio > 0) || !std::isfinite(o.doublet_sigma_ratio) || !std::isfinite(o.doublet_a_ratio)))
         return fail(ctx, THOR_ERR_ARG, "thor_run: bad doublet options");
@@ -616,7 +616,7 @@ extern "C" thor_status thor_run_noalloc(thor_ctx* ctx, unsigned long long n_phot
     if (o.spec_bins > 0 && !(o.spec_hi > o.spec_lo)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: spec_hi must exceed spec_lo");
     if (o.spec_mode != 0 && o.spec_mode != 1) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: spec_mode must be 0 or 1");
     if (o.spec_mode == 0 && !(o.spec_T_ref > 0)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: spec_T_ref must be > 0");
-    if ((o.walk_variant != 0 && o.walk_variant != 3 && o.walk_variant != 4) || (o.drain_mode != 0 && o.drain_mode != 1)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: bad walk_variant / drain_mode");
+    if (((o.walk_variant & ~16) != 0 && (o.walk_variant & ~16) != 3 && (o.walk_variant & ~16) != 4) || (o.drain_mode != 0 && o.drain_mode != 1)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: bad walk_variant / drain_mode");
     if (!(o.dust_albedo >= 0 && o.dust_albedo <= 1) || !(o.dust_g >= -1 && o.dust_g <= 1)) return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: dust_albedo must be in [0, 1] and dust_g in [-1, 1]");
     if (o.doublet_on && (!std::isfinite(o.doublet_dv_kms) || !(o.doublet_sigma_ratio >= 0) || !(o.doublet_a_ratio > 0) || !std::isfinite(o.doublet_sigma_ratio) || !std::isfinite(o.doublet_a_ratio)))
         return fail(ctx, THOR_ERR_ARG, "thor_run_noalloc: bad doublet options");

@@ -106,7 +106,7 @@ struct WalkParams {
     float dust_albedo, dust_g;
     int doublet_on;
     float db_dv, db_rs, db_ra;           // line 2: centre offset [km/s], sigma_0 ratio, a ratio
-    int walk_variant;                    // 0 = by grid size, 3 / 4 = force the cache-resident / beyond-L2 kernel (tests)
+    int walk_variant;                    // 0 = by grid size, 3 / 4 = force the cache-resident / beyond-L2 kernel; + 16 = the generic kernels (tests)
 };
 
 }  // namespace thor

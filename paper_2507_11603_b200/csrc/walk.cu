@@ -572,7 +572,7 @@ static cudaError_t launch_pair(const WalkParams& p, int n_sm, cudaStream_t strea
 // wing with each core-skipping mode (FIN = 1 / 2 / 3; finish_scatter) and for config 3's dipole core / isotropic wing (FIN = 4).  Everything else takes the generic kernels.
 template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL = false>
 static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {
-    if (p.doublet_on) return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, true, 0>(p, n_sm, stream, blocks_out);
+    if (p.doublet_on || (p.walk_variant & 16)) return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, true, 0>(p, n_sm, stream, blocks_out);   // 16: generic kernels (tests)
     if (p.phase_core == 1 && p.phase_wing == 0 && p.phase_frame == 0 && p.core_skip_mode == 1)
         return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, false, 4>(p, n_sm, stream, blocks_out);
     if (p.phase_core != 0 || p.phase_wing != 0) return launch_pair<HUBBLE, PEEL, MIN_CTAS, GL, false, 0>(p, n_sm, stream, blocks_out);
@@ -590,7 +590,7 @@ cudaError_t launch_walk(const WalkParams& p, int n_sm, cudaStream_t stream, int*
     const bool hub = p.hubble != 0.f, peel = p.peel_on != 0;
     const double cells = (double)p.g.nx * p.g.ny * p.g.nz;
     const double grid_bytes = cells * (p.packed ? 32.0 : (p.has_dust ? 24.0 : 20.0));
-    const bool beyond_l2 = p.walk_variant ? p.walk_variant == 4 : grid_bytes > 96.0e6;
+    const bool beyond_l2 = (p.walk_variant & ~16) ? (p.walk_variant & ~16) == 4 : grid_bytes > 96.0e6;
     if (peel) return hub ? launch_variant<true, true, THOR_PEEL_MIN_CTAS>(p, n_sm, stream, blocks_out)
                          : launch_variant<false, true, THOR_PEEL_MIN_CTAS>(p, n_sm, stream, blocks_out);
     if (beyond_l2) return hub ? launch_variant<true, false, 4>(p, n_sm, stream, blocks_out)

@@ -714,6 +714,29 @@ def test_run_async_overlaps_contexts_from_one_thread(thor):
     [c.close() for c in ctxs]                                          # destroying a context with a pending run waits for it
 
 
+def test_specialised_kernels_are_bit_identical_to_the_generic_ones(thor):
+    """Both kernels are compiled without the doublet and for the run's core-skipping mode and phase functions (isotropic /
+    isotropic with mode 0, 1, 2; config 3's dipole core).  walk_variant + 16 forces the generic kernels: same records, same
+    tallies, bit for bit — through the walk kernel and through the drain kernel."""
+    sph = W.static_sphere(n=16, tau0=1e5, T=10.0, n_photons=3000)
+    cases = [dict(W.expanding_shell(n=32, n_photons=20_000), tag="iso, no core-skipping"),
+             dict(sph, opts=dict(sph["opts"], core_skip_mode=1, x_crit=3.0), tag="iso, global core-skipping"),
+             dict(W.turbulent_box(n=32, n_src=256, n_photons=3000, peel_pix=16, peel_bins=20, cell_pc=1e-3), tag="iso, local core-skipping, peel"),
+             dict(W.cosmic_web(n=32, n_src=256, n_photons=3000, mean_n=1e-8, map_pix=16, v_max=40.0), tag="iso, local, Hubble, peel"),
+             dict(W.static_slab(n_photons=3000), tag="dipole core / isotropic wing, global core-skipping")]
+    for w in cases:
+        w["opts"] = dict(w["opts"], max_scatter=20_000)
+        for drain_mode in (0, 1):
+            a = thor.run_workload(w, drain_mode=drain_mode)
+            b = thor.run_workload(w, drain_mode=drain_mode, walk_variant=16)
+            assert a["raw"].tobytes() == b["raw"].tobytes(), w["tag"]
+            assert a["counters"] == b["counters"], w["tag"]
+            assert np.array_equal(a["spectrum"], b["spectrum"]) and np.array_equal(a["nscat_hist"], b["nscat_hist"])
+            if a["cube"] is not None:
+                assert np.array_equal(a["cube"], b["cube"]), w["tag"]
+            assert a["counters"]["scatterings"] > w["n_photons"]
+
+
 def test_mean_scattering_count_within_one_percent(thor, oracle):
     """BASELINE.json's bar as stated: mean scattering count within 1 % — on a rung where the standard error lets it bind
     (reading A23): tau0 = 1e2, 4e5 packets per side, 3 SE = 0.6 %.  Plain |dmean| <= 1 %, no SE allowance."""
