@@ -139,9 +139,12 @@ typedef struct thor_opts {
                                          beyond-L2 variant of the walk kernel; + 16: the generic kernels instead of the ones compiled
                                          for the run's doublet / core-skipping / phase-function options.  Results do not
                                          depend on it (tests, tuning) */
-    int32_t drain_mode;               /* 0 (default): once the photon counter is dry, warps left with <= 4 packets hand them
-                                         to the cooperative drain kernel; 1: the walk kernel finishes every
-                                         packet itself.  Results do not depend on it */
+    int32_t drain_mode;               /* how the tail of a run is walked once the photon counter is dry.  0 (default): in
+                                         two passes — a warp down to half its lanes parks its packets, a second launch of
+                                         the walk kernel re-packs them into full warps — and warps left with
+                                         <= 4 packets hand them to the cooperative drain kernel; 2: one pass,
+                                         then the drain kernel; 1: the walk kernel finishes every packet itself.  Results do
+                                         not depend on it */
     double dust_albedo;               /* PAPER.md 2.3.2, Eq. 8: with albedo > 0 kdust is the dust EXTINCTION coefficient and an
                                          interaction with dust scatters with this probability, else destroys (0: absorption
                                          only, as before; the paper's fiducial value is 0.32) */

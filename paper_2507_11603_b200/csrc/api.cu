@@ -15,6 +15,7 @@
 namespace thor {
 cudaError_t launch_walk(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out);
 long long walk_pool_slots(int n_sm);
+long long walk_pool_mid_slots(int n_sm);
 int walk_pool_words();
 cudaError_t launch_volume_render(const WalkParams& p, const TransferFn& tf, long long n_rays, const float* org,
                                  const float* dir, float* out_rgba, cudaStream_t stream);
@@ -54,6 +55,7 @@ struct thor_ctx {
     thor::RawRecord* d_raw = nullptr;
     size_t raw_cap = 0;
     uint32_t* d_pool = nullptr;                 // parked packets for the drain kernel
+    uint32_t* d_pool_mid = nullptr;             // parked packets between the two passes of the tail
     unsigned int* d_pool_order = nullptr;
     // last run
     bool have_run = false;
@@ -81,7 +83,7 @@ struct DevGuard {
 };
 
 static constexpr size_t SMALL_NEXT = 0, SMALL_COUNTERS = 1, SMALL_HIST = SMALL_COUNTERS + thor::N_COUNTERS,
-                        SMALL_SPEC = SMALL_HIST + 64, SMALL_TIMES = SMALL_SPEC + 4096 + 2, SMALL_MAXN = SMALL_TIMES + 2, SMALL_POOL = SMALL_MAXN + 1, SMALL_TOTAL = SMALL_POOL + 2;
+                        SMALL_SPEC = SMALL_HIST + 64, SMALL_TIMES = SMALL_SPEC + 4096 + 2, SMALL_MAXN = SMALL_TIMES + 2, SMALL_POOL = SMALL_MAXN + 1, SMALL_TOTAL = SMALL_POOL + 3;
 
 static thor_status fail(thor_ctx* c, thor_status s, const std::string& msg) {
     if (c) c->err = msg;
@@ -131,6 +133,7 @@ extern "C" void thor_grid_destroy(thor_ctx* ctx) {
     if (ctx->d_cube) cudaFree(ctx->d_cube);
     if (ctx->d_raw) cudaFree(ctx->d_raw);
     if (ctx->d_pool) cudaFree(ctx->d_pool);
+    if (ctx->d_pool_mid) cudaFree(ctx->d_pool_mid);
     if (ctx->d_pool_order) cudaFree(ctx->d_pool_order);
     if (ctx->l2_persist) {                        // drop the access-policy window of the caller's stream
         cudaStreamAttrValue av{};
@@ -397,7 +400,7 @@ extern "C" thor_status thor_run_async(thor_ctx* ctx, unsigned long long n_photon
     if (o.spec_bins > 0 && !(o.spec_hi > o.spec_lo)) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_hi must exceed spec_lo");
     if (o.spec_mode != 0 && o.spec_mode != 1) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_mode must be 0 or 1");
     if (o.spec_mode == 0 && !(o.spec_T_ref > 0)) return fail(ctx, THOR_ERR_ARG, "thor_run: spec_T_ref must be > 0");
-    if (((o.walk_variant & ~16) != 0 && (o.walk_variant & ~16) != 3 && (o.walk_variant & ~16) != 4) || (o.drain_mode != 0 && o.drain_mode != 1)) return fail(ctx, THOR_ERR_ARG, "thor_run: bad walk_variant / drain_mode");
+    if (((o.walk_variant & ~16) != 0 && (o.walk_variant & ~16) != 3 && (o.walk_variant & ~16) != 4) || (o.drain_mode < 0 || o.drain_mode > 2)) return fail(ctx, THOR_ERR_ARG, "thor_run: bad walk_variant / drain_mode");
     if (!(o.dust_albedo >= 0 && o.dust_albedo <= 1) || !(o.dust_g >= -1 && o.dust_g <= 1)) return fail(ctx, THOR_ERR_ARG, "thor_run: dust_albedo must be in [0, 1] and dust_g in [-1, 1]");
     if (o.doublet_on && (!std::isfinite(o.doublet_dv_kms) || !(o.doublet_sigma_ratio >= 0) || !(o.doublet_a_ratio > 0) || !std::isfinite(o.doublet_sigma_ratio) || !std::isfinite(o.doublet_a_ratio)))
         return fail(ctx, THOR_ERR_ARG, "thor_run: bad doublet options");
@@ -485,11 +488,14 @@ extern "C" thor_status thor_run_async(thor_ctx* ctx, unsigned long long n_photon
     p.doublet_on = o.doublet_on ? 1 : 0;
     p.db_dv = (float)o.doublet_dv_kms; p.db_rs = (float)o.doublet_sigma_ratio; p.db_ra = (float)o.doublet_a_ratio;
     DevGuard dev_guard(ctx->device);
-    if (o.drain_mode == 0 && !ctx->d_pool)
+    if (o.drain_mode != 1 && !ctx->d_pool)
         CU(cudaMalloc(&ctx->d_pool, (size_t)thor::walk_pool_slots(ctx->n_sm) * thor::walk_pool_words() * sizeof(uint32_t)));
-    if (o.drain_mode == 0 && !ctx->d_pool_order)
+    if (o.drain_mode != 1 && !ctx->d_pool_order)
         CU(cudaMalloc(&ctx->d_pool_order, (size_t)thor::walk_pool_slots(ctx->n_sm) * sizeof(unsigned int)));
-    p.pool = o.drain_mode == 0 ? ctx->d_pool : nullptr;
+    if (o.drain_mode == 0 && !ctx->d_pool_mid)
+        CU(cudaMalloc(&ctx->d_pool_mid, (size_t)thor::walk_pool_mid_slots(ctx->n_sm) * thor::walk_pool_words() * sizeof(uint32_t)));
+    p.pool = o.drain_mode != 1 ? ctx->d_pool : nullptr;
+    p.pool_mid = o.drain_mode == 0 ? ctx->d_pool_mid : nullptr;
     p.pool_order = ctx->d_pool_order;
     const bool keep = o.accumulate && ctx->have_run;
     if (keep) {
@@ -532,7 +538,8 @@ extern "C" thor_status thor_run_async(thor_ctx* ctx, unsigned long long n_photon
     p.t_dry = ctx->d_small + SMALL_TIMES + 1;
     p.pool_count = ctx->d_small + SMALL_POOL;
     p.pool_next = ctx->d_small + SMALL_POOL + 1;
-    CU(cudaMemsetAsync(ctx->d_small + SMALL_POOL, 0, 2 * sizeof(unsigned long long), ctx->stream));
+    p.pool_mid_count = ctx->d_small + SMALL_POOL + 2;
+    CU(cudaMemsetAsync(ctx->d_small + SMALL_POOL, 0, 3 * sizeof(unsigned long long), ctx->stream));
     p.counters = ctx->d_small + SMALL_COUNTERS;
     p.nscat_hist = ctx->d_small + SMALL_HIST;
     p.spectrum = ctx->d_small + SMALL_SPEC;
@@ -664,6 +671,7 @@ extern "C" thor_status thor_run_noalloc(thor_ctx* ctx, unsigned long long n_phot
     p.pool_count = small + 4; p.pool_next = small + 5;
     p.pool_order = reinterpret_cast<unsigned int*>(scratch + NOALLOC_ORDER_OFF);
     p.pool = o.drain_mode == 0 ? reinterpret_cast<uint32_t*>(scratch + NOALLOC_POOL_OFF) : nullptr;
+    p.pool_mid = nullptr; p.pool_mid_count = nullptr;       // single-pass tail: the static scratch holds one pool
     p.counters = counters_out; p.nscat_hist = nscat_hist_out; p.spectrum = spectrum_out;
     p.cube = nullptr; p.raw = nullptr;
     int blocks = 0;

@@ -95,6 +95,14 @@ struct WalkParams {
     unsigned long long* pool_count;      // packets parked
     unsigned long long* pool_next;       // next slot to pop
     unsigned int* pool_order;            // [slots]: pool slots by decreasing scattering count (longest first)
+    // two-pass tail: the first walk launch parks a warp's packets into pool_mid once the counter is dry and at
+    // most half its lanes are live; a second launch of the walk kernel re-packs them into full warps and walks on
+    uint32_t* pool_mid;                  // nullptr = single pass
+    unsigned long long* pool_mid_count;
+    // per launch of the walk kernel (set by the launcher):
+    int resume;                          // 1: no photon counter; lanes start from the packets of resume_in
+    const uint32_t* resume_in; const unsigned long long* resume_count;
+    uint32_t* park_out; unsigned long long* park_count; int park_lanes;   // where, and at how many live lanes, a warp parks
     // gridless dataset (PAPER.md 3.3: spherical shell / infinite slab with power-law density and velocity); gl_geom < 0 = grid
     int gl_geom;                         // -1 grid, 0 shell / sphere, 1 slab
     double gl_rin, gl_rout;              // length units

@@ -33,6 +33,10 @@ constexpr int REFILL_MIN_LANES = THOR_REFILL_MIN_LANES;
 #ifndef THOR_COOP_MAX_LANES
 #define THOR_COOP_MAX_LANES 4
 #endif
+#ifndef THOR_PARK1_LANES
+#define THOR_PARK1_LANES 16
+#endif
+constexpr int PARK1_LANES = THOR_PARK1_LANES;           // first pass of the tail: a warp parks at this many live lanes
 constexpr int COOP_MAX_LANES = THOR_COOP_MAX_LANES;     // cooperative drain when a warp has at most this many packets left
 constexpr int WIN_STRIDE = 20;                          // floats per window slot (16 used; 80 B keeps STS.128 conflict-free)
 constexpr int PK_WORDS = 48;                            // 32-bit words of a parked packet
@@ -413,7 +417,12 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
     UparEnvelope env;
     env.mTot = -1.f;
     uint32_t peel_rays = 0, peel_cells = 0, dust_scat = 0;
-    bool more = true;                                         // warp-uniform: photon counter not yet exhausted
+    bool more = !p.resume;                                    // warp-uniform: photon counter not yet exhausted
+    if (p.resume) {                                           // second pass of the tail: 32 parked packets per warp, densely
+        const unsigned long long n_in = *p.resume_count;
+        const unsigned long long idx = ((unsigned long long)blockIdx.x * (WALK_THREADS / 32) + (threadIdx.x >> 5)) * 32ull + lane;
+        state = idx < n_in ? park_load<GL>(p.resume_in + idx * PK_WORDS, k) : LS_OUT;
+    }
 
     for (;;) {
         // ---- a14 + a2/a3: refill idle lanes from the global photon counter, emit ----
@@ -453,16 +462,16 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
                 more = false;
             }
         }
-        if (!more && COOP_MAX_LANES > 0 && p.pool) {
+        if (!more && p.park_out) {
             // the counter is dry and this warp is down to a few packets: park them in the global pool for the drain
             // kernel (one warp per packet there) and leave
             const bool act = state == LS_MARCH || state == LS_TRIAL || state == LS_FINISH;
             const unsigned live = __ballot_sync(0xffffffffu, act);
-            if (live && __popc(live) <= COOP_MAX_LANES) {
+            if (live && __popc(live) <= p.park_lanes) {
                 unsigned long long base = 0;
-                if (lane == 0) base = atomicAdd(p.pool_count, (unsigned long long)__popc(live));
+                if (lane == 0) base = atomicAdd(p.park_count, (unsigned long long)__popc(live));
                 base = __shfl_sync(0xffffffffu, base, 0);
-                if (act) park_store<GL>(p.pool + (base + __popc(live & ((1u << lane) - 1u))) * PK_WORDS, k, state);
+                if (act) park_store<GL>(p.park_out + (base + __popc(live & ((1u << lane) - 1u))) * PK_WORDS, k, state);
                 break;
             }
         }
@@ -549,9 +558,27 @@ static cudaError_t launch_pair(const WalkParams& p, int n_sm, cudaStream_t strea
     const long long need = (long long)((p.n_photons + 31) / 32);   // few packets: spread the warps over the SMs
     if (need < blocks) blocks = need < 1 ? 1 : need;
     if (blocks_out) *blocks_out = (int)blocks;
-    walk<<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(p);
+    // The tail in two passes: once the counter is dry a warp of the first launch parks its packets as soon as at
+    // most PARK1_LANES are live; a second launch of the same kernel re-packs them, 32 to a warp, and walks on until a warp is down
+    // to COOP_MAX_LANES packets, which go to the cooperative drain.  Half-empty warps cost what full ones do.
+    const bool two_pass = p.pool != nullptr && p.pool_mid != nullptr;
+    WalkParams p1 = p;
+    p1.resume = 0; p1.resume_in = nullptr; p1.resume_count = nullptr;
+    p1.park_out = two_pass ? p.pool_mid : p.pool;
+    p1.park_count = two_pass ? p.pool_mid_count : p.pool_count;
+    p1.park_lanes = two_pass ? PARK1_LANES : COOP_MAX_LANES;
+    walk<<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(p1);
     e = cudaGetLastError();
     if (e != cudaSuccess || !p.pool) return e;
+    if (two_pass) {
+        WalkParams p2 = p;
+        p2.resume = 1; p2.resume_in = p.pool_mid; p2.resume_count = p.pool_mid_count;
+        p2.park_out = p.pool; p2.park_count = p.pool_count; p2.park_lanes = COOP_MAX_LANES;
+        blocks = (blocks * PARK1_LANES + 31) / 32;            // 32 parked packets per warp cover everything the first pass can park
+        walk<<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(p2);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
     const auto drain = drain_kernel<HUBBLE, PEEL, GL, DB, FIN>;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, drain, DRAIN_THREADS, 0);
     if (e != cudaSuccess) return e;
@@ -583,6 +610,7 @@ static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t st
 
 // Slots the pool must hold for a launch of `blocks` walk CTAs.
 long long walk_pool_slots(int n_sm) { return (long long)n_sm * 4 * (WALK_THREADS / 32) * COOP_MAX_LANES; }
+long long walk_pool_mid_slots(int n_sm) { return (long long)n_sm * 4 * (WALK_THREADS / 32) * PARK1_LANES; }
 int walk_pool_words() { return PK_WORDS; }
 
 cudaError_t launch_walk(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {
