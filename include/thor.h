@@ -140,8 +140,8 @@ typedef struct thor_opts {
                                          for the run's doublet / core-skipping / phase-function options.  Results do not
                                          depend on it (tests, tuning) */
     int32_t drain_mode;               /* how the tail of a run is walked once the photon counter is dry.  0 (default): in
-                                         two passes — a warp down to half its lanes parks its packets, a second launch of
-                                         the walk kernel re-packs them into full warps — and warps left with
+                                         passes — a warp down to half its lanes parks its packets, the next launch of the
+                                         walk kernel re-packs them into full warps — and warps left with
                                          <= 4 packets hand them to the cooperative drain kernel; 2: one pass,
                                          then the drain kernel; 1: the walk kernel finishes every packet itself.  Results do
                                          not depend on it */

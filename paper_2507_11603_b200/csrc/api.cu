@@ -55,7 +55,7 @@ struct thor_ctx {
     thor::RawRecord* d_raw = nullptr;
     size_t raw_cap = 0;
     uint32_t* d_pool = nullptr;                 // parked packets for the drain kernel
-    uint32_t* d_pool_mid = nullptr;             // parked packets between the two passes of the tail
+    uint32_t* d_pool_mid = nullptr;             // parked packets between the passes of the tail (two halves)
     unsigned int* d_pool_order = nullptr;
     // last run
     bool have_run = false;
@@ -83,7 +83,7 @@ struct DevGuard {
 };
 
 static constexpr size_t SMALL_NEXT = 0, SMALL_COUNTERS = 1, SMALL_HIST = SMALL_COUNTERS + thor::N_COUNTERS,
-                        SMALL_SPEC = SMALL_HIST + 64, SMALL_TIMES = SMALL_SPEC + 4096 + 2, SMALL_MAXN = SMALL_TIMES + 2, SMALL_POOL = SMALL_MAXN + 1, SMALL_TOTAL = SMALL_POOL + 3;
+                        SMALL_SPEC = SMALL_HIST + 64, SMALL_TIMES = SMALL_SPEC + 4096 + 2, SMALL_MAXN = SMALL_TIMES + 2, SMALL_POOL = SMALL_MAXN + 1, SMALL_TOTAL = SMALL_POOL + 4;
 
 static thor_status fail(thor_ctx* c, thor_status s, const std::string& msg) {
     if (c) c->err = msg;
@@ -493,7 +493,7 @@ extern "C" thor_status thor_run_async(thor_ctx* ctx, unsigned long long n_photon
     if (o.drain_mode != 1 && !ctx->d_pool_order)
         CU(cudaMalloc(&ctx->d_pool_order, (size_t)thor::walk_pool_slots(ctx->n_sm) * sizeof(unsigned int)));
     if (o.drain_mode == 0 && !ctx->d_pool_mid)
-        CU(cudaMalloc(&ctx->d_pool_mid, (size_t)thor::walk_pool_mid_slots(ctx->n_sm) * thor::walk_pool_words() * sizeof(uint32_t)));
+        CU(cudaMalloc(&ctx->d_pool_mid, 2 * (size_t)thor::walk_pool_mid_slots(ctx->n_sm) * thor::walk_pool_words() * sizeof(uint32_t)));   // two halves
     p.pool = o.drain_mode != 1 ? ctx->d_pool : nullptr;
     p.pool_mid = o.drain_mode == 0 ? ctx->d_pool_mid : nullptr;
     p.pool_order = ctx->d_pool_order;
@@ -539,7 +539,7 @@ extern "C" thor_status thor_run_async(thor_ctx* ctx, unsigned long long n_photon
     p.pool_count = ctx->d_small + SMALL_POOL;
     p.pool_next = ctx->d_small + SMALL_POOL + 1;
     p.pool_mid_count = ctx->d_small + SMALL_POOL + 2;
-    CU(cudaMemsetAsync(ctx->d_small + SMALL_POOL, 0, 3 * sizeof(unsigned long long), ctx->stream));
+    CU(cudaMemsetAsync(ctx->d_small + SMALL_POOL, 0, 4 * sizeof(unsigned long long), ctx->stream));
     p.counters = ctx->d_small + SMALL_COUNTERS;
     p.nscat_hist = ctx->d_small + SMALL_HIST;
     p.spectrum = ctx->d_small + SMALL_SPEC;

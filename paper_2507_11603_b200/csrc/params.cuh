@@ -95,10 +95,10 @@ struct WalkParams {
     unsigned long long* pool_count;      // packets parked
     unsigned long long* pool_next;       // next slot to pop
     unsigned int* pool_order;            // [slots]: pool slots by decreasing scattering count (longest first)
-    // two-pass tail: the first walk launch parks a warp's packets into pool_mid once the counter is dry and at
-    // most half its lanes are live; a second launch of the walk kernel re-packs them into full warps and walks on
-    uint32_t* pool_mid;                  // nullptr = single pass
-    unsigned long long* pool_mid_count;
+    // the tail in passes: a walk launch parks a warp's packets into pool_mid once the counter is dry and at
+    // most half its lanes are live; the next launch of the walk kernel re-packs them into full warps and walks on
+    uint32_t* pool_mid;                  // two halves the passes alternate between; nullptr = single pass
+    unsigned long long* pool_mid_count;  // [2]
     // per launch of the walk kernel (set by the launcher):
     int resume;                          // 1: no photon counter; lanes start from the packets of resume_in
     const uint32_t* resume_in; const unsigned long long* resume_count;

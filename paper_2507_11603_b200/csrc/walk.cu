@@ -36,7 +36,11 @@ constexpr int REFILL_MIN_LANES = THOR_REFILL_MIN_LANES;
 #ifndef THOR_PARK1_LANES
 #define THOR_PARK1_LANES 16
 #endif
-constexpr int PARK1_LANES = THOR_PARK1_LANES;           // first pass of the tail: a warp parks at this many live lanes
+constexpr int PARK1_LANES = THOR_PARK1_LANES;           // every pass of the tail but the last: a warp parks at this many live lanes
+#ifndef THOR_TAIL_PASSES
+#define THOR_TAIL_PASSES 3
+#endif
+constexpr int TAIL_PASSES = THOR_TAIL_PASSES;           // launches of the walk kernel per run (1 feed + re-packed passes of the tail)
 constexpr int COOP_MAX_LANES = THOR_COOP_MAX_LANES;     // cooperative drain when a warp has at most this many packets left
 constexpr int WIN_STRIDE = 20;                          // floats per window slot (16 used; 80 B keeps STS.128 conflict-free)
 constexpr int PK_WORDS = 48;                            // 32-bit words of a parked packet
@@ -547,6 +551,9 @@ __global__ void __launch_bounds__(WALK_THREADS, MIN_CTAS) walk_kernel(const __gr
 // issue-bound, 4 CTAs (64 registers, 32 warps) when it does not and the walk needs more gathers in flight
 // (+18 % on the 512^3 gather workload, -6 % on the cache-resident sphere); 2 CTAs with peel-off (<= 128 registers).
 // The drain kernel follows on the same stream: a persistent grid of 4-warp CTAs whose warps pop parked packets.
+// Slots of ONE half of pool_mid (the packets a pass can park).
+long long walk_pool_mid_slots(int n_sm) { return (long long)n_sm * 4 * (WALK_THREADS / 32) * PARK1_LANES; }
+
 template <bool HUBBLE, bool PEEL, int MIN_CTAS, bool GL, bool DB, int FIN>
 static cudaError_t launch_pair(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {
     int per_sm = 0;
@@ -558,27 +565,33 @@ static cudaError_t launch_pair(const WalkParams& p, int n_sm, cudaStream_t strea
     const long long need = (long long)((p.n_photons + 31) / 32);   // few packets: spread the warps over the SMs
     if (need < blocks) blocks = need < 1 ? 1 : need;
     if (blocks_out) *blocks_out = (int)blocks;
-    // The tail in two passes: once the counter is dry a warp of the first launch parks its packets as soon as at
-    // most PARK1_LANES are live; a second launch of the same kernel re-packs them, 32 to a warp, and walks on until a warp is down
-    // to COOP_MAX_LANES packets, which go to the cooperative drain.  Half-empty warps cost what full ones do.
-    const bool two_pass = p.pool != nullptr && p.pool_mid != nullptr;
-    WalkParams p1 = p;
-    p1.resume = 0; p1.resume_in = nullptr; p1.resume_count = nullptr;
-    p1.park_out = two_pass ? p.pool_mid : p.pool;
-    p1.park_count = two_pass ? p.pool_mid_count : p.pool_count;
-    p1.park_lanes = two_pass ? PARK1_LANES : COOP_MAX_LANES;
-    walk<<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(p1);
-    e = cudaGetLastError();
-    if (e != cudaSuccess || !p.pool) return e;
-    if (two_pass) {
-        WalkParams p2 = p;
-        p2.resume = 1; p2.resume_in = p.pool_mid; p2.resume_count = p.pool_mid_count;
-        p2.park_out = p.pool; p2.park_count = p.pool_count; p2.park_lanes = COOP_MAX_LANES;
-        blocks = (blocks * PARK1_LANES + 31) / 32;            // 32 parked packets per warp cover everything the first pass can park
-        walk<<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(p2);
+    // The tail in passes: once the counter is dry a warp parks its packets as soon as at most PARK1_LANES are
+    // live; the next launch of the same kernel re-packs them, 32 to a warp, and walks on; the warps of the last pass park at
+    // COOP_MAX_LANES packets, which go to the cooperative drain.  Half-empty warps cost what full ones do, and every pass halves
+    // the packets that reach the drain kernel, where a scattering costs a whole warp.  The passes alternate between the two
+    // halves of pool_mid.
+    const int passes = (p.pool != nullptr && p.pool_mid != nullptr) ? TAIL_PASSES : 1;
+    const long long mid_slots = walk_pool_mid_slots(n_sm);
+    uint32_t* const mid[2] = {p.pool_mid, p.pool_mid ? p.pool_mid + mid_slots * PK_WORDS : nullptr};
+    for (int pass = 0; pass < passes; ++pass) {
+        const bool last = pass == passes - 1;
+        WalkParams q = p;
+        q.resume = pass > 0 ? 1 : 0;
+        q.resume_in = pass > 0 ? mid[(pass - 1) & 1] : nullptr;
+        q.resume_count = pass > 0 ? p.pool_mid_count + ((pass - 1) & 1) : nullptr;
+        q.park_out = last ? p.pool : mid[pass & 1];
+        q.park_count = last ? p.pool_count : p.pool_mid_count + (pass & 1);
+        q.park_lanes = last ? COOP_MAX_LANES : PARK1_LANES;
+        if (pass >= 2 && !last) {                             // a half of pool_mid is used again: its count restarts
+            e = cudaMemsetAsync(p.pool_mid_count + (pass & 1), 0, sizeof(unsigned long long), stream);
+            if (e != cudaSuccess) return e;
+        }
+        walk<<<(unsigned)blocks, WALK_THREADS, 0, stream>>>(q);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
+        if (!last) blocks = (blocks * PARK1_LANES + 31) / 32;  // 32 parked packets per warp cover everything this pass can park
     }
+    if (!p.pool) return cudaSuccess;
     const auto drain = drain_kernel<HUBBLE, PEEL, GL, DB, FIN>;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, drain, DRAIN_THREADS, 0);
     if (e != cudaSuccess) return e;
@@ -610,7 +623,7 @@ static cudaError_t launch_variant(const WalkParams& p, int n_sm, cudaStream_t st
 
 // Slots the pool must hold for a launch of `blocks` walk CTAs.
 long long walk_pool_slots(int n_sm) { return (long long)n_sm * 4 * (WALK_THREADS / 32) * COOP_MAX_LANES; }
-long long walk_pool_mid_slots(int n_sm) { return (long long)n_sm * 4 * (WALK_THREADS / 32) * PARK1_LANES; }
+
 int walk_pool_words() { return PK_WORDS; }
 
 cudaError_t launch_walk(const WalkParams& p, int n_sm, cudaStream_t stream, int* blocks_out) {

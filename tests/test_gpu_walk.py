@@ -599,7 +599,7 @@ def test_drain_kernel_is_bit_identical(thor):
              dict(W.cosmic_web(n=32, n_src=256, n_photons=3000, mean_n=1e-8, map_pix=16, v_max=40.0), tag="web")]
     for w in cases:
         w["opts"] = dict(w["opts"], max_scatter=20_000)
-        a = thor.run_workload(w, drain_mode=0)                # two-pass tail + drain kernel
+        a = thor.run_workload(w, drain_mode=0)                # the tail in passes + drain kernel
         b = thor.run_workload(w, drain_mode=1)                # the walk kernel alone
         c = thor.run_workload(w, drain_mode=2)                # single-pass tail + drain kernel
         assert a["raw"].tobytes() == c["raw"].tobytes() and a["counters"] == c["counters"], w["tag"]
