@@ -693,7 +693,7 @@ def main():
            "cell_crossings_per_sec": head["cell_crossings_per_sec"], "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "serial_ms_per_step": head["serial_ms_per_step"], "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": head["config"], "clocks": head.get("clocks"),
-           "gpu_launches": 3 * args.steps, "phases": head["phases"], "counters": head["counters"],
+           "gpu_launches": 5 * args.steps, "phases": head["phases"], "counters": head["counters"],
            "roofline": head["roofline"]}
     for k in ("roofline_hbm", "roofline_alu", "e2e"):
         if k in head:
@@ -707,7 +707,7 @@ def main():
             out["workloads"][name] = {k: r[k] for k in ("value", "unit", "packets_per_sec", "cell_crossings_per_sec", "steps",
                                                          "warmup", "ms_per_step", "serial_ms_per_step", "config", "phases", "roofline")}
             out["workloads"][name]["roofline_other"] = r.get("roofline_hbm") or r.get("roofline_alu")
-            out["gpu_launches"] += 3 * args.sub_steps
+            out["gpu_launches"] += 5 * args.sub_steps
     # ---- cpu_baseline: the oracle on a bounded sample, rank 0 at N = 1 only
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.workload, args.cpu_budget, max(1, args.ref_chunk))
