@@ -523,7 +523,9 @@ def measure_walk(args, name, steps, warmup, rank, local, world, n_photons=0, sam
                    "longest_packet_scatterings": [int(v) for v in max_nscat],
                    "drain_ns_per_scattering_of_longest_packet": float(np.mean([1e6 * (k - f) / max(1, m) for k, f, m in
                                                                                zip(kern_ms, feed_ms, max_nscat)])),
-                   "source": "device %globaltimer at kernel entry and when the photon counter is first found exhausted (thor_last_run_feed_ms)"},
+                   "source": "device %globaltimer at kernel entry and when the photon counter is first found exhausted (thor_last_run_feed_ms)",
+                   "note": ("launches of different steps overlap: a launch's span (launch_ms_per_step, and the drain figures derived from it) includes the time its kernels "
+                            "wait for SMs held by the other steps; serial_ms_per_step is the span of a step alone") if C > 1 else "one step at a time"},
         "counters": c,
     }
     if note:
